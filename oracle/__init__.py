@@ -1,0 +1,207 @@
+"""ctypes front-end of the CPU oracle (``ut_oracle.cpp``).  TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It shares nothing with
+``paper_2002_11529_b200`` (no code, headers, tables or helpers); both take their
+inputs from ``synth``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from dataclasses import dataclass
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "ut_oracle.cpp")
+_LIB = os.path.join(_DIR, "liboracle.so")
+_lib = None
+_lock = threading.Lock()
+
+ST_UNKNOWN_SECTOR, ST_DUPLICATE_SECTOR, ST_BAD_BANK_SIZE, ST_CAPACITY = 1, 2, 4, 8
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (no FMA contraction: DESIGN.md A14)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC",
+                               "-shared", _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Geometry(C.Structure):
+    _fields_ = [("n_layers", C.c_uint32), ("n_sectors", C.c_uint32), ("n_groups", C.c_uint32),
+                ("id_table_size", C.c_uint32),
+                ("id_to_sector", C.c_void_p), ("sector_raw_id", C.c_void_p), ("sector_group", C.c_void_p),
+                ("x0", C.c_void_p), ("pitch", C.c_void_p), ("dxdy", C.c_void_p), ("z", C.c_void_p),
+                ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
+                ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
+                ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4)]
+
+
+class _Hits(C.Structure):
+    _fields_ = [("x_at_y0", C.c_void_p), ("z_at_y0", C.c_void_p), ("y_begin", C.c_void_p),
+                ("y_end", C.c_void_p), ("dxdy", C.c_void_p), ("weight", C.c_void_p), ("id", C.c_void_p),
+                ("capacity", C.c_uint64)]
+
+
+class _Config(C.Structure):
+    _fields_ = [("win_half", C.c_float * 4), ("y_tol", C.c_float), ("max_slope", C.c_float),
+                ("kink_tol", C.c_float), ("seed_tol", C.c_float), ("w_velo", C.c_float),
+                ("max_chi2_ndf", C.c_float), ("kappa", C.c_float), ("z_mag", C.c_float),
+                ("min_hits", C.c_int32), ("max_candidates_per_layer", C.c_int32)]
+
+
+def _load():
+    global _lib
+    with _lock:
+        if _lib is None:
+            build()
+            lib = C.CDLL(_LIB)
+            lib.oracle_decode.restype = C.c_int32
+            lib.oracle_compass.restype = C.c_int32
+            lib.oracle_fit.restype = C.c_int32
+            _lib = lib
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _geom_struct(geom):
+    keep = [np.ascontiguousarray(getattr(geom, n)) for n in
+            ("id_to_sector", "sector_raw_id", "sector_group", "x0", "pitch", "dxdy", "z", "y_begin", "y_end",
+             "weight", "group_xmin", "group_xmax")]
+    s = _Geometry(geom.n_layers, geom.n_sectors, geom.n_groups, geom.id_table_size, *[_p(a) for a in keep])
+    s.layer_z[:] = [float(v) for v in geom.layer_z]
+    s.layer_dxdy[:] = [float(v) for v in geom.layer_dxdy]
+    return s, keep
+
+
+def _config_struct(p):
+    c = _Config()
+    c.win_half[:] = list(p.win_half)
+    for n in ("y_tol", "max_slope", "kink_tol", "seed_tol", "w_velo", "max_chi2_ndf", "kappa", "z_mag",
+              "min_hits", "max_candidates_per_layer"):
+        setattr(c, n, getattr(p, n))
+    return c
+
+
+@dataclass
+class Hits:
+    x_at_y0: np.ndarray
+    z_at_y0: np.ndarray
+    y_begin: np.ndarray
+    y_end: np.ndarray
+    dxdy: np.ndarray
+    weight: np.ndarray
+    id: np.ndarray
+    hit_offsets: np.ndarray      # u32 [n_events*n_groups + 1]
+    status: int
+    n_hits: int
+
+    FIELDS = ("x_at_y0", "z_at_y0", "y_begin", "y_end", "dxdy", "weight", "id")
+
+    def _struct(self):
+        return _Hits(*[_p(getattr(self, f)) for f in self.FIELDS], C.c_uint64(self.x_at_y0.shape[0]))
+
+
+@dataclass
+class Tracks:
+    hit_idx: np.ndarray          # i32 [4, T]
+    n_hits: np.ndarray           # i32 [T]
+    qop: np.ndarray              # f32 [T]
+    chi2: np.ndarray             # f32 [T]
+    runner_chi2: np.ndarray      # f32 [T]  2nd-best chi2 among valid tracklets with the same n (inf if none)
+    cand_n: np.ndarray           # i32 [T, 4] candidates per layer before the cap
+    cand_list: np.ndarray        # i32 [T, 4, C] post-cap candidate hit indices (-1 pad)
+    n_fits: np.ndarray           # i32 [T]
+
+
+def decode(raw: np.ndarray, bank_offsets: np.ndarray, n_events: int, geom, capacity: int | None = None) -> Hits:
+    """PAPER.md section IV as the plain definition."""
+    lib = _load()
+    raw = np.ascontiguousarray(raw, dtype=np.uint8)
+    bank_offsets = np.ascontiguousarray(bank_offsets, dtype=np.uint32)
+    if capacity is None:
+        capacity = max((int(raw.size) - 6 * n_events * geom.n_sectors) // 2, 0)
+    f = lambda: np.zeros(capacity, np.float32)
+    h = Hits(f(), f(), f(), f(), f(), f(), np.zeros(capacity, np.uint32),
+             np.zeros(n_events * geom.n_groups + 1, np.uint32), 0, 0)
+    gs, keep = _geom_struct(geom)
+    hs = h._struct()
+    st = C.c_uint32(0)
+    rc = lib.oracle_decode(_p(raw), _p(bank_offsets), C.c_int32(n_events), C.byref(gs), C.byref(hs),
+                           _p(h.hit_offsets), C.byref(st))
+    if rc != 0:
+        raise RuntimeError(f"oracle_decode rc={rc}")
+    h.status = int(st.value)
+    h.n_hits = int(h.hit_offsets[-1])
+    return h
+
+
+def compass(hits: Hits, velo_x, velo_y, velo_tx, velo_ty, velo_z: float, velo_offsets, n_events: int, geom,
+            params, mode: int = 0, event_range: tuple | None = None) -> Tracks:
+    """PAPER.md section V step by step.  mode 0 windowed, 1 linear-scan candidates (BF-1),
+    2 exhaustive combinations without cap (BF-2)."""
+    lib = _load()
+    T = int(velo_offsets[n_events])
+    Cc = int(params.max_candidates_per_layer)
+    out = Tracks(np.full((4, T), -1, np.int32), np.zeros(T, np.int32), np.zeros(T, np.float32),
+                 np.zeros(T, np.float32), np.full(T, np.inf, np.float32), np.zeros((T, 4), np.int32),
+                 np.full((T, 4, Cc), -1, np.int32), np.zeros(T, np.int32))
+    compass_into(out, hits, velo_x, velo_y, velo_tx, velo_ty, velo_z, velo_offsets, n_events, geom, params, mode)
+    return out
+
+
+def compass_into(out: Tracks, hits: Hits, velo_x, velo_y, velo_tx, velo_ty, velo_z, velo_offsets, n_events,
+                 geom, params, mode=0, first_event=0, n_sub=None, extras=True):
+    """Run events [first_event, first_event+n_sub) writing into ``out`` (disjoint event chunks may run in
+    different threads: ctypes releases the GIL)."""
+    lib = _load()
+    n_sub = n_events - first_event if n_sub is None else n_sub
+    velo_offsets = np.ascontiguousarray(velo_offsets, dtype=np.uint32)
+    gs, keep = _geom_struct(geom)
+    cs = _config_struct(params)
+    hs = hits._struct()
+    vo = velo_offsets[first_event:]
+    ho = hits.hit_offsets[first_event * geom.n_groups:]
+    T = out.n_hits.shape[0]
+    # outputs are indexed by global track id; hit_idx rows have stride T, so pass the base pointers
+    rc = lib.oracle_compass(
+        C.c_int32(mode), C.byref(hs), _p(ho), _p(np.ascontiguousarray(velo_x, np.float32)),
+        _p(np.ascontiguousarray(velo_y, np.float32)), _p(np.ascontiguousarray(velo_tx, np.float32)),
+        _p(np.ascontiguousarray(velo_ty, np.float32)), C.c_float(velo_z), _p(vo), C.c_int32(n_sub),
+        C.byref(gs), C.byref(cs), _p(out.hit_idx), _p(out.n_hits), _p(out.qop), _p(out.chi2),
+        _p(out.runner_chi2) if extras else None, _p(out.cand_n) if extras else None,
+        _p(out.cand_list) if extras and mode != 2 else None, _p(out.n_fits) if extras else None,
+        C.c_int64(T))
+    if rc != 0:
+        raise RuntimeError(f"oracle_compass rc={rc}")
+
+
+def fit(d, z, w, params):
+    """Step 6 alone: returns (a, b, chi2, qop) as float32 scalars."""
+    lib = _load()
+    d, z, w = (np.ascontiguousarray(v, np.float32) for v in (d, z, w))
+    cs = _config_struct(params)
+    a, b, c2, q = C.c_float(), C.c_float(), C.c_float(), C.c_float()
+    rc = lib.oracle_fit(C.c_int32(len(d)), _p(d), _p(z), _p(w), C.byref(cs), C.byref(a), C.byref(b),
+                        C.byref(c2), C.byref(q))
+    if rc != 0:
+        raise RuntimeError(f"oracle_fit rc={rc}")
+    return np.float32(a.value), np.float32(b.value), np.float32(c2.value), np.float32(q.value)
+
+
+def run_batch(batch, geom, params, mode: int = 0):
+    """Decode + Compass on a synth.Batch; returns (Hits, Tracks)."""
+    h = decode(batch.raw, batch.bank_offsets, batch.n_events, geom, batch.hit_capacity)
+    t = compass(h, batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z, batch.velo_offsets,
+                batch.n_events, geom, params, mode)
+    return h, t
