@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py -- UT decode + Compass events/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A step = one pass of the whole hot path (ut_decode + compass_track) over one
+synthetic batch (config 3: 1000 events, ~2000 hits and ~150 VELO tracks each, seed 3; rank r of N takes
+events [r*1000, (r+1)*1000) of the same stream: weak scaling, no collective on the data path).
+Timing: CUDA events on the launching stream around every step, L2 flushed (256 MiB memset) between
+steps, barrier + synchronize on both sides of the timed region, max over ranks.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ut_decode_compass_events_per_s"
+UNIT = "events/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 is the metric's workload")
+    ap.add_argument("--events", type=int, default=None, help="override the number of events per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config 5: all 18 settings with efficiency / ghost rate")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------
+# algorithmic bytes per launch: what the method must move once
+# ---------------------------------------------------------------------------------------------------
+def algorithmic_bytes(batch, geom, n_hits):
+    ne, T = batch.n_events, batch.n_velo_total
+    decode = batch.raw.size + 4 * (ne * geom.n_sectors + 1) + 28 * n_hits + 4 * (ne * geom.n_groups + 1)
+    compass = 24 * n_hits + 4 * (ne * geom.n_groups + 1) + 4 * (ne + 1) + 16 * T + 28 * T
+    e2e = decode + 4 * (ne + 1) + 16 * T + 28 * T
+    return dict(decode=int(decode), compass=int(compass), e2e=int(e2e))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the GPU is under load (B200_PROFILING.md recipe)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "50", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+        self.marks = []
+
+    def mark(self):
+        self.marks.append(time.time())
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=2)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = []
+        for line in open(self.f.name):
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) >= 9:
+                try:
+                    ts = time.mktime(time.strptime(parts[0].split(".")[0], "%Y/%m/%d %H:%M:%S")) + \
+                        float("0." + parts[0].split(".")[1]) if "." in parts[0] else 0.0
+                    rows.append((ts, float(parts[1]), float(parts[2]), parts[3], parts[5:9]))
+                except ValueError:
+                    pass
+        os.unlink(self.f.name)
+        lo, hi = (self.marks + [0, 0])[:2] if len(self.marks) >= 2 else (0, 1e18)
+        sel = [r for r in rows if lo - 0.05 <= r[0] <= hi + 0.05] or rows
+        if not sel:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in sel for i, v in enumerate(r[4]) if v.lower().startswith("active")})
+        return {"sm_mhz": statistics.median(r[1] for r in sel), "sm_max_mhz": sel[0][2], "reasons": reasons,
+                "samples": len(sel)}
+
+
+def oracle_chunked(batch, geom, params, lo, hi, threads):
+    """The oracle, as it stands, over disjoint event chunks on `threads` host threads (ctypes drops the GIL)."""
+    import oracle
+    cuts = np.linspace(lo, hi, threads + 1).astype(int)
+    ns, ng = geom.n_sectors, geom.n_groups
+
+    def work(a, b):
+        if b <= a:
+            return
+        bo = batch.bank_offsets[a * ns:b * ns + 1]
+        cap = (int(bo[-1]) - int(bo[0]) - 6 * (b - a) * ns) // 2
+        h = oracle.decode(batch.raw, bo, b - a, geom, cap)
+        vo = batch.velo_offsets[a:b + 1]
+        T = int(vo[-1]) - int(vo[0])
+        out = oracle.Tracks(np.full((4, T), -1, np.int32), np.zeros(T, np.int32), np.zeros(T, np.float32),
+                            np.zeros(T, np.float32), None, None, None, None)
+        v0 = int(vo[0])
+        sl = slice(v0, v0 + T)
+        oracle.compass_into(out, h, batch.velo_x[sl], batch.velo_y[sl], batch.velo_tx[sl], batch.velo_ty[sl],
+                            batch.velo_z, (vo - vo[0]).astype(np.uint32), b - a, geom, params, 0, extras=False)
+
+    ts = [threading.Thread(target=work, args=(int(a), int(b))) for a, b in zip(cuts[:-1], cuts[1:])]
+    t0 = time.perf_counter()
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(batch, geom, params, budget_s=4.0):
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    n = batch.n_events
+    oracle_chunked(batch, geom, params, 0, min(n, 4 * cores), cores)      # warm the library
+    reps, total = 0, 0.0
+    while total < budget_s and reps < 50:
+        total += oracle_chunked(batch, geom, params, 0, n, cores)
+        reps += 1
+    return {"value": n * reps / total, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"all {n} events of the workload x {reps} passes, oracle decode+compass on {cores} threads "
+                      f"over disjoint event chunks ({total:.1f} s wall)"}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle on the host cores, same metric / config."""
+    if rank != 0:
+        return
+    import synth
+    cfg = synth.CONFIGS[args.config]
+    cores = os.cpu_count() or 1
+    n = min(args.events or cfg.n_events, 250)        # bounded sample per step
+    geom, batch, params = synth.make_workload(args.config, n_events=n, workers=min(8, cores))
+    import oracle
+    oracle.build()
+    for _ in range(max(args.warmup, 1)):
+        oracle_chunked(batch, geom, params, 0, min(n, 4 * cores), cores)
+    t = 0.0
+    for _ in range(args.steps):
+        t += oracle_chunked(batch, geom, params, 0, n, cores)
+    value = n * args.steps / t
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "impl": "reference",
+            "config": {"workload": cfg.name, "events_per_step": n, "note": "CPU oracle (oracle/ut_oracle.cpp), "
+                       f"bounded sample of {n} events per step on {cores} host threads"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"first {n} events of {cfg.name} per step"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import synth
+    cfg = synth.CONFIGS[args.config]
+    n_events = args.events or cfg.n_events
+    # generate before CUDA is initialised (the generator may fork workers)
+    geom_t, batch, params = synth.make_workload(args.config, n_events=n_events, workers=min(8, os.cpu_count() or 1),
+                                                first_event=rank * n_events)
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as entry
+    if rank == 0:
+        entry.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    torch.cuda.set_device(local_rank)
+    from paper_2002_11529_b200 import binding as B
+    dev = torch.device("cuda", local_rank)
+
+    geom = B.ut_geometry_upload(geom_t)
+    hits = B.Hits(batch.hit_capacity, batch.n_events, geom)
+    raw_d, bo_d = B.to_device_raw(batch.raw), B.to_device_u32(batch.bank_offsets)
+    velo = B.VeloStates(batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z)
+    vo_d = B.to_device_u32(batch.velo_offsets)
+    tracks = B.Tracks(batch.n_velo_total)
+    config = B.make_config(params)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
+        B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
+
+    step()
+    torch.cuda.synchronize()
+    launches_per_step = 2
+    info = B.last_launch_info()
+    n_hits = int(hits.hit_offsets[batch.n_events * geom.n_groups].item()) & 0xFFFFFFFF
+    status = (int(hits.status.item()) | int(tracks.status.item())) & 0xFFFFFFFF
+    abytes = algorithmic_bytes(batch, geom_t, n_hits)
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    if sampler:
+        sampler.mark()
+    torch.cuda.synchronize()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.zero_()
+        ev[k][0].record(stream)
+        B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
+        ev[k][1].record(stream)
+        B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
+        ev[k][2].record(stream)
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    if sampler:
+        sampler.mark()
+    if world > 1:
+        dist.barrier()
+    t_dec = [e[0].elapsed_time(e[1]) for e in ev]
+    t_cmp = [e[1].elapsed_time(e[2]) for e in ev]
+    t_step = [e[0].elapsed_time(e[2]) for e in ev]
+    total_ms = float(sum(t_step))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        ne = torch.tensor([batch.n_events], dtype=torch.float64, device=dev)
+        dist.all_reduce(ne, op=dist.ReduceOp.SUM)
+        events_all = float(ne.item())
+    else:
+        events_all = float(batch.n_events)
+    clocks = sampler.stop() if sampler else None
+
+    # ---- end to end through the host-buffer C-ABI call (H2D + kernels + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        T = batch.n_velo_total
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        raw_h = pin(np.concatenate([batch.raw, np.zeros(32, np.uint8)]))
+        bo_h, vo_h = pin(batch.bank_offsets.view(np.int32)), pin(batch.velo_offsets.view(np.int32))
+        velo_h = [pin(v) for v in (batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty)]
+        out_h = {"hit_idx": torch.empty(4 * max(T, 1), dtype=torch.int32).pin_memory(),
+                 "n_hits": torch.empty(max(T, 1), dtype=torch.int32).pin_memory(),
+                 "qop": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
+                 "chi2": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
+                 "status": torch.zeros(2, dtype=torch.int32).pin_memory(),
+                 "n_hits_total": torch.zeros(1, dtype=torch.int32).pin_memory()}
+        pipe = B.Pipeline(geom, batch.n_events, int(batch.raw.size) + 32, batch.hit_capacity, max(T, 1))
+        run = lambda: pipe.run_host(raw_h, int(batch.raw.size), bo_h, velo_h, batch.velo_z, vo_h, T, batch.n_events,
+                                    config, out_h)
+        for _ in range(3):
+            run()
+        torch.cuda.synchronize()
+        k_e2e = max(10, min(args.steps, 100))
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            flush.zero_()
+            run()
+            torch.cuda.synchronize()       # the step's result is on the host before the next one starts
+        t_e2e = time.perf_counter() - t0
+        t_flush0 = time.perf_counter()
+        for _ in range(k_e2e):
+            flush.zero_()
+            torch.cuda.synchronize()
+        t_e2e -= time.perf_counter() - t_flush0          # the flush is not part of the step
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        h2d = int(batch.raw.size) + 4 * (batch.bank_offsets.size + batch.velo_offsets.size) + 16 * T
+        e2e = {"value": events_all * k_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": 28 * T + 12, "steps": k_e2e,
+               "api": "ut_pipeline_run_host (pinned host buffers in, host track SoA out, sync per step)"}
+        ok = np.array_equal(out_h["n_hits"][:T].numpy(), tracks.n_hits[:T].cpu().numpy())
+        e2e["matches_device_path"] = bool(ok)
+        pipe.destroy()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "MEASURED_PEAKS.json hbm_gbs (measured copy)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    md, mc, ms = statistics.mean(t_dec), statistics.mean(t_cmp), statistics.mean(t_step)
+    kern = {
+        "ut_decode_kernel": {"ms": md, "bytes": abytes["decode"], "gbs": abytes["decode"] / md / 1e6,
+                             "frac_hbm": abytes["decode"] / md / 1e6 / hbm_peak,
+                             "events_per_s": batch.n_events / md * 1e3},
+        "compass_kernel": {"ms": mc, "bytes": abytes["compass"], "gbs": abytes["compass"] / mc / 1e6,
+                           "frac_hbm": abytes["compass"] / mc / 1e6 / hbm_peak,
+                           "events_per_s": batch.n_events / mc * 1e3},
+    }
+    dom = "ut_decode_kernel" if md >= mc else "compass_kernel"
+    roof = {"kernel": dom, "bound": "hbm", "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
+            "frac": kern[dom]["frac_hbm"], "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": kern[dom]["bytes"],
+            "end_to_end": {"bytes": abytes["e2e"], "gbs": abytes["e2e"] / ms / 1e6,
+                           "frac": abytes["e2e"] / ms / 1e6 / hbm_peak, "frac_of_8TBs": abytes["e2e"] / ms / 1e6 / 8000.0}}
+    line = {
+        "metric": METRIC, "value": events_all * args.steps / (total_ms * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "events_per_gpu": batch.n_events, "hits": n_hits,
+                   "velo_tracks": batch.n_velo_total, "min_hits": params.min_hits,
+                   "max_candidates_per_layer": params.max_candidates_per_layer, "p_min_gev": cfg.p_min_gev,
+                   "window_scale": cfg.window_scale, "l2": "flushed (256 MiB memset) between timed steps",
+                   "timing": "cuda events per step on the launch stream, sum over steps, max over ranks",
+                   "status_word": status, "launch": info},
+        "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "e2e": e2e,
+        "roofline": roof, "kernels": kern,
+        "median_ms": {"decode": statistics.median(t_dec), "compass": statistics.median(t_cmp),
+                      "step": statistics.median(t_step), "step_min": min(t_step)},
+        "wall_events_per_s_incl_flush": batch.n_events * args.steps / t_wall,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(batch, geom_t, params)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

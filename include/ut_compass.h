@@ -1,0 +1,198 @@
+/* ut_compass.h -- C ABI of libutcompass: UT raw-bank decoding and Compass tracking on one B200.
+ *
+ * The two hot-path calls follow the problem statement of arxiv/paper_2002_11529
+ * ("A parallel-computing algorithm for high-energy physics particle tracking and decoding
+ * using GPU architectures"; citations are lines of the paper text, PAPER.md):
+ *
+ *   ut_decode      section IV: UT raw banks -> SoA hit container
+ *                  {LHCbID, zAtYEq0, xAtYEq0, yBegin, yEnd, weight} (+ dxdy) grouped into sector
+ *                  groups and sorted inside each group, plus the offsets array.
+ *   compass_track  section V: every VELO track is extrapolated to the four UT
+ *                  layers, window hits are collected per layer, 3/4-hit tracklets are enumerated from
+ *                  seed pairs, fitted (chi2, q/p) and the best one is kept.
+ *
+ * Conventions
+ *   - Plain C, no CUDA or torch types.  `ut_stream_t` is a cudaStream_t / CUstream handle (0 = default).
+ *   - Unless a comment says HOST, every data pointer is a DEVICE pointer owned by the caller; the
+ *     library never frees or reallocates it.  The descriptor structs themselves live in HOST memory.
+ *   - Hot-path calls are asynchronous on `stream`, perform no host synchronisation and no allocation,
+ *     and are CUDA-graph capturable.
+ *   - Return value: 0 = launched; < 0 = invalid argument detected on the host (UT_ERR_*).
+ *     Data-dependent errors set bits in the device `status` word of the output struct (UT_STATUS_*);
+ *     kernels never write past `capacity`.
+ *   - Arithmetic: IEEE fp32, round-to-nearest, no FMA contraction, operations in the order written
+ *     in DESIGN.md section 3, so results are bit-identical to the reference definition.
+ */
+#ifndef UT_COMPASS_H
+#define UT_COMPASS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef void* ut_stream_t;
+
+#define UT_N_LAYERS 4
+
+/* host-detected errors */
+#define UT_OK 0
+#define UT_ERR_NULL (-1)        /* required pointer is null */
+#define UT_ERR_ARG (-2)         /* negative size, bad config value, misaligned buffer */
+#define UT_ERR_GEOMETRY (-3)    /* geometry table violates the container contract */
+#define UT_ERR_CUDA (-4)        /* CUDA runtime error (allocation, launch) */
+#define UT_ERR_LIMIT (-5)       /* table larger than the compiled limits (UT_MAX_*) */
+
+/* data-dependent status bits (device word) */
+#define UT_STATUS_UNKNOWN_SECTOR 1u    /* raw sector id not in id_to_sector            (bank ignored)   */
+#define UT_STATUS_DUPLICATE_SECTOR 2u  /* two banks of one event name the same sector  (one ignored)    */
+#define UT_STATUS_BAD_BANK_SIZE 4u     /* bank bytes != round4(6 + 2*count) or misaligned (bank ignored) */
+#define UT_STATUS_CAPACITY 8u          /* hits would exceed `capacity`; that event's hits are not written */
+#define UT_STATUS_BAD_OFFSETS 16u      /* compass_track: offsets not monotone / inconsistent            */
+#define UT_STATUS_EVENT_TOO_LARGE 32u  /* compass_track: > 65535 hits in one layer of one event; no tracks */
+
+#define UT_MAX_SECTORS 1024
+#define UT_MAX_GROUPS 128
+#define UT_MAX_CANDIDATES 32
+
+/* Geometry tables (stand-in for the detector conditions of PAPER.md:231, :274).
+ * Dense sector index s in [0, n_sectors): the sectors of one group are contiguous and groups are
+ * numbered layer-major, so `sector_group` is non-decreasing; group g belongs to layer
+ * g / (n_groups / n_layers).  A sector group is a region of unique X.
+ * Contract checked by ut_geometry_upload: n_layers == 4; n_groups % 4 == 0; every group non-empty;
+ * dxdy constant inside a group; group_xmin and group_xmax non-decreasing inside a layer;
+ * pitch > 0; every x a sector can produce lies in [group_xmin, group_xmax] of its group. */
+typedef struct {
+  uint32_t n_layers, n_sectors, n_groups;
+  uint32_t id_table_size;
+  const uint32_t* id_to_sector;   /* [id_table_size] raw id -> dense s, 0xFFFFFFFF = invalid */
+  const uint32_t* sector_raw_id;  /* [n_sectors] */
+  const uint32_t* sector_group;   /* [n_sectors] */
+  const float *x0, *pitch, *dxdy, *z, *y_begin, *y_end, *weight; /* [n_sectors] */
+  const float *group_xmin, *group_xmax;                          /* [n_groups] bounds of xAtYEq0 */
+  float layer_z[UT_N_LAYERS], layer_dxdy[UT_N_LAYERS];           /* HOST values inside the struct */
+  /* filled by ut_geometry_upload (device, library-owned until ut_geometry_free) */
+  const uint32_t* group_first_sector; /* [n_groups + 1] */
+  const float* group_inv_span;        /* [n_groups] 1 / (group_xmax - group_xmin) */
+  void* owner;                        /* opaque allocation handle, NULL for caller-owned tables */
+} ut_geometry;
+
+/* Copies HOST tables (`host_tables` holds HOST pointers in the array fields) to the device, checks
+ * the contract above and fills `device_out` with device pointers.  Synchronous; call once at set-up. */
+int32_t ut_geometry_upload(const ut_geometry* host_tables, ut_geometry* device_out);
+int32_t ut_geometry_free(ut_geometry* device_geometry);
+
+/* SoA hit container.  All arrays have `capacity` elements.
+ * Order: events ascending; inside an event sector groups ascending; inside a group ascending
+ * x_at_y0, ties in fill order (dense sector, then word order in the bank).
+ *   x_at_y0 = x0[s] + ((2*strip + frac)*0.5f + 0.25f) * pitch[s]     (fp32, two roundings)
+ *   z_at_y0, y_begin, y_end, dxdy, weight = the sector's table row;  id = (raw_id << 9) | strip. */
+typedef struct {
+  float *x_at_y0, *z_at_y0, *y_begin, *y_end, *dxdy, *weight;
+  uint32_t* id;
+  uint64_t capacity;          /* (total_raw_bytes - 6*n_banks)/2 is always enough */
+  const ut_geometry* geom;    /* HOST pointer to the device-table descriptor used to decode */
+  uint32_t* status;           /* device word, OR-ed with UT_STATUS_* (caller zeroes it) */
+  void* workspace;            /* device, ut_decode_workspace_bytes() bytes, zeroed once by
+                                 ut_decode_workspace_init(); reusable across calls on one stream */
+} ut_hits;
+
+size_t ut_decode_workspace_bytes(int32_t max_events);
+int32_t ut_decode_workspace_init(void* workspace, int32_t max_events, ut_stream_t stream);
+
+/* ut_decode -- PAPER.md section IV.
+ * raw_banks    : device bytes, 16-byte aligned, readable up to the next multiple of 16 past the end.
+ *                Bank = u32 raw sector id | u16 count | count x u16 word | zero pad to 4 bytes;
+ *                word = 9-bit strip | frac << 9 | ADC << 10 (ADC ignored).  Little endian.
+ * bank_offsets : device u32 [n_events*n_sectors + 1], 16-byte aligned: byte offset of every bank and the
+ *                end; the banks of an event are contiguous, one per sector, in any order.
+ * hit_offsets_out : device u32 [n_events*n_groups + 1]: global exclusive prefix of group sizes; event e
+ *                owns hits [off[n_groups*e], off[n_groups*(e+1)]).  Always exact, even on CAPACITY.
+ * One kernel launch: per-sector count -> event total -> chained exclusive prefix over events
+ * (decoupled look-back, no host sync; the paper reads the total back) -> bucketed fill
+ * -> stable in-group ordering -> coalesced SoA store. */
+int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_t n_events,
+                  const ut_geometry* geometry, ut_hits* hits_out, uint32_t* hit_offsets_out,
+                  ut_stream_t stream);
+
+/* VELO states: straight lines x(z) = x + tx*(z - z0), same for y, SoA. */
+typedef struct {
+  const float *x, *y, *tx, *ty; /* [n_velo_total] */
+  float z;                      /* z0 of all states (770 mm in the synthetic workloads) */
+} velo_states;
+
+/* Compass configuration.  Derived fields are computed on the host once (double, rounded once).
+ * The paper's two knobs -- sectors searched {1,3,5} and hit candidates {1..16} --
+ * appear as the window half-widths and max_candidates_per_layer (readings A6, A7). */
+typedef struct {
+  float win_half[UT_N_LAYERS]; /* |d| <= win_half[l] selects window hits of layer l [mm] */
+  float y_tol;                 /* y_begin - y_tol <= y_e <= y_end + y_tol [mm] */
+  float max_slope;             /* |seed slope in residual space| limit */
+  float kink_tol;              /* |seed-line intercept at z_mag| limit [mm] */
+  float seed_tol;              /* |residual to the seed line| limit in the other two layers [mm] */
+  float w_velo;                /* weight of the VELO pseudo-point (dz = 0, d = 0) in the fit */
+  float max_chi2_ndf;          /* valid iff chi2 <= max_chi2_ndf * (n_hits - 1) */
+  float kappa;                 /* q/p = slope / kappa  [MeV] */
+  float z_mag;                 /* kick plane [mm] */
+  int32_t min_hits;            /* 3 or 4 */
+  int32_t max_candidates_per_layer; /* 1 .. UT_MAX_CANDIDATES, closest-first in |d| */
+} compass_config;
+
+/* win_half[l] = window_scale * (kappa/p_min_mev) * (layer_z[l] - z_mag) + 0.5,
+ * max_slope = window_scale * kappa / p_min_mev + 0.0015, other fields DESIGN.md A8 defaults. */
+int32_t compass_config_default(float p_min_mev, float window_scale, int32_t min_hits,
+                               int32_t max_candidates_per_layer, const ut_geometry* geometry,
+                               compass_config* out /* HOST */);
+
+/* Track output: dense, one slot per VELO track (PAPER.md:348 without the atomicAdd; A13). */
+typedef struct {
+  int32_t* hit_idx;  /* [4][n_velo_total], row l = global hit index in layer l or -1 */
+  int32_t* n_hits;   /* [n_velo_total] 0 (no tracklet), 3 or 4 */
+  float* qop;        /* [n_velo_total] q/p in 1/MeV, sign = charge; 0 if none */
+  float* chi2;       /* [n_velo_total] 0 if none */
+  uint32_t* status;  /* device word */
+} ut_tracks;
+
+/* compass_track -- PAPER.md section V, fused (window search + tracklet finding in one kernel; the
+ * paper's CPU port does the same).
+ * hits, hit_offsets : as produced by ut_decode (hits->geom gives the group tables).
+ * velo_offsets      : device u32 [n_events + 1]; n_velo_total = velo_offsets[n_events] (read on device). */
+int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                      const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                      ut_tracks* tracks_out, ut_stream_t stream);
+
+/* End-to-end convenience for HOST buffers (bench.py "e2e"): H2D of raw banks, offsets and VELO
+ * states, ut_decode, compass_track, D2H of the track SoA, all asynchronous on `stream`.
+ * The arena holds the device staging buffers (library-owned). Host buffers should be pinned. */
+typedef struct ut_pipeline ut_pipeline;
+int32_t ut_pipeline_create(const ut_geometry* device_geometry, int32_t max_events, size_t max_raw_bytes,
+                           uint64_t max_hits, uint32_t max_velo, ut_pipeline** out);
+int32_t ut_pipeline_destroy(ut_pipeline* p);
+/* All pointers HOST.  tracks_host receives hit_idx/n_hits/qop/chi2; *status_host the OR of both status
+ * words; *n_hits_host the total decoded hits.  Returns after enqueueing; sync the stream to read. */
+int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_banks_host, size_t raw_bytes,
+                             const uint32_t* bank_offsets_host, const velo_states* velo_host,
+                             const uint32_t* velo_offsets_host, uint32_t n_velo_total, int32_t n_events,
+                             const compass_config* config, ut_tracks* tracks_host, uint32_t* status_host,
+                             uint32_t* n_hits_host, ut_stream_t stream);
+/* Device views of the arena (valid after a run): decoded hits and offsets, for inspection. */
+int32_t ut_pipeline_device_hits(ut_pipeline* p, ut_hits* hits_out, const uint32_t** hit_offsets_out);
+
+/* Launch statistics of the most recent call on this thread (host side, no sync). */
+typedef struct {
+  int32_t kernels_launched;     /* kernels enqueued by the last hot-path call */
+  int32_t decode_grid, decode_block, decode_smem_bytes, decode_buckets_per_group, decode_hit_stage;
+  int32_t compass_grid, compass_block, compass_smem_bytes, compass_hit_stage;
+} ut_launch_info;
+void ut_last_launch_info(ut_launch_info* out);
+
+const char* ut_version(void);
+/* Text of the last UT_ERR_CUDA on this thread ("<call>: <cuda error string>"), "" if none. */
+const char* ut_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UT_COMPASS_H */

@@ -1,0 +1,299 @@
+// api.cu -- the extern "C" surface of libutcompass (include/ut_compass.h): argument checks on the
+// host, geometry upload, workspace, the two hot-path launches and the host-buffer pipeline.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace utc {
+int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
+                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream);
+int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                       const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
+                       cudaStream_t stream);
+
+ut_launch_info& launch_info() {
+  static thread_local ut_launch_info info = {};
+  return info;
+}
+
+static thread_local char g_last_error[256] = "";
+int32_t cuda_fail(const char* what, cudaError_t err) {
+  snprintf(g_last_error, sizeof(g_last_error), "%s: %s", what, cudaGetErrorString(err));
+  return UT_ERR_CUDA;
+}
+
+struct GeomOwner {
+  void* block = nullptr;     // one device allocation holding every table
+};
+
+static bool geometry_ok(const ut_geometry* g) {
+  return g && g->n_layers == UT_N_LAYERS && g->n_groups >= 4 && g->n_groups % 4 == 0 && g->n_sectors >= g->n_groups &&
+         g->id_to_sector && g->sector_raw_id && g->sector_group && g->x0 && g->pitch && g->dxdy && g->z &&
+         g->y_begin && g->y_end && g->weight && g->group_xmin && g->group_xmax;
+}
+}  // namespace utc
+
+using namespace utc;
+
+extern "C" {
+
+const char* ut_version(void) { return "ut-compass-b200 0.1 (sm_100a)"; }
+
+const char* ut_last_error(void) { return g_last_error; }
+
+void ut_last_launch_info(ut_launch_info* out) {
+  if (out) *out = launch_info();
+}
+
+int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
+  if (!h || !out) return UT_ERR_NULL;
+  if (!geometry_ok(h)) return UT_ERR_GEOMETRY;
+  const uint32_t ns = h->n_sectors, ng = h->n_groups, gpl = ng / UT_N_LAYERS;
+  if (ns > UT_MAX_SECTORS || ng > UT_MAX_GROUPS || h->id_table_size == 0) return UT_ERR_LIMIT;
+  // ---- container contract (include/ut_compass.h) ----
+  std::vector<uint32_t> first(ng + 1, 0);
+  std::vector<float> inv(ng);
+  {
+    uint32_t prev = 0;
+    std::vector<uint32_t> cnt(ng, 0);
+    for (uint32_t s = 0; s < ns; ++s) {
+      const uint32_t g = h->sector_group[s];
+      if (g >= ng || g < prev) return UT_ERR_GEOMETRY;
+      prev = g;
+      ++cnt[g];
+      if (!(h->pitch[s] > 0.f) || h->sector_raw_id[s] >= h->id_table_size) return UT_ERR_GEOMETRY;
+      if (h->id_to_sector[h->sector_raw_id[s]] != s) return UT_ERR_GEOMETRY;
+    }
+    for (uint32_t g = 0; g < ng; ++g) {
+      if (cnt[g] == 0) return UT_ERR_GEOMETRY;
+      first[g + 1] = first[g] + cnt[g];
+      for (uint32_t s = first[g]; s < first[g + 1]; ++s)
+        if (h->dxdy[s] != h->dxdy[first[g]]) return UT_ERR_GEOMETRY;      // one stereo angle per group
+      const float span = h->group_xmax[g] - h->group_xmin[g];
+      if (!(span > 0.f)) return UT_ERR_GEOMETRY;
+      inv[g] = 1.0f / span;
+      if (g % gpl != 0 && (h->group_xmin[g] < h->group_xmin[g - 1] || h->group_xmax[g] < h->group_xmax[g - 1]))
+        return UT_ERR_GEOMETRY;                                           // bounds monotone inside a layer
+    }
+  }
+  // ---- one device block, 256-byte aligned sub-tables ----
+  auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
+  const size_t sz_id = up(h->id_table_size * 4), sz_s = up(ns * 4), sz_g = up((ng + 1) * 4);
+  const size_t total = sz_id + 9 * sz_s + 4 * sz_g;
+  unsigned char* dev = nullptr;
+  if (cudaMalloc(&dev, total) != cudaSuccess) return UT_ERR_CUDA;
+  std::vector<unsigned char> host(total, 0);
+  size_t off = 0;
+  auto put = [&](const void* src, size_t bytes, size_t slot) {
+    const void* d = dev + off;
+    memcpy(host.data() + off, src, bytes);
+    off += slot;
+    return d;
+  };
+  *out = *h;
+  out->id_to_sector = (const uint32_t*)put(h->id_to_sector, h->id_table_size * 4, sz_id);
+  out->sector_raw_id = (const uint32_t*)put(h->sector_raw_id, ns * 4, sz_s);
+  out->sector_group = (const uint32_t*)put(h->sector_group, ns * 4, sz_s);
+  out->x0 = (const float*)put(h->x0, ns * 4, sz_s);
+  out->pitch = (const float*)put(h->pitch, ns * 4, sz_s);
+  out->dxdy = (const float*)put(h->dxdy, ns * 4, sz_s);
+  out->z = (const float*)put(h->z, ns * 4, sz_s);
+  out->y_begin = (const float*)put(h->y_begin, ns * 4, sz_s);
+  out->y_end = (const float*)put(h->y_end, ns * 4, sz_s);
+  out->weight = (const float*)put(h->weight, ns * 4, sz_s);
+  out->group_xmin = (const float*)put(h->group_xmin, ng * 4, sz_g);
+  out->group_xmax = (const float*)put(h->group_xmax, ng * 4, sz_g);
+  out->group_first_sector = (const uint32_t*)put(first.data(), (ng + 1) * 4, sz_g);
+  out->group_inv_span = (const float*)put(inv.data(), ng * 4, sz_g);
+  if (cudaMemcpy(dev, host.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaFree(dev);
+    return UT_ERR_CUDA;
+  }
+  GeomOwner* own = new (std::nothrow) GeomOwner;
+  if (!own) { cudaFree(dev); return UT_ERR_CUDA; }
+  own->block = dev;
+  out->owner = own;
+  return UT_OK;
+}
+
+int32_t ut_geometry_free(ut_geometry* g) {
+  if (!g) return UT_ERR_NULL;
+  if (g->owner) {
+    GeomOwner* own = static_cast<GeomOwner*>(g->owner);
+    cudaFree(own->block);
+    delete own;
+    g->owner = nullptr;
+  }
+  return UT_OK;
+}
+
+size_t ut_decode_workspace_bytes(int32_t max_events) {
+  return 16 + 8 * (size_t)(max_events > 0 ? max_events : 0) + 8;
+}
+
+int32_t ut_decode_workspace_init(void* workspace, int32_t max_events, ut_stream_t stream) {
+  if (!workspace) return UT_ERR_NULL;
+  if (max_events < 0) return UT_ERR_ARG;
+  return cudaMemsetAsync(workspace, 0, ut_decode_workspace_bytes(max_events), (cudaStream_t)stream) == cudaSuccess
+             ? UT_OK : UT_ERR_CUDA;
+}
+
+int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_t n_events,
+                  const ut_geometry* geometry, ut_hits* hits_out, uint32_t* hit_offsets_out, ut_stream_t stream) {
+  launch_info().kernels_launched = 0;
+  if (!bank_offsets || !geometry || !hits_out || !hit_offsets_out) return UT_ERR_NULL;
+  if (n_events < 0) return UT_ERR_ARG;
+  if (!geometry->group_first_sector || !geometry->group_inv_span) return UT_ERR_GEOMETRY;   // not uploaded
+  if (geometry->n_sectors > UT_MAX_SECTORS || geometry->n_groups > UT_MAX_GROUPS) return UT_ERR_LIMIT;
+  if (!hits_out->x_at_y0 || !hits_out->z_at_y0 || !hits_out->y_begin || !hits_out->y_end || !hits_out->dxdy ||
+      !hits_out->weight || !hits_out->id)
+    if (hits_out->capacity > 0) return UT_ERR_NULL;
+  if (!hits_out->status || !hits_out->workspace) return UT_ERR_NULL;
+  if ((reinterpret_cast<uintptr_t>(raw_banks) & 15u) || (reinterpret_cast<uintptr_t>(bank_offsets) & 15u) ||
+      (reinterpret_cast<uintptr_t>(hits_out->workspace) & 15u))
+    return UT_ERR_ARG;
+  hits_out->geom = geometry;
+  if (n_events == 0)      // the offsets array still has its single entry
+    return cudaMemsetAsync(hit_offsets_out, 0, 4, (cudaStream_t)stream) == cudaSuccess ? UT_OK : UT_ERR_CUDA;
+  if (!raw_banks) return UT_ERR_NULL;
+  return launch_decode(raw_banks, bank_offsets, n_events, geometry, hits_out, hit_offsets_out, (cudaStream_t)stream);
+}
+
+int32_t compass_config_default(float p_min_mev, float window_scale, int32_t min_hits, int32_t max_candidates_per_layer,
+                               const ut_geometry* geometry, compass_config* out) {
+  if (!geometry || !out) return UT_ERR_NULL;
+  if (!(p_min_mev > 0.f) || !(window_scale > 0.f)) return UT_ERR_ARG;
+  const double kappa = 60.0, z_mag = 1750.0;
+  const double kick = (double)window_scale * kappa / (double)p_min_mev;
+  for (int l = 0; l < UT_N_LAYERS; ++l) out->win_half[l] = (float)(kick * ((double)geometry->layer_z[l] - z_mag) + 0.5);
+  out->y_tol = 0.5f; out->max_slope = (float)(kick + 0.0015); out->kink_tol = 1.5f; out->seed_tol = 0.5f;
+  out->w_velo = 100.0f; out->max_chi2_ndf = 9.0f; out->kappa = (float)kappa; out->z_mag = (float)z_mag;
+  out->min_hits = min_hits; out->max_candidates_per_layer = max_candidates_per_layer;
+  return UT_OK;
+}
+
+static int32_t check_config(const compass_config* c) {
+  if (c->min_hits != 3 && c->min_hits != 4) return UT_ERR_ARG;
+  if (c->max_candidates_per_layer < 1 || c->max_candidates_per_layer > UT_MAX_CANDIDATES) return UT_ERR_ARG;
+  for (int l = 0; l < UT_N_LAYERS; ++l) if (!(c->win_half[l] >= 0.f)) return UT_ERR_ARG;
+  return UT_OK;
+}
+
+int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                      const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                      ut_tracks* tracks_out, ut_stream_t stream) {
+  launch_info().kernels_launched = 0;
+  if (!hits || !hit_offsets || !velo || !velo_offsets || !config || !tracks_out || !hits->geom) return UT_ERR_NULL;
+  if (n_events < 0) return UT_ERR_ARG;
+  if (const int32_t rc = check_config(config)) return rc;
+  if (!tracks_out->status) return UT_ERR_NULL;
+  if (n_events == 0) return UT_OK;
+  if (!tracks_out->hit_idx || !tracks_out->n_hits || !tracks_out->qop || !tracks_out->chi2 || !velo->x || !velo->y ||
+      !velo->tx || !velo->ty)
+    return UT_ERR_NULL;
+  if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
+  return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Host-buffer pipeline (bench.py "e2e"): one arena of device buffers, async copies around the two calls.
+// ---------------------------------------------------------------------------------------------------
+struct ut_pipeline {
+  ut_geometry geom;
+  int32_t max_events;
+  size_t max_raw;
+  uint64_t max_hits;
+  uint32_t max_velo;
+  unsigned char* block;
+  uint8_t* raw;
+  uint32_t *bank_offsets, *hit_offsets, *velo_offsets, *status /* [2] */;
+  float *vx, *vy, *vtx, *vty;
+  ut_hits hits;
+  ut_tracks tracks;
+};
+
+int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_raw_bytes, uint64_t max_hits,
+                           uint32_t max_velo, ut_pipeline** out) {
+  if (!g || !out) return UT_ERR_NULL;
+  if (max_events < 1) return UT_ERR_ARG;
+  ut_pipeline* p = new (std::nothrow) ut_pipeline;
+  if (!p) return UT_ERR_CUDA;
+  memset(p, 0, sizeof(*p));
+  p->geom = *g; p->geom.owner = nullptr;
+  p->max_events = max_events; p->max_raw = max_raw_bytes; p->max_hits = max_hits; p->max_velo = max_velo;
+  auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
+  const size_t s_raw = up(max_raw_bytes + 16), s_bo = up(((size_t)max_events * g->n_sectors + 1) * 4),
+               s_ho = up(((size_t)max_events * g->n_groups + 1) * 4), s_vo = up(((size_t)max_events + 1) * 4),
+               s_st = 256, s_v = up((size_t)max_velo * 4), s_h = up((size_t)max_hits * 4),
+               s_ws = up(ut_decode_workspace_bytes(max_events)), s_ti = up((size_t)max_velo * 16);
+  const size_t total = s_raw + s_bo + s_ho + s_vo + s_st + 4 * s_v + 7 * s_h + s_ws + s_ti + 3 * s_v;
+  if (cudaMalloc(&p->block, total) != cudaSuccess) { delete p; return UT_ERR_CUDA; }
+  unsigned char* q = p->block;
+  auto take = [&](size_t n) { unsigned char* r = q; q += n; return r; };
+  p->raw = take(s_raw);
+  p->bank_offsets = (uint32_t*)take(s_bo); p->hit_offsets = (uint32_t*)take(s_ho);
+  p->velo_offsets = (uint32_t*)take(s_vo); p->status = (uint32_t*)take(s_st);
+  p->vx = (float*)take(s_v); p->vy = (float*)take(s_v); p->vtx = (float*)take(s_v); p->vty = (float*)take(s_v);
+  p->hits.x_at_y0 = (float*)take(s_h); p->hits.z_at_y0 = (float*)take(s_h); p->hits.y_begin = (float*)take(s_h);
+  p->hits.y_end = (float*)take(s_h); p->hits.dxdy = (float*)take(s_h); p->hits.weight = (float*)take(s_h);
+  p->hits.id = (uint32_t*)take(s_h);
+  p->hits.capacity = max_hits; p->hits.geom = &p->geom; p->hits.status = p->status;
+  p->hits.workspace = take(s_ws);
+  p->tracks.hit_idx = (int32_t*)take(s_ti);
+  p->tracks.n_hits = (int32_t*)take(s_v); p->tracks.qop = (float*)take(s_v); p->tracks.chi2 = (float*)take(s_v);
+  p->tracks.status = p->status + 1;
+  if (cudaMemset(p->block, 0, total) != cudaSuccess) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
+  *out = p;
+  return UT_OK;
+}
+
+int32_t ut_pipeline_destroy(ut_pipeline* p) {
+  if (!p) return UT_ERR_NULL;
+  cudaFree(p->block);
+  delete p;
+  return UT_OK;
+}
+
+int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_bytes, const uint32_t* bo_h,
+                             const velo_states* velo_h, const uint32_t* vo_h, uint32_t n_velo, int32_t n_events,
+                             const compass_config* config, ut_tracks* tracks_h, uint32_t* status_h, uint32_t* n_hits_h,
+                             ut_stream_t stream_) {
+  if (!p || !bo_h || !velo_h || !vo_h || !config || !tracks_h) return UT_ERR_NULL;
+  if (n_events < 0 || n_events > p->max_events || raw_bytes > p->max_raw || n_velo > p->max_velo) return UT_ERR_ARG;
+  if (n_events > 0 && !raw_h) return UT_ERR_NULL;
+  cudaStream_t s = (cudaStream_t)stream_;
+  const ut_geometry* g = &p->geom;
+  auto h2d = [&](void* d, const void* h, size_t n) { return n == 0 || cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, s) == cudaSuccess; };
+  auto d2h = [&](void* h, const void* d, size_t n) { return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, s) == cudaSuccess; };
+  bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess;
+  ok = ok && h2d(p->raw, raw_h, raw_bytes) && h2d(p->bank_offsets, bo_h, ((size_t)n_events * g->n_sectors + 1) * 4) &&
+       h2d(p->velo_offsets, vo_h, ((size_t)n_events + 1) * 4) && h2d(p->vx, velo_h->x, (size_t)n_velo * 4) &&
+       h2d(p->vy, velo_h->y, (size_t)n_velo * 4) && h2d(p->vtx, velo_h->tx, (size_t)n_velo * 4) &&
+       h2d(p->vty, velo_h->ty, (size_t)n_velo * 4);
+  if (!ok) return UT_ERR_CUDA;
+  int32_t rc = ut_decode(p->raw, p->bank_offsets, n_events, g, &p->hits, p->hit_offsets, stream_);
+  if (rc) return rc;
+  int launched = launch_info().kernels_launched;
+  velo_states vd = {p->vx, p->vy, p->vtx, p->vty, velo_h->z};
+  rc = compass_track(&p->hits, p->hit_offsets, &vd, p->velo_offsets, n_events, config, &p->tracks, stream_);
+  if (rc) return rc;
+  launch_info().kernels_launched += launched;
+  ok = d2h(tracks_h->hit_idx, p->tracks.hit_idx, (size_t)n_velo * 16) && d2h(tracks_h->n_hits, p->tracks.n_hits, (size_t)n_velo * 4) &&
+       d2h(tracks_h->qop, p->tracks.qop, (size_t)n_velo * 4) && d2h(tracks_h->chi2, p->tracks.chi2, (size_t)n_velo * 4);
+  if (status_h) ok = ok && d2h(status_h, p->status, 8);
+  if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * g->n_groups, 4);
+  return ok ? UT_OK : UT_ERR_CUDA;
+}
+
+int32_t ut_pipeline_device_hits(ut_pipeline* p, ut_hits* hits_out, const uint32_t** hit_offsets_out) {
+  if (!p || !hits_out || !hit_offsets_out) return UT_ERR_NULL;
+  *hits_out = p->hits;
+  *hit_offsets_out = p->hit_offsets;
+  return UT_OK;
+}
+
+}  // extern "C"

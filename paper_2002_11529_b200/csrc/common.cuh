@@ -1,0 +1,126 @@
+// common.cuh -- device helpers shared by the decode and Compass kernels (sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ut_compass.h"
+
+namespace utc {
+
+constexpr uint32_t kInvalid = 0xFFFFFFFFu;
+constexpr int kWarp = 32;
+
+// Device-side view of the geometry tables (passed by value in kernel parameters).
+struct GeomDev {
+  uint32_t n_sectors, n_groups, id_table_size, groups_per_layer;
+  const uint32_t *id_to_sector, *sector_raw_id, *sector_group, *group_first_sector;
+  const float *x0, *pitch, *dxdy, *z, *y_begin, *y_end, *weight;
+  const float *group_xmin, *group_xmax, *group_inv_span;
+  float layer_z[4], layer_dxdy[4];
+};
+
+inline GeomDev make_geom_dev(const ut_geometry* g) {
+  GeomDev d;
+  d.n_sectors = g->n_sectors; d.n_groups = g->n_groups; d.id_table_size = g->id_table_size;
+  d.groups_per_layer = g->n_groups / UT_N_LAYERS;
+  d.id_to_sector = g->id_to_sector; d.sector_raw_id = g->sector_raw_id; d.sector_group = g->sector_group;
+  d.group_first_sector = g->group_first_sector;
+  d.x0 = g->x0; d.pitch = g->pitch; d.dxdy = g->dxdy; d.z = g->z; d.y_begin = g->y_begin; d.y_end = g->y_end;
+  d.weight = g->weight; d.group_xmin = g->group_xmin; d.group_xmax = g->group_xmax;
+  d.group_inv_span = g->group_inv_span;
+  for (int l = 0; l < 4; ++l) { d.layer_z[l] = g->layer_z[l]; d.layer_dxdy[l] = g->layer_dxdy[l]; }
+  return d;
+}
+
+// thread-local record of the last launches (ut_last_launch_info)
+ut_launch_info& launch_info();
+// records "<what>: <cuda error string>" for ut_last_error(); returns UT_ERR_CUDA
+int32_t cuda_fail(const char* what, cudaError_t err);
+#define UTC_CUDA(call)                                              \
+  do {                                                              \
+    const cudaError_t utc_err__ = (call);                           \
+    if (utc_err__ != cudaSuccess) return utc::cuda_fail(#call, utc_err__); \
+  } while (0)
+
+#ifdef __CUDACC__
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+// ---- mbarrier + 1-D bulk copy (TMA unit, SASS UBLKCP) ----------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// ---- single-word flags in global memory --------------------------------------------------------------
+__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// ---- warp helpers -------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+  return v;
+}
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, v, o);
+    if (lane >= o) v += t;
+  }
+  return v;
+}
+
+// bump allocator over dynamic shared memory, 16-byte granules
+struct Carver {
+  unsigned char* p;
+  __device__ explicit Carver(unsigned char* base) : p(base) {}
+  template <typename T>
+  __device__ T* take(size_t n) {
+    T* r = reinterpret_cast<T*>(p);
+    p += (n * sizeof(T) + 15) & ~size_t(15);
+    return r;
+  }
+};
+
+#endif  // __CUDACC__
+
+inline size_t align16(size_t v) { return (v + 15) & ~size_t(15); }
+
+}  // namespace utc

@@ -1,0 +1,216 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from synth import geometry as G
+from synth.events import EventModel, encode_event, generate_batch, assemble_batch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu(geom):
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from gpu_helpers import GpuRunner
+    return GpuRunner(geom)
+
+
+def oracle_run(b, geom, p):
+    return oracle.run_batch(b, geom, p)
+
+
+def check_batch(gpu, geom, b, p):
+    from gpu_helpers import compare_decode, compare_tracks
+    h_ref, t_ref = oracle_run(b, geom, p)
+    hits, trk = gpu.run(b, p)
+    got, off, st = gpu.hits_numpy(hits, b.n_events)
+    compare_decode(h_ref, got, off, st)
+    n_diff, n_tie = compare_tracks(t_ref, trk)
+    # identical fp32 arithmetic on both sides: even the flagged near-ties are expected to agree
+    assert n_diff == 0
+    assert np.array_equal(trk["chi2"].view(np.uint32), t_ref.chi2.view(np.uint32))
+    assert np.array_equal(trk["qop"].view(np.uint32), t_ref.qop.view(np.uint32))
+    return h_ref, t_ref
+
+
+def test_config1(gpu, wl):
+    geom, b, p = wl(1)
+    h, t = check_batch(gpu, geom, b, p)
+    assert (t.n_hits > 0).sum() >= 10
+
+
+def test_config2(gpu, wl):
+    geom, b, p = wl(2)
+    check_batch(gpu, geom, b, p)
+
+
+def test_config3_subset(gpu, wl):
+    geom, b, p = wl(3, 300)          # several waves of CTAs, ragged tail
+    check_batch(gpu, geom, b, p)
+
+
+def test_config4_subset(gpu, wl):
+    geom, b, p = wl(4, 40)
+    h, t = check_batch(gpu, geom, b, p)
+    assert (t.cand_n > p.max_candidates_per_layer).any()      # the candidate cap path runs on the GPU too
+
+
+@pytest.mark.parametrize("min_hits", [3, 4])
+@pytest.mark.parametrize("scale", [0.5, 1.0, 2.0])
+@pytest.mark.parametrize("C", [8, 16, 32])
+def test_config5_sweep_subset(gpu, wl, min_hits, scale, C):
+    geom, b, _ = wl(5, 60)
+    p = synth.CONFIGS[5].compass_params(min_hits=min_hits, window_scale=scale, max_candidates_per_layer=C)
+    from gpu_helpers import compare_tracks
+    if not hasattr(gpu, "_c5"):
+        gpu._c5 = (gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity),
+                   oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity))
+    hits, h_ref = gpu._c5
+    t_ref = oracle.compass(h_ref, b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z, b.velo_offsets, b.n_events,
+                           geom, p)
+    trk = gpu.compass(hits, b, p)
+    n_diff, _ = compare_tracks(t_ref, trk)
+    assert n_diff == 0
+
+
+def test_small_candidate_caps(gpu, wl):
+    geom, b, _ = wl(2, 30)
+    from gpu_helpers import compare_tracks
+    hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+    h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+    for C in (1, 2, 3, 5):
+        p = synth.make_compass_params(max_candidates_per_layer=C, window_scale=2.0)
+        t_ref = oracle.compass(h_ref, b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z, b.velo_offsets,
+                               b.n_events, geom, p)
+        assert (t_ref.cand_n > C).any()
+        n_diff, _ = compare_tracks(t_ref, gpu.compass(hits, b, p))
+        assert n_diff == 0
+
+
+def _one_event(geom, sector, strip, frac, order=None):
+    n = len(sector)
+    raw, offs = encode_event(geom, np.asarray(sector, dtype=np.int64), np.asarray(strip), np.asarray(frac),
+                             np.zeros(n, int), order)
+    return dict(raw=raw, bank_offs=offs, velo=tuple(np.zeros(0, np.float32) for _ in range(4)),
+                truth_hit_id=np.zeros((0, 4), np.int64), q=np.zeros(0, np.int8), p=np.zeros(0), n_hits=n)
+
+
+def test_decode_edge_cases(gpu, geom):
+    from gpu_helpers import compare_decode
+    rng = np.random.default_rng(5)
+    s_full = G.dense_sector(2, 7, 6)
+    strips = np.arange(511, -1, -1)
+    sec1 = np.repeat(np.arange(14) + G.dense_sector(1, 0, 0), 512)     # all hits of an event in one group
+    st1 = np.tile(np.arange(512), 14)
+    perm = rng.permutation(sec1.size)
+    events = [
+        _one_event(geom, [], [], []),                                   # empty event
+        _one_event(geom, np.full(512, s_full), strips, strips % 2),     # one 512-word bank, descending order
+        _one_event(geom, sec1[perm], st1[perm], np.zeros(sec1.size, int), rng.permutation(896)),
+        _one_event(geom, [], [], []),
+        _one_event(geom, [5, 5, 9, 895, 0], [1, 2, 3, 511, 0], [0, 1, 0, 1, 0]),
+    ]
+    b = assemble_batch(geom, events)
+    ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+    hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+    got, off, st = gpu.hits_numpy(hits, b.n_events)
+    compare_decode(ref, got, off, st)
+    # no events
+    hits = gpu.decode(np.zeros(0, np.uint8), np.zeros(1, np.uint32), 0, 0)
+    assert int(hits.hit_offsets[0].item()) == 0
+
+
+def test_decode_stable_ties(gpu, geom):
+    from gpu_helpers import compare_decode
+    # X layers: identical strips in every row of a column -> 14-way exact ties, order = dense sector
+    sec = np.concatenate([np.arange(14) + G.dense_sector(0, c, 0) for c in (3, 8)])
+    sec = np.repeat(sec, 3)
+    strip = np.tile([100, 7, 300], 28)
+    rng = np.random.default_rng(1)
+    perm = rng.permutation(sec.size)
+    b = assemble_batch(geom, [_one_event(geom, sec[perm], strip[perm], np.ones(sec.size, int), rng.permutation(896))])
+    ref = oracle.decode(b.raw, b.bank_offsets, 1, geom, b.hit_capacity)
+    hits = gpu.decode(b.raw, b.bank_offsets, 1, b.hit_capacity)
+    got, off, st = gpu.hits_numpy(hits, 1)
+    compare_decode(ref, got, off, st)
+
+
+def test_decode_error_status(gpu, geom):
+    e = _one_event(geom, [5, 5, 9], [1, 2, 3], [0, 0, 0])
+    raw, offs = e["raw"], e["bank_offs"].astype(np.uint32)
+
+    def both(r, capacity=None):
+        cap = 3 if capacity is None else capacity
+        ref = oracle.decode(r, offs, 1, geom, cap)
+        hits = gpu.decode(r, offs, 1, cap)
+        got, off, st = gpu.hits_numpy(hits, 1)
+        return ref, got, off, st
+
+    bad = raw.copy(); bad[int(offs[0]):int(offs[0]) + 4] = np.frombuffer(np.uint32(15).tobytes(), np.uint8)
+    ref, got, off, st = both(bad)
+    assert st == ref.status == oracle.ST_UNKNOWN_SECTOR and np.array_equal(off, ref.hit_offsets)
+    bad = raw.copy(); bad[int(offs[0]):int(offs[0]) + 4] = raw[int(offs[1]):int(offs[1]) + 4]
+    ref, got, off, st = both(bad)
+    assert st == ref.status == oracle.ST_DUPLICATE_SECTOR
+    bad = raw.copy(); bad[int(offs[5]) + 4] = 7
+    ref, got, off, st = both(bad)
+    assert st == ref.status == oracle.ST_BAD_BANK_SIZE and np.array_equal(off, ref.hit_offsets)
+    ref, got, off, st = both(raw, capacity=2)
+    assert st == ref.status == oracle.ST_CAPACITY and np.array_equal(off, ref.hit_offsets)
+
+
+def test_repeated_calls_reuse_workspace(gpu, wl):
+    """The look-back workspace re-arms itself: same buffers, several calls, different batch sizes."""
+    from gpu_helpers import compare_decode
+    geom, b, p = wl(2)
+    ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+    B, torch = gpu.B, gpu.torch
+    hits = B.Hits(b.hit_capacity, b.n_events, gpu.geom)
+    raw_d, bo_d = B.to_device_raw(b.raw), B.to_device_u32(b.bank_offsets)
+    for n in (100, 37, 100, 1, 100):
+        hits.hit_offsets.zero_()
+        B.ut_decode(raw_d, bo_d, n, gpu.geom, hits)
+        torch.cuda.synchronize()
+        off = hits.hit_offsets[:n * 64 + 1].cpu().numpy().view(np.uint32)
+        assert np.array_equal(off, ref.hit_offsets[:n * 64 + 1])
+    got, off, st = gpu.hits_numpy(hits, 100)
+    compare_decode(ref, got, off, st)
+
+
+def test_small_staging_takes_generic_paths(gpu, wl, monkeypatch):
+    """Force the events through the non-staged decode path and the global-memory Compass path."""
+    geom, b, p = wl(2, 12)
+    monkeypatch.setenv("UT_DECODE_HIT_STAGE", "256")
+    monkeypatch.setenv("UT_DECODE_RAW_STAGE", "4096")
+    monkeypatch.setenv("UT_COMPASS_HIT_STAGE", "512")
+    check_batch(gpu, geom, b, p)
+
+
+def test_tracks_empty_cases(gpu, geom):
+    p = synth.make_compass_params()
+    b = generate_batch(geom, EventModel(fixed_tracks=0, noise_mean=50.0), seed=2, n_events=3)
+    hits, trk = gpu.run(b, p)
+    assert trk["n_hits"].shape == (0,)
+    b = generate_batch(geom, EventModel(fixed_tracks=5, noise_mean=0.0, efficiency=0.0), seed=2, n_events=2)
+    hits, trk = gpu.run(b, p)
+    assert np.all(trk["n_hits"] == 0) and np.all(trk["hit_idx"] == -1) and np.all(trk["qop"] == 0)
+
+
+def test_invalid_arguments(gpu, wl):
+    geom, b, p = wl(1)
+    B = gpu.B
+    hits = gpu.decode(b.raw, b.bank_offsets, 1, b.hit_capacity)
+    velo = B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z)
+    vo = B.to_device_u32(b.velo_offsets)
+    tracks = B.Tracks(20)
+    for bad in (dataclasses.replace(p, min_hits=2), dataclasses.replace(p, max_candidates_per_layer=0),
+                dataclasses.replace(p, max_candidates_per_layer=33)):
+        with pytest.raises(B.UTError):
+            B.compass_track(hits, hits.hit_offsets, velo, vo, 1, B.make_config(bad), tracks)
+    with pytest.raises(B.UTError):
+        B.ut_decode(B.to_device_raw(b.raw), B.to_device_u32(b.bank_offsets), -1, gpu.geom, hits)
