@@ -51,7 +51,8 @@ typedef void* ut_stream_t;
 #define UT_STATUS_BAD_BANK_SIZE 4u     /* bank bytes != round4(6 + 2*count) or misaligned (bank ignored) */
 #define UT_STATUS_CAPACITY 8u          /* hits would exceed `capacity`; that event's hits are not written */
 #define UT_STATUS_BAD_OFFSETS 16u      /* compass_track: offsets not monotone / inconsistent            */
-#define UT_STATUS_EVENT_TOO_LARGE 32u  /* compass_track: > 65535 hits in one layer of one event; no tracks */
+#define UT_STATUS_EVENT_TOO_LARGE 32u  /* compass_track: > 65535 hits in one event; no tracks for that event */
+#define UT_STATUS_BAD_HIT_ID 64u       /* compass_track: a hit id names no sector of the geometry (hit ignored) */
 
 #define UT_MAX_SECTORS 1024
 #define UT_MAX_GROUPS 128
@@ -76,8 +77,13 @@ typedef struct {
   /* filled by ut_geometry_upload (device, library-owned until ut_geometry_free) */
   const uint32_t* group_first_sector; /* [n_groups + 1] */
   const float* group_inv_span;        /* [n_groups] 1 / (group_xmax - group_xmin) */
+  uint32_t flags;                     /* UT_GEOM_* properties found by ut_geometry_upload */
   void* owner;                        /* opaque allocation handle, NULL for caller-owned tables */
 } ut_geometry;
+
+/* y_begin and y_end are non-decreasing over the sectors of every group: the sector row a track crosses
+ * can be found by binary search (else compass_track scans the group's sectors). */
+#define UT_GEOM_ROWS_SORTED 1u
 
 /* Copies HOST tables (`host_tables` holds HOST pointers in the array fields) to the device, checks
  * the contract above and fills `device_out` with device pointers.  Synchronous; call once at set-up. */

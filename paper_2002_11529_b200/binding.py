@@ -22,7 +22,7 @@ _lib = C.CDLL(_LIBPATH)
 
 UT_OK = 0
 UT_STATUS_UNKNOWN_SECTOR, UT_STATUS_DUPLICATE_SECTOR, UT_STATUS_BAD_BANK_SIZE, UT_STATUS_CAPACITY = 1, 2, 4, 8
-UT_STATUS_BAD_OFFSETS, UT_STATUS_EVENT_TOO_LARGE = 16, 32
+UT_STATUS_BAD_OFFSETS, UT_STATUS_EVENT_TOO_LARGE, UT_STATUS_BAD_HIT_ID = 16, 32, 64
 UT_MAX_CANDIDATES = 32
 
 
@@ -34,7 +34,8 @@ class ut_geometry(C.Structure):
                 ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
                 ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
                 ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
-                ("group_first_sector", C.c_void_p), ("group_inv_span", C.c_void_p), ("owner", C.c_void_p)]
+                ("group_first_sector", C.c_void_p), ("group_inv_span", C.c_void_p), ("flags", C.c_uint32),
+                ("owner", C.c_void_p)]
 
 
 class ut_hits(C.Structure):

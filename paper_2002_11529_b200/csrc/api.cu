@@ -57,6 +57,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   // ---- container contract (include/ut_compass.h) ----
   std::vector<uint32_t> first(ng + 1, 0);
   std::vector<float> inv(ng);
+  bool rows_sorted = true;
   {
     uint32_t prev = 0;
     std::vector<uint32_t> cnt(ng, 0);
@@ -71,8 +72,10 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
     for (uint32_t g = 0; g < ng; ++g) {
       if (cnt[g] == 0) return UT_ERR_GEOMETRY;
       first[g + 1] = first[g] + cnt[g];
-      for (uint32_t s = first[g]; s < first[g + 1]; ++s)
+      for (uint32_t s = first[g]; s < first[g + 1]; ++s) {
         if (h->dxdy[s] != h->dxdy[first[g]]) return UT_ERR_GEOMETRY;      // one stereo angle per group
+        if (s > first[g] && (h->y_begin[s] < h->y_begin[s - 1] || h->y_end[s] < h->y_end[s - 1])) rows_sorted = false;
+      }
       const float span = h->group_xmax[g] - h->group_xmin[g];
       if (!(span > 0.f)) return UT_ERR_GEOMETRY;
       inv[g] = 1.0f / span;
@@ -95,6 +98,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
     return d;
   };
   *out = *h;
+  out->flags = rows_sorted ? UT_GEOM_ROWS_SORTED : 0u;
   out->id_to_sector = (const uint32_t*)put(h->id_to_sector, h->id_table_size * 4, sz_id);
   out->sector_raw_id = (const uint32_t*)put(h->sector_raw_id, ns * 4, sz_s);
   out->sector_group = (const uint32_t*)put(h->sector_group, ns * 4, sz_s);

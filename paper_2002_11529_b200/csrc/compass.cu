@@ -2,20 +2,32 @@
 //
 // The paper runs two kernels: "search UT windows" (2-D: 4 panels x tracks) writes
 // (first hit, size) ranges to global memory, then "tracklet finding" (thread per track)
-// reads them back through a shared-memory cache.  On a B200 the whole event fits in one
-// SM's shared memory, so one CTA takes one event:
+// reads them back through a shared-memory cache.  That shape leaves a B200 warp at
+// 7 of 32 lanes (profiles/r1a_first_path.md).  Here one CTA takes one event and keeps it on chip:
 //
-//   stage the event's x / yBegin / yEnd / z / weight arrays in smem (read HBM/L2 once per event)
-//   phase 1, lane = (track, layer)  -- the paper's 2-D window kernel shape:
-//       straight-line extrapolation, group range by binary search on the group x-bounds, binary
-//       search of the first hit with d >= -win, scan while d <= +win with the y test; the accepted
-//       hits (closest `max_candidates_per_layer` in |d|) go to a per-(track, layer) list in smem
-//   phase 2, the 4 lanes of a track split the seed pairs (a, b): slope + kink cuts, compatible hits
-//       in the other two layers as 32-bit masks, every 3/4-hit combination fitted (linear chi2 fit
-//       with the VELO pseudo-point), packed (n, chi2, positions) key, min over the quad = the
-//       deterministic best tracklet; forward seeds first, backward only if forward found nothing.
-//   The candidate lists never leave the SM; the two phases are separated by __syncwarp only.
+//   stage    the event's hits are re-bucketed PER SECTOR into shared memory (x and the hit index only;
+//            count -> block scan -> scatter).  A sector's y range, stereo slope, z and weight are rows of
+//            the geometry table, so the y test of the window search becomes a per-sector test: the scan
+//            touches the ~2 hits of the one sector row the track crosses instead of the ~20 hits of all
+//            14 rows of the column group.
+//   phase 1  lane = (track, layer), 8 tracks per warp (the paper's 2-D window kernel shape):
+//            straight-line extrapolation, column groups by binary search on the group x bounds, sector
+//            row by binary search on the y bounds, |d| <= win test on the sector's hits; accepted hits go
+//            to the (track, layer) candidate list in shared memory, kept sorted by hit index and capped
+//            to the `max_candidates_per_layer` closest in |d|.
+//   phase 2  the nested loops of the tracklet search are flattened over the 32 lanes of the warp:
+//            (a) all seed pairs (a, b) of the 8 tracks, one pair per lane: slope + kink cuts; survivors are
+//                compacted (ballot) into a per-warp seed queue;
+//            (b) whenever 32 seeds are queued, one seed per lane: compatible hits in the other two layers
+//                as 32-bit masks, giving the number of 3/4-hit combinations of the seed;
+//            (c) all combinations of those 32 seeds, one fit per lane (linear chi2 fit with the VELO
+//                pseudo-point), packed (n, chi2, positions) key, atomicMin into the track's best key.
+//            Forward seeds first, backward only for tracks where forward found nothing valid (A11).
+//   Candidate lists, queues and best keys never leave the SM; the phases of a warp are separated by
+//   __syncwarp only, and the warps of a CTA pull 8-track batches from a shared-memory ticket.
 //
+// Events that do not fit the staging buffer take the same phases with a group-level binary search on the
+// global x-sorted arrays (the plain definition of the window, per-hit y test).
 // fp32 arithmetic uses __f*_rn intrinsics in the order of DESIGN.md section 3 (bit-exact, no FMA).
 #include <algorithm>
 #include <cstdlib>
@@ -26,22 +38,27 @@ namespace utc {
 
 constexpr float kGroupEps = 0.01f;     // slack of the group pre-selection [mm] (A17)
 constexpr unsigned long long kNoKey = ~0ull;
+constexpr int kTPW = 8;                // tracks per warp batch (x 4 layers = 32 lanes)
+constexpr int kSeedQ = 64;             // per-warp seed ring (<= 31 left over + <= 32 new)
 
 struct CompassArgs {
-  const float *hx, *hz, *hyb, *hye, *hdxdy, *hw;
+  const float* hx;
+  const uint32_t* hid;
+  const float *hyb, *hye;              // per-hit y range: only the global (unstaged) path reads them
   const uint32_t* hit_offsets;
   const float *vx, *vy, *vtx, *vty;
   float vz;
   const uint32_t* velo_offsets;
   int32_t n_events;
-  uint32_t n_groups, gpl;
-  const float *group_xmin, *group_xmax;
+  uint32_t n_sectors, n_groups, gpl, id_table_size, rows_sorted;
+  const uint32_t *id_to_sector, *group_first_sector;
+  const float *group_xmin, *group_xmax, *sec_yb, *sec_ye, *sec_dxdy, *sec_z, *sec_w;
   float layer_z[4], layer_dxdy[4];
   compass_config c;
   int32_t *out_idx, *out_n;
   float *out_qop, *out_chi2;
   uint32_t* status;
-  uint32_t hit_stage;     // elements per staged array
+  uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
 };
 
 struct FitResult { float chi2, b; bool valid; };
@@ -67,24 +84,20 @@ __device__ __forceinline__ float fit_res(bool p, float d, float dz, float w, flo
 }
 
 // Weighted linear LSQ of d vs dz = z - z_mag with the VELO pseudo-point (0, 0, w_velo); hits in layer order.
-__device__ __forceinline__ FitResult fit_tracklet(bool p0, float d0, float z0, float w0, bool p1, float d1, float z1,
-                                                  float w1, bool p2, float d2, float z2, float w2, bool p3, float d3,
-                                                  float z3, float w3, int n, const compass_config& c) {
-  const float dz0 = __fsub_rn(z0, c.z_mag), dz1 = __fsub_rn(z1, c.z_mag), dz2 = __fsub_rn(z2, c.z_mag),
-              dz3 = __fsub_rn(z3, c.z_mag);
+__device__ __forceinline__ FitResult fit_tracklet(const bool (&p)[4], const float (&d)[4], const float (&z)[4],
+                                                  const float (&w)[4], int n, const compass_config& c) {
+  float dz[4];
+#pragma unroll
+  for (int l = 0; l < 4; ++l) dz[l] = __fsub_rn(z[l], c.z_mag);
   float S0 = c.w_velo, S1 = 0.f, S2 = 0.f, T0 = 0.f, T1 = 0.f;
-  fit_acc(p0, d0, dz0, w0, S0, S1, S2, T0, T1);
-  fit_acc(p1, d1, dz1, w1, S0, S1, S2, T0, T1);
-  fit_acc(p2, d2, dz2, w2, S0, S1, S2, T0, T1);
-  fit_acc(p3, d3, dz3, w3, S0, S1, S2, T0, T1);
+#pragma unroll
+  for (int l = 0; l < 4; ++l) fit_acc(p[l], d[l], dz[l], w[l], S0, S1, S2, T0, T1);
   const float det = __fsub_rn(__fmul_rn(S0, S2), __fmul_rn(S1, S1));
   const float a = __fdiv_rn(__fsub_rn(__fmul_rn(T0, S2), __fmul_rn(T1, S1)), det);
   const float b = __fdiv_rn(__fsub_rn(__fmul_rn(T1, S0), __fmul_rn(T0, S1)), det);
   float chi2 = __fmul_rn(__fmul_rn(c.w_velo, a), a);
-  chi2 = fit_res(p0, d0, dz0, w0, a, b, chi2);
-  chi2 = fit_res(p1, d1, dz1, w1, a, b, chi2);
-  chi2 = fit_res(p2, d2, dz2, w2, a, b, chi2);
-  chi2 = fit_res(p3, d3, dz3, w3, a, b, chi2);
+#pragma unroll
+  for (int l = 0; l < 4; ++l) chi2 = fit_res(p[l], d[l], dz[l], w[l], a, b, chi2);
   FitResult r;
   r.chi2 = chi2;
   r.b = b;
@@ -99,187 +112,278 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, uint32
          (unsigned long long)((p0 << 18) | (p1 << 12) | (p2 << 6) | p3);
 }
 
-struct CandView {           // per-(track, layer) candidate lists, entry i of slot s at [i * slots + s]
-  float* d;
-  uint16_t* h;
-  uint32_t slots;
+// Per-warp working set in shared memory.  Candidate i of lane-slot s (= track-in-batch * 4 + layer) lives at
+// [i * 32 + s]: the 32 lanes of phase 1 append without bank conflicts.
+struct WarpArea {
+  float* cd;                   // [C * 32] residual d of the candidate
+  uint32_t* chs;               // [C * 32] (hit index relative to the event) << 16 | dense sector
+  uint2* seedq;                // [kSeedQ] (track << 10 | ia << 5 | ib, seed slope bits)
+  unsigned long long* best;    // [kTPW]
+  int* n;                      // [32] candidates per slot
 };
 
-// One search direction for the pairs owned by this lane.  DIR 0: seeds (L0, L2), others (L1, L3);
-// DIR 1: seeds (L3, L1), others (L2, L0).
-template <int DIR>
-__device__ __forceinline__ unsigned long long search_direction(const CandView& cv, const float* __restrict__ Z,
-                                                               const float* __restrict__ W, uint32_t qslot, int ql,
-                                                               const int (&n)[4], const uint32_t (&lf)[4],
-                                                               const compass_config& c) {
-  constexpr int LA = DIR ? 3 : 0, LB = DIR ? 1 : 2, LC = DIR ? 2 : 1, LD = DIR ? 0 : 3;
-  const int nA = n[LA], nB = n[LB], nC = n[LC], nD = n[LD];
-  const uint32_t sA = qslot + LA, sB = qslot + LB, sC = qslot + LC, sD = qslot + LD;
-  unsigned long long best = kNoKey;
-  const int P = nA * nB;
-  if (ql >= P) return best;
-  int ia = ql / nB, ib = ql - ia * nB;
-  for (int p = ql; p < P; p += 4) {
-    const float da = cv.d[ia * cv.slots + sA], db = cv.d[ib * cv.slots + sB];
-    const uint32_t ha = lf[LA] + cv.h[ia * cv.slots + sA], hb = lf[LB] + cv.h[ib * cv.slots + sB];
-    const float za = Z[ha], zb = Z[hb];
-    const float bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
-    const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, c.z_mag)));
-    if (fabsf(bs) <= c.max_slope && fabsf(a0) <= c.kink_tol) {
-      uint32_t mC = 0, mD = 0;
-      for (int i = 0; i < nC; ++i) {
-        const float dc = cv.d[i * cv.slots + sC];
-        const float zc = Z[lf[LC] + cv.h[i * cv.slots + sC]];
-        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
-        if (fabsf(__fsub_rn(dc, pred)) <= c.seed_tol) mC |= 1u << i;
-      }
-      for (int i = 0; i < nD; ++i) {
-        const float dd = cv.d[i * cv.slots + sD];
-        const float zd = Z[lf[LD] + cv.h[i * cv.slots + sD]];
-        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
-        if (fabsf(__fsub_rn(dd, pred)) <= c.seed_tol) mD |= 1u << i;
-      }
-      const float wa = W[ha], wb = W[hb];
-      // every (c or none) x (d or none) with >= min_hits hits in total
-      uint32_t remC = mC;
-      for (int ci = -1;;) {
-        float dc = 0.f, zc = 0.f, wc = 0.f;
-        if (ci >= 0) {
-          const uint32_t hc = lf[LC] + cv.h[ci * cv.slots + sC];
-          dc = cv.d[ci * cv.slots + sC]; zc = Z[hc]; wc = W[hc];
-        }
-        uint32_t remD = mD;
-        for (int di = -1;;) {
-          const int nh = 2 + (ci >= 0) + (di >= 0);
-          if (nh >= c.min_hits) {
-            float dd = 0.f, zd = 0.f, wd = 0.f;
-            if (di >= 0) {
-              const uint32_t hd = lf[LD] + cv.h[di * cv.slots + sD];
-              dd = cv.d[di * cv.slots + sD]; zd = Z[hd]; wd = W[hd];
-            }
-            const uint32_t pc = ci >= 0 ? (uint32_t)ci : 63u, pd = di >= 0 ? (uint32_t)di : 63u;
-            FitResult r;
-            unsigned long long key;
-            if (DIR == 0) {      // layer order L0 = a, L1 = c, L2 = b, L3 = d
-              r = fit_tracklet(true, da, za, wa, ci >= 0, dc, zc, wc, true, db, zb, wb, di >= 0, dd, zd, wd, nh, c);
-              key = make_key(nh, r.chi2, (uint32_t)ia, pc, (uint32_t)ib, pd);
-            } else {             // layer order L0 = d, L1 = b, L2 = c, L3 = a
-              r = fit_tracklet(di >= 0, dd, zd, wd, true, db, zb, wb, ci >= 0, dc, zc, wc, true, da, za, wa, nh, c);
-              key = make_key(nh, r.chi2, pd, (uint32_t)ib, pc, (uint32_t)ia);
-            }
-            if (r.valid && key < best) best = key;
-          }
-          if (!remD) break;
-          di = __ffs(remD) - 1;
-          remD &= remD - 1;
-        }
-        if (!remC) break;
-        ci = __ffs(remC) - 1;
-        remC &= remC - 1;
-      }
-    }
-    ib += 4;
-    while (ib >= nB) { ib -= nB; ++ia; }
-  }
-  return best;
+__host__ __device__ inline size_t warp_area_bytes(int C) {
+  return (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8 + 32 * 4;
 }
 
-template <bool STAGED>
-__device__ __forceinline__ void track_loop(const CompassArgs& a, const float* __restrict__ X,
-                                           const float* __restrict__ YB, const float* __restrict__ YE,
-                                           const float* __restrict__ Z, const float* __restrict__ W,
-                                           const uint32_t* s_goff, const float* s_gdxdy, const float* s_gxmin,
-                                           const float* s_gxmax, const CandView cv, uint32_t a0, uint32_t t0,
-                                           uint32_t t1, uint32_t T) {
-  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
-  const int l = tid & 3;                         // layer of this lane in phase 1, lane-in-quad in phase 2
-  const uint32_t qslot = tid & ~3u, slot = tid;
-  const unsigned qmask = 0xFu << (lane & ~3);
-  const uint32_t gpl = a.gpl;
-  const int C = a.c.max_candidates_per_layer;
-  uint32_t lf[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) lf[k] = s_goff[k * gpl];
-  const uint32_t my_lf = lf[0] * (l == 0) + lf[1] * (l == 1) + lf[2] * (l == 2) + lf[3] * (l == 3);
+// Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
+__device__ __forceinline__ void cand_insert(const WarpArea& wa, int slot, int& n, int C, float d, uint32_t hs) {
+  if (n == C) {
+    int worst = 0;
+    float wabs = fabsf(wa.cd[slot]);
+    uint32_t whs = wa.chs[slot];
+    for (int i = 1; i < C; ++i) {
+      const float v = fabsf(wa.cd[i * 32 + slot]);
+      const uint32_t k = wa.chs[i * 32 + slot];
+      if (v > wabs || (v == wabs && k > whs)) { wabs = v; whs = k; worst = i; }
+    }
+    const float nabs = fabsf(d);
+    if (!(nabs < wabs || (nabs == wabs && hs < whs))) return;
+    for (int i = worst; i < C - 1; ++i) {
+      wa.cd[i * 32 + slot] = wa.cd[(i + 1) * 32 + slot];
+      wa.chs[i * 32 + slot] = wa.chs[(i + 1) * 32 + slot];
+    }
+    n = C - 1;
+  }
+  int i = n;
+  while (i > 0) {
+    const uint32_t k = wa.chs[(i - 1) * 32 + slot];
+    if (k < hs) break;
+    wa.chs[i * 32 + slot] = k;
+    wa.cd[i * 32 + slot] = wa.cd[(i - 1) * 32 + slot];
+    --i;
+  }
+  wa.cd[i * 32 + slot] = d;
+  wa.chs[i * 32 + slot] = hs;
+  ++n;
+}
 
-  for (uint32_t tb = t0; tb < t1; tb += (uint32_t)(nt >> 2)) {
-    const uint32_t tg = tb + (uint32_t)(tid >> 2);
+// ---- phase 1: candidate list of one (track, layer) -------------------------------------
+template <bool BUCKETED>
+__device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, int slot, int l, float x_e,
+                                              float y_e, const uint16_t* __restrict__ s_off,
+                                              const float* __restrict__ s_hx, const uint16_t* __restrict__ s_hh,
+                                              const uint32_t* __restrict__ s_goff, uint32_t h0) {
+  const int C = a.c.max_candidates_per_layer;
+  const float D = a.c.win_half[l], negD = -D, y_tol = a.c.y_tol;
+  const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
+  const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
+  const uint32_t gend = (l + 1) * a.gpl;
+  uint32_t g = l * a.gpl;
+  for (uint32_t cnt = a.gpl; cnt > 0;) {            // first group with group_xmax >= lo
+    const uint32_t half = cnt >> 1, mid = g + half;
+    if (__ldg(a.group_xmax + mid) >= lo) cnt = half; else { g = mid + 1; cnt -= half + 1; }
+  }
+  int n = 0;
+  for (; g < gend && __ldg(a.group_xmin + g) <= hi; ++g) {
+    const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
+    if (ga == gb) continue;
+    const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
+    if (BUCKETED) {
+      uint32_t s = sa;
+      if (a.rows_sorted) {                          // first sector row with y_e <= y_end + y_tol
+        for (uint32_t cnt = sb - sa; cnt > 0;) {
+          const uint32_t half = cnt >> 1, mid = s + half;
+          if (y_e <= __fadd_rn(__ldg(a.sec_ye + mid), y_tol)) cnt = half; else { s = mid + 1; cnt -= half + 1; }
+        }
+      }
+      for (; s < sb; ++s) {
+        const bool in_lo = __fsub_rn(__ldg(a.sec_yb + s), y_tol) <= y_e;
+        if (!in_lo) { if (a.rows_sorted) break; continue; }
+        if (!(y_e <= __fadd_rn(__ldg(a.sec_ye + s), y_tol))) continue;
+        const uint32_t p0 = s_off[s], p1 = s_off[s + 1];
+        if (p0 == p1) continue;
+        const float syg = __fmul_rn(__ldg(a.sec_dxdy + s), y_e);
+        for (uint32_t p = p0; p < p1; ++p) {
+          const float d = __fsub_rn(__fadd_rn(s_hx[p], syg), x_e);
+          if (fabsf(d) <= D) cand_insert(wa, slot, n, C, d, ((uint32_t)s_hh[p] << 16) | s);
+        }
+      }
+    } else {
+      const float syg = __fmul_rn(__ldg(a.sec_dxdy + sa), y_e);      // one stereo angle per group (contract)
+      const float* X = a.hx + h0;
+      uint32_t first = ga;
+      for (uint32_t cnt = gb - ga; cnt > 0;) {      // first hit with d >= -D
+        const uint32_t half = cnt >> 1, mid = first + half;
+        const float d = __fsub_rn(__fadd_rn(__ldg(X + mid), syg), x_e);
+        if (d >= negD) cnt = half; else { first = mid + 1; cnt -= half + 1; }
+      }
+      for (uint32_t h = first; h < gb; ++h) {
+        const float d = __fsub_rn(__fadd_rn(__ldg(X + h), syg), x_e);
+        if (!(d <= D)) break;
+        if (!(__fsub_rn(__ldg(a.hyb + h0 + h), y_tol) <= y_e && y_e <= __fadd_rn(__ldg(a.hye + h0 + h), y_tol))) continue;
+        const uint32_t rid = __ldg(a.hid + h0 + h) >> 9;
+        const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+        if (s >= a.n_sectors) continue;             // reported by the staging pass of the bucketed path only
+        cand_insert(wa, slot, n, C, d, (h << 16) | s);
+      }
+    }
+  }
+  return n;
+}
+
+// ---- phase 2 (b) + (c): `cnt` queued seeds, one per lane, then all their 3/4-hit combinations --------------
+__device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpArea& wa, int lane, int cnt, int qhead,
+                                              int dir) {
+  const int LA = dir ? 3 : 0, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
+  const bool min3 = a.c.min_hits == 3;
+  uint32_t pk = 0, mC = 0, mD = 0, k = 0;
+  if (lane < cnt) {
+    const uint2 sd = wa.seedq[(qhead + lane) & (kSeedQ - 1)];
+    pk = sd.x;
+    const float bs = __uint_as_float(sd.y);
+    const int j4 = (int)(pk >> 10) * 4, ia = (pk >> 5) & 31;
+    const float da = wa.cd[ia * 32 + j4 + LA];
+    const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + j4 + LA] & 0xFFFFu));
+    const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
+    for (int i = 0; i < nC; ++i) {
+      const float dc = wa.cd[i * 32 + j4 + LC];
+      const float zc = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LC] & 0xFFFFu));
+      const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
+      if (fabsf(__fsub_rn(dc, pred)) <= a.c.seed_tol) mC |= 1u << i;
+    }
+    for (int i = 0; i < nD; ++i) {
+      const float dd = wa.cd[i * 32 + j4 + LD];
+      const float zd = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LD] & 0xFFFFu));
+      const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
+      if (fabsf(__fsub_rn(dd, pred)) <= a.c.seed_tol) mD |= 1u << i;
+    }
+    const uint32_t pc = __popc(mC), pd = __popc(mD);
+    k = min3 ? (pc + 1) * (pd + 1) - 1 : pc * pd;   // (c or none) x (d or none) with >= min_hits hits in total
+  }
+  const uint32_t incl = warp_incl_scan(k, lane), excl = incl - k;
+  const uint32_t K = __shfl_sync(0xFFFFFFFFu, incl, 31);
+  for (uint32_t base = 0; base < K; base += 32) {
+    const uint32_t i = base + lane;
+    int q = 0;                                       // owner seed: largest q with excl[q] <= i
+#pragma unroll
+    for (int step = 16; step > 0; step >>= 1) {
+      const uint32_t e = __shfl_sync(0xFFFFFFFFu, excl, q + step);
+      if (e <= i) q += step;
+    }
+    const uint32_t r = i - __shfl_sync(0xFFFFFFFFu, excl, q);
+    const uint32_t pkq = __shfl_sync(0xFFFFFFFFu, pk, q);
+    const uint32_t mCq = __shfl_sync(0xFFFFFFFFu, mC, q), mDq = __shfl_sync(0xFFFFFFFFu, mD, q);
+    if (i < K) {
+      const uint32_t pc = __popc(mCq);
+      uint32_t selC, selD;                           // 0 = none, else 1-based ordinal of the set bit
+      if (min3) { const uint32_t r1 = r + 1, w = pc + 1; selD = r1 / w; selC = r1 - selD * w; }
+      else { selD = r / pc; selC = r - selD * pc + 1; selD += 1; }
+      int ci = -1, di = -1;
+      if (selC) { uint32_t m = mCq; for (uint32_t t = 1; t < selC; ++t) m &= m - 1; ci = __ffs(m) - 1; }
+      if (selD) { uint32_t m = mDq; for (uint32_t t = 1; t < selD; ++t) m &= m - 1; di = __ffs(m) - 1; }
+      const int j = (int)(pkq >> 10), ia = (pkq >> 5) & 31, ib = pkq & 31;
+      int pos[4];                                    // candidate position per layer, -1 = none
+      if (dir == 0) { pos[0] = ia; pos[1] = ci; pos[2] = ib; pos[3] = di; }
+      else { pos[0] = di; pos[1] = ib; pos[2] = ci; pos[3] = ia; }
+      bool pr[4];
+      float d[4], z[4], w[4];
+      int nh = 0;
+#pragma unroll
+      for (int l = 0; l < 4; ++l) {
+        pr[l] = pos[l] >= 0;
+        d[l] = z[l] = w[l] = 0.f;
+        if (pr[l]) {
+          const uint32_t s = wa.chs[pos[l] * 32 + j * 4 + l] & 0xFFFFu;
+          d[l] = wa.cd[pos[l] * 32 + j * 4 + l];
+          z[l] = __ldg(a.sec_z + s);
+          w[l] = __ldg(a.sec_w + s);
+          ++nh;
+        }
+      }
+      const FitResult fr = fit_tracklet(pr, d, z, w, nh, a.c);
+      if (fr.valid)
+        atomicMin(&wa.best[j], make_key(nh, fr.chi2, (uint32_t)pos[0] & 63u, (uint32_t)pos[1] & 63u,
+                                        (uint32_t)pos[2] & 63u, (uint32_t)pos[3] & 63u));
+    }
+  }
+  (void)LA;
+}
+
+template <bool BUCKETED>
+__device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const uint16_t* s_off,
+                                           const float* s_hx, const uint16_t* s_hh, const uint32_t* s_goff,
+                                           int* s_ticket, uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T) {
+  const int lane = threadIdx.x & 31;
+  const int l = lane & 3;                         // layer of this lane in phase 1 and in the output
+  const int j = lane & 7;                         // track-in-batch this lane does the bookkeeping for (lanes 0..7)
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  for (;;) {
+    int batch = 0;
+    if (lane == 0) batch = atomicAdd(s_ticket, 1);
+    batch = __shfl_sync(0xFFFFFFFFu, batch, 0);
+    const uint32_t tb = t0 + (uint32_t)batch * kTPW;
+    if (tb >= t1) break;
+    const uint32_t tg = tb + (uint32_t)(lane >> 2);
     const bool active = tg < t1;
-    // ---------------- phase 1: window search, lane = (track, layer) ----------------
+    // ---------------- phase 1: window search, lane = (track, layer) ---------------------------------------
     int n_st = 0;
     if (active) {
       const float vx = __ldg(a.vx + tg), vy = __ldg(a.vy + tg), vtx = __ldg(a.vtx + tg), vty = __ldg(a.vty + tg);
       const float dzv = __fsub_rn(a.layer_z[l], a.vz);
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
-      const float D = a.c.win_half[l], negD = -D, y_tol = a.c.y_tol;
-      const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
-      const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
-      const uint32_t gend = (l + 1) * gpl;
-      uint32_t g = l * gpl;
-      for (uint32_t cnt = gpl; cnt > 0;) {            // first group with group_xmax >= lo
-        const uint32_t half = cnt >> 1, mid = g + half;
-        if (s_gxmax[mid] >= lo) cnt = half; else { g = mid + 1; cnt -= half + 1; }
-      }
-      int worst = -1;
-      float worst_abs = 0.f;
-      for (; g < gend && s_gxmin[g] <= hi; ++g) {
-        const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
-        if (ga == gb) continue;
-        const float syg = __fmul_rn(s_gdxdy[g], y_e);
-        uint32_t first = ga;
-        for (uint32_t cnt = gb - ga; cnt > 0;) {      // first hit with d >= -D
-          const uint32_t half = cnt >> 1, mid = first + half;
-          const float d = __fsub_rn(__fadd_rn(X[mid], syg), x_e);
-          if (d >= negD) cnt = half; else { first = mid + 1; cnt -= half + 1; }
-        }
-        for (uint32_t h = first; h < gb; ++h) {
-          const float d = __fsub_rn(__fadd_rn(X[h], syg), x_e);
-          if (!(d <= D)) break;
-          if (!(__fsub_rn(YB[h], y_tol) <= y_e && y_e <= __fadd_rn(YE[h], y_tol))) continue;
-          if (n_st < C) {
-            cv.d[n_st * cv.slots + slot] = d;
-            cv.h[n_st * cv.slots + slot] = (uint16_t)(h - my_lf);
-            ++n_st;
-          } else {                                    // keep the C closest in (|d|, h); list stays ascending in h
-            if (worst < 0) {
-              worst = 0; worst_abs = fabsf(cv.d[slot]);
-              for (int i = 1; i < C; ++i) {
-                const float v = fabsf(cv.d[i * cv.slots + slot]);
-                if (v >= worst_abs) { worst_abs = v; worst = i; }
-              }
-            }
-            if (fabsf(d) < worst_abs) {
-              for (int i = worst; i < C - 1; ++i) {
-                cv.d[i * cv.slots + slot] = cv.d[(i + 1) * cv.slots + slot];
-                cv.h[i * cv.slots + slot] = cv.h[(i + 1) * cv.slots + slot];
-              }
-              cv.d[(C - 1) * cv.slots + slot] = d;
-              cv.h[(C - 1) * cv.slots + slot] = (uint16_t)(h - my_lf);
-              worst = -1;
-            }
-          }
-        }
-      }
+      n_st = collect_window<BUCKETED>(a, wa, lane, l, x_e, y_e, s_off, s_hx, s_hh, s_goff, h0);
     }
+    wa.n[lane] = n_st;
+    if (lane < kTPW) wa.best[lane] = kNoKey;
     __syncwarp();
-    // ---------------- phase 2: tracklet finding, 4 lanes per track -----------------
-    int n[4];
+    // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
+    const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
+    uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
+    for (int dir = 0; dir < 2 && todo; ++dir) {   // forward seeds (L0, L2), then backward (L3, L1)
+      const int LA = dir ? 3 : 0, LB = dir ? 1 : 2;
+      const uint32_t nA = wa.n[4 * j + LA], nB = wa.n[4 * j + LB];
+      const uint32_t P = (lane < kTPW && ((todo >> j) & 1u)) ? nA * nB : 0u;
+      const uint32_t rcpB = nB ? (65536u + nB - 1u) / nB : 0u;     // r / nB == (r * rcpB) >> 16 for r < 1024
+      const uint32_t incl = warp_incl_scan(P, lane), excl = incl - P;
+      const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+      int qn = 0, qhead = 0;
+      for (uint32_t base = 0; base < total; base += 32) {
+        const uint32_t i = base + lane;
+        int jj = 0;                               // owner track: largest jj < 8 with excl[jj] <= i
 #pragma unroll
-    for (int k = 0; k < 4; ++k) n[k] = __shfl_sync(0xFFFFFFFFu, n_st, (lane & ~3) + k);
-    const int nonempty = (n[0] > 0) + (n[1] > 0) + (n[2] > 0) + (n[3] > 0);
-    unsigned long long best = kNoKey;
-    if (nonempty >= a.c.min_hits) {
-      best = search_direction<0>(cv, Z, W, qslot, l, n, lf, a.c);
-      best = min(best, __shfl_xor_sync(qmask, best, 1));
-      best = min(best, __shfl_xor_sync(qmask, best, 2));
-      if (best == kNoKey) {                          // backward only if forward found nothing valid (A11)
-        best = search_direction<1>(cv, Z, W, qslot, l, n, lf, a.c);
-        best = min(best, __shfl_xor_sync(qmask, best, 1));
-        best = min(best, __shfl_xor_sync(qmask, best, 2));
+        for (int step = 4; step > 0; step >>= 1) {
+          const uint32_t e = __shfl_sync(0xFFFFFFFFu, excl, jj + step);
+          if (e <= i) jj += step;
+        }
+        const uint32_t r = i - __shfl_sync(0xFFFFFFFFu, excl, jj);
+        const uint32_t nBj = __shfl_sync(0xFFFFFFFFu, nB, jj), rcp = __shfl_sync(0xFFFFFFFFu, rcpB, jj);
+        bool pass = false;
+        uint32_t ia = 0, ib = 0;
+        float bs = 0.f;
+        if (i < total) {
+          ia = (r * rcp) >> 16;
+          ib = r - ia * nBj;
+          const int sA = jj * 4 + LA, sB = jj * 4 + LB;
+          const float da = wa.cd[ia * 32 + sA], db = wa.cd[ib * 32 + sB];
+          const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + sA] & 0xFFFFu));
+          const float zb = __ldg(a.sec_z + (wa.chs[ib * 32 + sB] & 0xFFFFu));
+          bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
+          const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, a.c.z_mag)));
+          pass = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
+        }
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
+        if (pass)
+          wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] =
+              make_uint2(((uint32_t)jj << 10) | (ia << 5) | ib, __float_as_uint(bs));
+        qn += __popc(m);
+        __syncwarp();
+        if (qn >= 32) {
+          process_seeds(a, wa, lane, 32, qhead, dir);
+          qhead += 32;
+          qn -= 32;
+          __syncwarp();
+        }
       }
+      if (qn > 0) process_seeds(a, wa, lane, qn, qhead, dir);
+      __syncwarp();
+      todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);   // backward only if nothing valid (A11)
     }
+    // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
+      const int q4 = lane & ~3;
+      const unsigned long long best = wa.best[lane >> 2];
       int nh = 0, hidx = -1;
       float qop = 0.f, chi2 = 0.f;
       if (best != kNoKey) {
@@ -294,40 +398,37 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const float* __
           pr[k] = pp[k] != 63u;
           d[k] = z[k] = w[k] = 0.f;
           if (pr[k]) {
-            const uint32_t hh = lf[k] + cv.h[pp[k] * cv.slots + qslot + k];
-            d[k] = cv.d[pp[k] * cv.slots + qslot + k]; z[k] = Z[hh]; w[k] = W[hh];
-            if (k == l) hidx = (int)(a0 + hh);
+            const uint32_t hs = wa.chs[pp[k] * 32 + q4 + k];
+            d[k] = wa.cd[pp[k] * 32 + q4 + k];
+            z[k] = __ldg(a.sec_z + (hs & 0xFFFFu));
+            w[k] = __ldg(a.sec_w + (hs & 0xFFFFu));
+            if (k == l) hidx = (int)(h0 + (hs >> 16));
           }
         }
-        const FitResult r = fit_tracklet(pr[0], d[0], z[0], w[0], pr[1], d[1], z[1], w[1], pr[2], d[2], z[2], w[2],
-                                         pr[3], d[3], z[3], w[3], nh, a.c);
+        const FitResult r = fit_tracklet(pr, d, z, w, nh, a.c);
         qop = __fdiv_rn(r.b, a.c.kappa);
       }
       a.out_idx[(size_t)l * T + tg] = hidx;
       if (l == 0) { a.out_n[tg] = nh; a.out_qop[tg] = qop; a.out_chi2[tg] = chi2; }
     }
-    __syncwarp();
+    __syncwarp();                                 // the batch is consumed before its lists are overwritten
   }
 }
 
-__global__ void __launch_bounds__(512) compass_kernel(const CompassArgs a) {
+__global__ void __launch_bounds__(256, 3) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int tid = threadIdx.x, nt = blockDim.x;
-  const uint32_t ng = a.n_groups;
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
+  const uint32_t ng = a.n_groups, ns = a.n_sectors;
+  const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
-  float* s_x = cvr.take<float>(a.hit_stage);
-  float* s_yb = cvr.take<float>(a.hit_stage);
-  float* s_ye = cvr.take<float>(a.hit_stage);
-  float* s_z = cvr.take<float>(a.hit_stage);
-  float* s_w = cvr.take<float>(a.hit_stage);
-  CandView cv;
-  cv.slots = (uint32_t)nt;
-  cv.d = cvr.take<float>((size_t)a.c.max_candidates_per_layer * nt);
-  cv.h = cvr.take<uint16_t>((size_t)a.c.max_candidates_per_layer * nt);
-  uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);
-  float* s_gdxdy = cvr.take<float>(ng);
-  float* s_gxmin = cvr.take<float>(ng);
-  float* s_gxmax = cvr.take<float>(ng);
+  uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);           // group offsets relative to the event's first hit
+  uint16_t* s_off = cvr.take<uint16_t>(ns + 1);            // bucketed position of every sector's first hit
+  float* s_hx = cvr.take<float>(a.hit_stage);
+  uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage);
+  unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by s_cnt below
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp_areas);
+  __shared__ uint32_t s_scan[32];
+  __shared__ int s_ticket;
 
   const int e = blockIdx.x;
   const uint32_t T = __ldg(a.velo_offsets + a.n_events);
@@ -338,22 +439,15 @@ __global__ void __launch_bounds__(512) compass_kernel(const CompassArgs a) {
     if (tid == 0) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_OFFSETS);
     return;
   }
-  const uint32_t a0 = h0 & ~3u;                    // staged arrays start at a 16-byte aligned element
   bool bad = h1 < h0;
   for (uint32_t g = tid; g <= ng; g += nt) {
     const uint32_t o = __ldg(go + g);
-    s_goff[g] = o - a0;
-    if (g < ng) {
-      const uint32_t o1 = __ldg(go + g + 1);
-      bad |= o1 < o;
-      s_gdxdy[g] = (o1 > o) ? __ldg(a.hdxdy + o) : 0.f;
-      s_gxmin[g] = __ldg(a.group_xmin + g);
-      s_gxmax[g] = __ldg(a.group_xmax + g);
-    }
+    s_goff[g] = o - h0;
+    if (g < ng) bad |= __ldg(go + g + 1) < o;
   }
-  uint32_t too_large = 0;
-  if (tid < 4 && !bad) too_large = (__ldg(go + (tid + 1) * a.gpl) - __ldg(go + tid * a.gpl)) > 65535u;
-  const int flag = __syncthreads_or((bad ? 1 : 0) | (too_large ? 2 : 0));
+  if (tid == 0) s_ticket = 0;
+  const uint32_t n = h1 - h0;
+  const int flag = __syncthreads_or((bad ? 1 : 0) | ((!bad && n > 65535u) ? 2 : 0));
   if (flag) {                                      // uniform: report and emit "no tracklet" for every track
     if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
                                          (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u));
@@ -363,17 +457,61 @@ __global__ void __launch_bounds__(512) compass_kernel(const CompassArgs a) {
     }
     return;
   }
-  const uint32_t n_al = h1 - a0;
-  if (n_al <= a.hit_stage) {
-    for (uint32_t i = tid; i < n_al; i += nt) {
-      s_x[i] = __ldg(a.hx + a0 + i); s_yb[i] = __ldg(a.hyb + a0 + i); s_ye[i] = __ldg(a.hye + a0 + i);
-      s_z[i] = __ldg(a.hz + a0 + i); s_w[i] = __ldg(a.hw + a0 + i);
+  if (t1 == t0) return;
+  WarpArea wa;
+  {
+    unsigned char* p = s_warp_areas + (size_t)warp * warp_area_bytes(C);
+    wa.cd = reinterpret_cast<float*>(p);
+    wa.chs = reinterpret_cast<uint32_t*>(p + (size_t)C * 32 * 4);
+    wa.seedq = reinterpret_cast<uint2*>(p + (size_t)C * 32 * 8);
+    wa.best = reinterpret_cast<unsigned long long*>(p + (size_t)C * 32 * 8 + kSeedQ * 8);
+    wa.n = reinterpret_cast<int*>(p + (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8);
+  }
+  if (n <= a.hit_stage) {
+    // ---- stage: re-bucket the event's hits per sector (count, block scan, scatter) ------------------------
+    for (uint32_t s = tid; s < ns; s += nt) s_cnt[s] = 0;
+    __syncthreads();
+    bool bad_id = false;
+    for (uint32_t i = tid; i < n; i += nt) {
+      const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+      const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+      if (s < ns) atomicAdd(&s_cnt[s], 1u); else bad_id = true;
+    }
+    if (bad_id) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_HIT_ID);
+    __syncthreads();
+    {
+      const uint32_t ipt = (ns + nt - 1) / nt;
+      const uint32_t c0 = min(ns, tid * ipt), c1 = min(ns, c0 + ipt);
+      uint32_t sum = 0;
+      for (uint32_t i = c0; i < c1; ++i) sum += s_cnt[i];
+      const uint32_t incl = warp_incl_scan(sum, lane);
+      if (lane == 31) s_scan[warp] = incl;
+      __syncthreads();
+      if (warp == 0) {
+        const uint32_t v = lane < nwarps ? s_scan[lane] : 0u;
+        const uint32_t iv = warp_incl_scan(v, lane);
+        s_scan[lane] = iv - v;
+      }
+      __syncthreads();
+      uint32_t ex = s_scan[warp] + incl - sum;
+      for (uint32_t i = c0; i < c1; ++i) { const uint32_t v = s_cnt[i]; s_cnt[i] = ex; s_off[i] = (uint16_t)ex; ex += v; }
+      if (c1 == ns && c0 < ns) s_off[ns] = (uint16_t)ex;
+      if (ns == 0 && tid == 0) s_off[0] = 0;
     }
     __syncthreads();
-    track_loop<true>(a, s_x, s_yb, s_ye, s_z, s_w, s_goff, s_gdxdy, s_gxmin, s_gxmax, cv, a0, t0, t1, T);
-  } else {                                         // event larger than the staging size: same code on global memory
-    track_loop<false>(a, a.hx + a0, a.hyb + a0, a.hye + a0, a.hz + a0, a.hw + a0, s_goff, s_gdxdy, s_gxmin, s_gxmax,
-                      cv, a0, t0, t1, T);
+    for (uint32_t i = tid; i < n; i += nt) {
+      const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+      const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+      if (s < ns) {
+        const uint32_t p = atomicAdd(&s_cnt[s], 1u);
+        s_hx[p] = __ldg(a.hx + h0 + i);
+        s_hh[p] = (uint16_t)i;
+      }
+    }
+    __syncthreads();                               // s_cnt is dead from here on: the warp areas take its place
+    track_loop<true>(a, wa, s_off, s_hx, s_hh, s_goff, &s_ticket, h0, t0, t1, T);
+  } else {                                         // event larger than the staging size: window search on global memory
+    track_loop<false>(a, wa, s_off, s_hx, s_hh, s_goff, &s_ticket, h0, t0, t1, T);
   }
 }
 
@@ -382,21 +520,22 @@ static int env_int(const char* name, int dflt) {
   return v && *v ? atoi(v) : dflt;
 }
 
-static size_t compass_smem_bytes(uint32_t ng, uint32_t hit_stage, int C, int block) {
-  size_t b = 5 * align16((size_t)hit_stage * 4);
-  b += align16((size_t)C * block * 4) + align16((size_t)C * block * 2);
-  b += align16((ng + 1) * 4) + 3 * align16(ng * 4);
+static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block) {
+  size_t b = align16((ng + 1) * 4) + align16((ns + 1) * 2);
+  b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
+  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)), align16((size_t)ns * 4));
   return b;
 }
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
                        cudaStream_t stream) {
-  static int max_smem = 0;               // largest dynamic size this kernel may ask for
+  static int max_smem = 0, n_sm = 0;     // max_smem = largest dynamic size this kernel may ask for
   if (!max_smem) {
     int dev = 0, optin = 0;
     UTC_CUDA(cudaGetDevice(&dev));
     UTC_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    UTC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     cudaFuncAttributes fa;
     UTC_CUDA(cudaFuncGetAttributes(&fa, compass_kernel));
     const int dyn = optin - (int)fa.sharedSizeBytes;
@@ -405,30 +544,34 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   const ut_geometry* geom = hits->geom;
   CompassArgs a;
-  a.hx = hits->x_at_y0; a.hz = hits->z_at_y0; a.hyb = hits->y_begin; a.hye = hits->y_end; a.hdxdy = hits->dxdy;
-  a.hw = hits->weight; a.hit_offsets = hit_offsets;
+  a.hx = hits->x_at_y0; a.hid = hits->id; a.hyb = hits->y_begin; a.hye = hits->y_end;
+  a.hit_offsets = hit_offsets;
   a.vx = velo->x; a.vy = velo->y; a.vtx = velo->tx; a.vty = velo->ty; a.vz = velo->z;
   a.velo_offsets = velo_offsets; a.n_events = n_events;
-  a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
+  a.n_sectors = geom->n_sectors; a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
+  a.id_table_size = geom->id_table_size; a.rows_sorted = (geom->flags & UT_GEOM_ROWS_SORTED) ? 1u : 0u;
+  a.id_to_sector = geom->id_to_sector; a.group_first_sector = geom->group_first_sector;
   a.group_xmin = geom->group_xmin; a.group_xmax = geom->group_xmax;
+  a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 
+  const int C = cfg->max_candidates_per_layer;
   int block = env_int("UT_COMPASS_BLOCK", 256);
-  block = std::max(32, std::min(512, (block / 32) * 32));
+  block = std::max(32, std::min(256, (block / 32) * 32));
   const unsigned long long avg = hits->capacity / (unsigned long long)n_events + 1;
-  uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 127) / 128) * 128 + 128, 1u << 16);
+  uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 127) / 128) * 128 + 128, 65536ull);
   hit_stage = (uint32_t)env_int("UT_COMPASS_HIT_STAGE", (int)hit_stage);
   const size_t budget = (size_t)max_smem;
-  size_t smem = compass_smem_bytes(geom->n_groups, hit_stage, cfg->max_candidates_per_layer, block);
-  while (smem > budget && block > 128) {            // fewer tracks in flight before giving up staging
-    block -= 64;
-    smem = compass_smem_bytes(geom->n_groups, hit_stage, cfg->max_candidates_per_layer, block);
+  size_t smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
+  while (smem > budget && block > 64) {             // fewer warps before giving up staging
+    block -= 32;
+    smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
   }
   while (smem > budget && hit_stage > 0) {
     hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
-    smem = compass_smem_bytes(geom->n_groups, hit_stage, cfg->max_candidates_per_layer, block);
+    smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
