@@ -158,49 +158,77 @@ __device__ __forceinline__ void cand_insert(const WarpArea& wa, int slot, int& n
   ++n;
 }
 
+// Shared-memory view of one CTA: geometry tables (staged once per CTA) and the current event's hits.
+struct SmemView {
+  const float4* gA;      // [ng]  group: xmin, xmax, dxdy, row-hint base (y_hi of the first sector)
+  const uint2* gB;       // [ng]  group: row-hint scale (float bits), first sector | end sector << 16
+  const float2* yr;      // [ns]  sector: y_begin - y_tol, y_end + y_tol
+  const float2* lay;     // [4]   layer: group-hint base (xmax of the first group), scale
+  const uint32_t* goff;  // [ng + 1] group offsets relative to the event's first hit
+  const uint16_t* off;   // [ns + 1] bucketed position of every sector's first hit
+  const float* hx;       // [hit_stage] x_at_y0, bucketed per sector, x-sorted inside the sector
+  const uint16_t* hh;    // [hit_stage] hit index relative to the event
+};
+
 // ---- phase 1: candidate list of one (track, layer) -------------------------------------
+// Group and sector row are found from a linear guess corrected against the tables (exact lower bound of
+// the same predicates the oracle's search uses; O(1) on a regular layout, any sorted layout works).
 template <bool BUCKETED>
-__device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, int slot, int l, float x_e,
-                                              float y_e, const uint16_t* __restrict__ s_off,
-                                              const float* __restrict__ s_hx, const uint16_t* __restrict__ s_hh,
-                                              const uint32_t* __restrict__ s_goff, uint32_t h0) {
+__device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
+                                              int l, float x_e, float y_e, uint32_t h0) {
   const int C = a.c.max_candidates_per_layer;
-  const float D = a.c.win_half[l], negD = -D, y_tol = a.c.y_tol;
+  const float D = a.c.win_half[l], negD = -D;
   const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
   const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
-  const uint32_t gend = (l + 1) * a.gpl;
-  uint32_t g = l * a.gpl;
-  for (uint32_t cnt = a.gpl; cnt > 0;) {            // first group with group_xmax >= lo
-    const uint32_t half = cnt >> 1, mid = g + half;
-    if (__ldg(a.group_xmax + mid) >= lo) cnt = half; else { g = mid + 1; cnt -= half + 1; }
+  const int g0 = l * (int)a.gpl, g1 = g0 + (int)a.gpl;
+  int g;
+  {                                                 // first group with group_xmax >= lo
+    const float2 hint = S.lay[l];
+    const int guess = (int)ceilf((lo - hint.x) * hint.y);
+    g = g0 + max(0, min(guess, (int)a.gpl - 1));
+    while (g > g0 && lo <= S.gA[g - 1].y) --g;
+    while (g < g1 && !(lo <= S.gA[g].y)) ++g;
   }
   int n = 0;
-  for (; g < gend && __ldg(a.group_xmin + g) <= hi; ++g) {
-    const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
+  uint32_t last = 0;
+  for (; g < g1; ++g) {
+    const float4 grp = S.gA[g];
+    if (!(grp.x <= hi)) break;
+    const uint32_t ga = S.goff[g], gb = S.goff[g + 1];
     if (ga == gb) continue;
-    const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
+    const float syg = __fmul_rn(grp.z, y_e);        // one stereo angle per group (container contract)
     if (BUCKETED) {
-      uint32_t s = sa;
+      const uint2 gi = S.gB[g];
+      const int sa = (int)(gi.y & 0xFFFFu), sb = (int)(gi.y >> 16);
+      int s = sa;
       if (a.rows_sorted) {                          // first sector row with y_e <= y_end + y_tol
-        for (uint32_t cnt = sb - sa; cnt > 0;) {
-          const uint32_t half = cnt >> 1, mid = s + half;
-          if (y_e <= __fadd_rn(__ldg(a.sec_ye + mid), y_tol)) cnt = half; else { s = mid + 1; cnt -= half + 1; }
-        }
+        const int guess = (int)ceilf((y_e - grp.w) * __uint_as_float(gi.x));
+        s = sa + max(0, min(guess, sb - sa - 1));
+        while (s > sa && y_e <= S.yr[s - 1].y) --s;
+        while (s < sb && !(y_e <= S.yr[s].y)) ++s;
       }
       for (; s < sb; ++s) {
-        const bool in_lo = __fsub_rn(__ldg(a.sec_yb + s), y_tol) <= y_e;
-        if (!in_lo) { if (a.rows_sorted) break; continue; }
-        if (!(y_e <= __fadd_rn(__ldg(a.sec_ye + s), y_tol))) continue;
-        const uint32_t p0 = s_off[s], p1 = s_off[s + 1];
-        if (p0 == p1) continue;
-        const float syg = __fmul_rn(__ldg(a.sec_dxdy + s), y_e);
-        for (uint32_t p = p0; p < p1; ++p) {
-          const float d = __fsub_rn(__fadd_rn(s_hx[p], syg), x_e);
-          if (fabsf(d) <= D) cand_insert(wa, slot, n, C, d, ((uint32_t)s_hh[p] << 16) | s);
+        const float2 yr = S.yr[s];
+        if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
+        if (!(y_e <= yr.y)) continue;
+        const uint32_t p1 = S.off[s + 1];
+        for (uint32_t p = S.off[s]; p < p1; ++p) {
+          const float d = __fsub_rn(__fadd_rn(S.hx[p], syg), x_e);
+          if (fabsf(d) <= D) {
+            const uint32_t hs = ((uint32_t)S.hh[p] << 16) | (uint32_t)s;
+            if (n < C && (n == 0 || last < hs)) {   // hits arrive in ascending index almost always: append
+              wa.cd[n * 32 + slot] = d;
+              wa.chs[n * 32 + slot] = hs;
+              last = hs;
+              ++n;
+            } else {
+              cand_insert(wa, slot, n, C, d, hs);
+              last = wa.chs[(n - 1) * 32 + slot];
+            }
+          }
         }
       }
     } else {
-      const float syg = __fmul_rn(__ldg(a.sec_dxdy + sa), y_e);      // one stereo angle per group (contract)
       const float* X = a.hx + h0;
       uint32_t first = ga;
       for (uint32_t cnt = gb - ga; cnt > 0;) {      // first hit with d >= -D
@@ -211,7 +239,8 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
       for (uint32_t h = first; h < gb; ++h) {
         const float d = __fsub_rn(__fadd_rn(__ldg(X + h), syg), x_e);
         if (!(d <= D)) break;
-        if (!(__fsub_rn(__ldg(a.hyb + h0 + h), y_tol) <= y_e && y_e <= __fadd_rn(__ldg(a.hye + h0 + h), y_tol))) continue;
+        if (!(__fsub_rn(__ldg(a.hyb + h0 + h), a.c.y_tol) <= y_e && y_e <= __fadd_rn(__ldg(a.hye + h0 + h), a.c.y_tol)))
+          continue;
         const uint32_t rid = __ldg(a.hid + h0 + h) >> 9;
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;             // reported by the staging pass of the bucketed path only
@@ -301,9 +330,8 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 }
 
 template <bool BUCKETED>
-__device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const uint16_t* s_off,
-                                           const float* s_hx, const uint16_t* s_hh, const uint32_t* s_goff,
-                                           int* s_ticket, uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T) {
+__device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
+                                           uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T) {
   const int lane = threadIdx.x & 31;
   const int l = lane & 3;                         // layer of this lane in phase 1 and in the output
   const int j = lane & 7;                         // track-in-batch this lane does the bookkeeping for (lanes 0..7)
@@ -323,7 +351,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       const float dzv = __fsub_rn(a.layer_z[l], a.vz);
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
-      n_st = collect_window<BUCKETED>(a, wa, lane, l, x_e, y_e, s_off, s_hx, s_hh, s_goff, h0);
+      n_st = collect_window<BUCKETED>(a, wa, S, lane, l, x_e, y_e, h0);
     }
     wa.n[lane] = n_st;
     if (lane < kTPW) wa.best[lane] = kNoKey;
@@ -415,49 +443,44 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
   }
 }
 
-__global__ void __launch_bounds__(256, 3) compass_kernel(const CompassArgs a) {
+// One CTA works through events blockIdx.x, blockIdx.x + gridDim.x, ...  Geometry tables are staged once.
+template <int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
   const uint32_t ng = a.n_groups, ns = a.n_sectors;
   const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
-  uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);           // group offsets relative to the event's first hit
-  uint16_t* s_off = cvr.take<uint16_t>(ns + 1);            // bucketed position of every sector's first hit
+  float4* s_gA = cvr.take<float4>(ng);
+  uint2* s_gB = cvr.take<uint2>(ng);
+  float2* s_yr = cvr.take<float2>(ns);
+  uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);
+  uint16_t* s_off = cvr.take<uint16_t>(ns + 1);
   float* s_hx = cvr.take<float>(a.hit_stage);
   uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage);
   unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by s_cnt below
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp_areas);
-  __shared__ uint32_t s_scan[32];
+  __shared__ float2 s_lay[4];
   __shared__ int s_ticket;
+  const uint32_t lt_mask = (1u << lane) - 1u;
 
-  const int e = blockIdx.x;
-  const uint32_t T = __ldg(a.velo_offsets + a.n_events);
-  const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
-  const uint32_t* go = a.hit_offsets + (size_t)e * ng;
-  const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
-  if (t1 < t0 || t1 > T) {                         // inconsistent VELO offsets: nothing can be written safely
-    if (tid == 0) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_OFFSETS);
-    return;
+  // ---- geometry tables, once per CTA ---------------------------------------------------------------------
+  for (uint32_t s = tid; s < ns; s += nt)
+    s_yr[s] = make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
+  for (uint32_t g = tid; g < ng; g += nt) {
+    const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
+    const float y0 = __fadd_rn(__ldg(a.sec_ye + sa), a.c.y_tol), y1 = __fadd_rn(__ldg(a.sec_ye + sb - 1), a.c.y_tol);
+    const float inv = (sb - sa > 1 && y1 > y0) ? (float)(sb - sa - 1) / (y1 - y0) : 0.f;
+    s_gA[g] = make_float4(__ldg(a.group_xmin + g), __ldg(a.group_xmax + g), __ldg(a.sec_dxdy + sa), y0);
+    s_gB[g] = make_uint2(__float_as_uint(inv), sa | (sb << 16));
   }
-  bool bad = h1 < h0;
-  for (uint32_t g = tid; g <= ng; g += nt) {
-    const uint32_t o = __ldg(go + g);
-    s_goff[g] = o - h0;
-    if (g < ng) bad |= __ldg(go + g + 1) < o;
+  if (tid < 4) {
+    const uint32_t ga = tid * a.gpl, gb = ga + a.gpl;
+    const float x0 = __ldg(a.group_xmax + ga), x1 = __ldg(a.group_xmax + gb - 1);
+    s_lay[tid] = make_float2(x0, (a.gpl > 1 && x1 > x0) ? (float)(a.gpl - 1) / (x1 - x0) : 0.f);
   }
-  if (tid == 0) s_ticket = 0;
-  const uint32_t n = h1 - h0;
-  const int flag = __syncthreads_or((bad ? 1 : 0) | ((!bad && n > 65535u) ? 2 : 0));
-  if (flag) {                                      // uniform: report and emit "no tracklet" for every track
-    if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
-                                         (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u));
-    for (uint32_t t = t0 + tid; t < t1; t += nt) {
-      for (int k = 0; k < 4; ++k) a.out_idx[(size_t)k * T + t] = -1;
-      a.out_n[t] = 0; a.out_qop[t] = 0.f; a.out_chi2[t] = 0.f;
-    }
-    return;
-  }
-  if (t1 == t0) return;
+  SmemView S;
+  S.gA = s_gA; S.gB = s_gB; S.yr = s_yr; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
   WarpArea wa;
   {
     unsigned char* p = s_warp_areas + (size_t)warp * warp_area_bytes(C);
@@ -467,51 +490,89 @@ __global__ void __launch_bounds__(256, 3) compass_kernel(const CompassArgs a) {
     wa.best = reinterpret_cast<unsigned long long*>(p + (size_t)C * 32 * 8 + kSeedQ * 8);
     wa.n = reinterpret_cast<int*>(p + (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8);
   }
-  if (n <= a.hit_stage) {
-    // ---- stage: re-bucket the event's hits per sector (count, block scan, scatter) ------------------------
-    for (uint32_t s = tid; s < ns; s += nt) s_cnt[s] = 0;
-    __syncthreads();
-    bool bad_id = false;
-    for (uint32_t i = tid; i < n; i += nt) {
-      const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
-      const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
-      if (s < ns) atomicAdd(&s_cnt[s], 1u); else bad_id = true;
+  const uint32_t T = __ldg(a.velo_offsets + a.n_events);
+
+  for (int e = blockIdx.x; e < a.n_events; e += gridDim.x) {
+    __syncthreads();                               // tables staged / previous event fully consumed
+    const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
+    const uint32_t* go = a.hit_offsets + (size_t)e * ng;
+    const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
+    if (t1 < t0 || t1 > T) {                       // inconsistent VELO offsets: nothing can be written safely
+      if (tid == 0) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_OFFSETS);
+      continue;
     }
-    if (bad_id) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_HIT_ID);
-    __syncthreads();
-    {
-      const uint32_t ipt = (ns + nt - 1) / nt;
-      const uint32_t c0 = min(ns, tid * ipt), c1 = min(ns, c0 + ipt);
-      uint32_t sum = 0;
-      for (uint32_t i = c0; i < c1; ++i) sum += s_cnt[i];
-      const uint32_t incl = warp_incl_scan(sum, lane);
-      if (lane == 31) s_scan[warp] = incl;
-      __syncthreads();
-      if (warp == 0) {
-        const uint32_t v = lane < nwarps ? s_scan[lane] : 0u;
-        const uint32_t iv = warp_incl_scan(v, lane);
-        s_scan[lane] = iv - v;
+    bool bad = h1 < h0;
+    for (uint32_t g = tid; g <= ng; g += nt) {
+      const uint32_t o = __ldg(go + g);
+      s_goff[g] = o - h0;
+      if (g < ng) bad |= __ldg(go + g + 1) < o;
+    }
+    if (tid == 0) s_ticket = 0;
+    const uint32_t n = h1 - h0;
+    const int flag = __syncthreads_or((bad ? 1 : 0) | ((!bad && n > 65535u) ? 2 : 0));
+    if (flag) {                                    // uniform: report and emit "no tracklet" for every track
+      if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
+                                           (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u));
+      for (uint32_t t = t0 + tid; t < t1; t += nt) {
+        for (int k = 0; k < 4; ++k) a.out_idx[(size_t)k * T + t] = -1;
+        a.out_n[t] = 0; a.out_qop[t] = 0.f; a.out_chi2[t] = 0.f;
       }
-      __syncthreads();
-      uint32_t ex = s_scan[warp] + incl - sum;
-      for (uint32_t i = c0; i < c1; ++i) { const uint32_t v = s_cnt[i]; s_cnt[i] = ex; s_off[i] = (uint16_t)ex; ex += v; }
-      if (c1 == ns && c0 < ns) s_off[ns] = (uint16_t)ex;
-      if (ns == 0 && tid == 0) s_off[0] = 0;
+      continue;
     }
-    __syncthreads();
-    for (uint32_t i = tid; i < n; i += nt) {
-      const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
-      const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
-      if (s < ns) {
-        const uint32_t p = atomicAdd(&s_cnt[s], 1u);
-        s_hx[p] = __ldg(a.hx + h0 + i);
-        s_hh[p] = (uint16_t)i;
+    if (t1 == t0) continue;
+    if (n <= a.hit_stage) {
+      // ---- stage: a warp re-buckets one sector group at a time, per sector, keeping the x order -----------
+      // (count -> warp scan over the group's sectors -> ordered scatter with match.any; no block barrier)
+      bool bad_id = false;
+      for (uint32_t g = warp; g < ng; g += nwarps) {
+        const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
+        const uint32_t sa = s_gB[g].y & 0xFFFFu, sb = s_gB[g].y >> 16;
+        for (uint32_t s = sa + lane; s < sb; s += 32) s_cnt[s] = 0;
+        __syncwarp();
+        for (uint32_t i = ga + lane; i < gb; i += 32) {
+          const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+          const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+          if (s >= sa && s < sb) atomicAdd(&s_cnt[s], 1u); else bad_id = true;
+        }
+        __syncwarp();
+        uint32_t run = ga;
+        for (uint32_t s0 = sa; s0 < sb; s0 += 32) {
+          const uint32_t s = s0 + lane;
+          const uint32_t c = s < sb ? s_cnt[s] : 0u;
+          const uint32_t incl = warp_incl_scan(c, lane);
+          if (s < sb) { s_off[s] = (uint16_t)(run + incl - c); s_cnt[s] = run + incl - c; }
+          run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+        }
+        if (g == ng - 1 && lane == 0) s_off[ns] = (uint16_t)n;
+        __syncwarp();
+        for (uint32_t i0 = ga; i0 < gb; i0 += 32) {
+          const uint32_t i = i0 + lane;
+          uint32_t s = kInvalid;
+          float x = 0.f;
+          if (i < gb) {
+            const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+            s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+            if (!(s >= sa && s < sb)) s = kInvalid;
+            x = __ldg(a.hx + h0 + i);
+          }
+          const uint32_t peers = __match_any_sync(0xFFFFFFFFu, s);
+          const uint32_t rank = __popc(peers & lt_mask);
+          if (s != kInvalid) {
+            const uint32_t p = s_cnt[s] + rank;
+            s_hx[p] = x;
+            s_hh[p] = (uint16_t)i;
+          }
+          __syncwarp();
+          if (s != kInvalid && rank == 0) s_cnt[s] += __popc(peers);
+          __syncwarp();
+        }
       }
+      if (bad_id) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_HIT_ID);
+      __syncthreads();                             // s_cnt is dead from here on: the warp areas take its place
+      track_loop<true>(a, wa, S, &s_ticket, h0, t0, t1, T);
+    } else {                                       // event larger than the staging size: window search on global memory
+      track_loop<false>(a, wa, S, &s_ticket, h0, t0, t1, T);
     }
-    __syncthreads();                               // s_cnt is dead from here on: the warp areas take its place
-    track_loop<true>(a, wa, s_off, s_hx, s_hh, s_goff, &s_ticket, h0, t0, t1, T);
-  } else {                                         // event larger than the staging size: window search on global memory
-    track_loop<false>(a, wa, s_off, s_hx, s_hh, s_goff, &s_ticket, h0, t0, t1, T);
   }
 }
 
@@ -521,25 +582,33 @@ static int env_int(const char* name, int dflt) {
 }
 
 static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block) {
-  size_t b = align16((ng + 1) * 4) + align16((ns + 1) * 2);
+  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + align16((size_t)ns * 8);
+  b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
   b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
   b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)), align16((size_t)ns * 4));
   return b;
 }
 
+// Two register budgets: CTAs of <= 256 threads at >= 3 per SM, and larger CTAs (big events / C = 32,
+// where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
+static const void* const kKernelSmall = reinterpret_cast<const void*>(&compass_kernel<256, 3>);
+static const void* const kKernelLarge = reinterpret_cast<const void*>(&compass_kernel<768, 1>);
+
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
                        cudaStream_t stream) {
-  static int max_smem = 0, n_sm = 0;     // max_smem = largest dynamic size this kernel may ask for
+  static int max_smem = 0, n_sm = 0, sm_smem = 0;     // max_smem = largest dynamic size a CTA may ask for
   if (!max_smem) {
     int dev = 0, optin = 0;
     UTC_CUDA(cudaGetDevice(&dev));
     UTC_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     UTC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    UTC_CUDA(cudaDeviceGetAttribute(&sm_smem, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
     cudaFuncAttributes fa;
-    UTC_CUDA(cudaFuncGetAttributes(&fa, compass_kernel));
+    UTC_CUDA(cudaFuncGetAttributes(&fa, kKernelSmall));
     const int dyn = optin - (int)fa.sharedSizeBytes;
-    UTC_CUDA(cudaFuncSetAttribute(compass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    UTC_CUDA(cudaFuncSetAttribute(kKernelSmall, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    UTC_CUDA(cudaFuncSetAttribute(kKernelLarge, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
     max_smem = dyn;
   }
   const ut_geometry* geom = hits->geom;
@@ -558,27 +627,47 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 
   const int C = cfg->max_candidates_per_layer;
-  int block = env_int("UT_COMPASS_BLOCK", 256);
-  block = std::max(32, std::min(256, (block / 32) * 32));
+  const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
   const unsigned long long avg = hits->capacity / (unsigned long long)n_events + 1;
   uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 127) / 128) * 128 + 128, 65536ull);
   hit_stage = (uint32_t)env_int("UT_COMPASS_HIT_STAGE", (int)hit_stage);
   const size_t budget = (size_t)max_smem;
-  size_t smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
+  // Block size: the one that keeps the most warps resident per SM (shared memory is the limit; about 24
+  // warps per SM is what the register budget of the small variant allows).
+  int block = env_int("UT_COMPASS_BLOCK", 0);
+  if (block <= 0) {
+    int best_warps = -1;
+    for (int b = 192; b <= 768; b += 64) {
+      const size_t sm = compass_smem_bytes(ns, ng, hit_stage, C, b) + 1024;
+      if (sm > budget) continue;
+      const int regs_warps = b <= 256 ? 24 : 21;
+      const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
+      const int warps = ctas * (b / 32);
+      if (warps > best_warps) { best_warps = warps; block = b; }
+    }
+    if (block <= 0) block = 192;
+  }
+  block = std::max(32, std::min(768, (block / 32) * 32));
+  size_t smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
   while (smem > budget && block > 64) {             // fewer warps before giving up staging
     block -= 32;
-    smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
   }
   while (smem > budget && hit_stage > 0) {
     hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
-    smem = compass_smem_bytes(geom->n_sectors, geom->n_groups, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  compass_kernel<<<n_events, block, smem, stream>>>(a);
-  UTC_CUDA(cudaGetLastError());
+  const void* kernel = block <= 256 ? kKernelSmall : kKernelLarge;
+  int per_sm = 0;
+  UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
+  if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);
+  const int grid = std::max(1, std::min(n_events, n_sm * per_sm));
+  void* params[] = {&a};
+  UTC_CUDA(cudaLaunchKernel(kernel, dim3(grid), dim3(block), params, smem, stream));
   ut_launch_info& li = launch_info();
-  li.kernels_launched = 1; li.compass_grid = n_events; li.compass_block = block; li.compass_smem_bytes = (int)smem;
+  li.kernels_launched = 1; li.compass_grid = grid; li.compass_block = block; li.compass_smem_bytes = (int)smem;
   li.compass_hit_stage = (int)hit_stage;
   return UT_OK;
 }
