@@ -182,6 +182,78 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args, local_rank):
+    """--sweep: BASELINE.json configs[4] -- 10000 events of the config-2 distribution, Compass run with
+    {min_hits 3, 4} x {window scale 0.5, 1, 2} x {max_candidates_per_layer 8, 16, 32}; per setting
+    events/s (decode + Compass, L2 flushed between steps) with efficiency and ghost rate of the GPU
+    tracklets against the generator truth (synth/truth.py)."""
+    import synth
+    from synth.configs import SWEEP_MIN_HITS, SWEEP_SCALE, SWEEP_CANDIDATES
+    cfg = synth.CONFIGS[5]
+    n_events = args.events or cfg.n_events
+    geom_t, batch, _ = synth.make_workload(5, n_events=n_events, workers=min(8, os.cpu_count() or 1))
+    import torch
+    import __graft_entry__ as entry
+    entry.build()
+    torch.cuda.set_device(local_rank)
+    from paper_2002_11529_b200 import binding as B
+    dev = torch.device("cuda", local_rank)
+    geom = B.ut_geometry_upload(geom_t)
+    hits = B.Hits(batch.hit_capacity, batch.n_events, geom)
+    raw_d, bo_d = B.to_device_raw(batch.raw), B.to_device_u32(batch.bank_offsets)
+    velo = B.VeloStates(batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z)
+    vo_d = B.to_device_u32(batch.velo_offsets)
+    tracks = B.Tracks(batch.n_velo_total)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    steps = max(3, min(args.steps, 20))
+    rows = []
+    for mh in SWEEP_MIN_HITS:
+        for sc in SWEEP_SCALE:
+            for C in SWEEP_CANDIDATES:
+                params = cfg.compass_params(min_hits=mh, window_scale=sc, max_candidates_per_layer=C)
+                config = B.make_config(params)
+                for _ in range(3):
+                    flush.zero_()
+                    B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
+                    B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
+                ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+                torch.cuda.synchronize()
+                for k in range(steps):
+                    flush.zero_()
+                    ev[k][0].record(stream)
+                    B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
+                    ev[k][1].record(stream)
+                    B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
+                    ev[k][2].record(stream)
+                torch.cuda.synchronize()
+                md = statistics.mean(e[0].elapsed_time(e[1]) for e in ev)
+                mc = statistics.mean(e[1].elapsed_time(e[2]) for e in ev)
+                idx, nh, qop, _chi2 = tracks.numpy()
+                n_hits = int(hits.hit_offsets[batch.n_events * geom.n_groups].item()) & 0xFFFFFFFF
+                ids = hits.id[:n_hits].cpu().numpy().view(np.uint32)
+                m = synth.physics_metrics(batch.truth_hit_id, batch.truth_q, ids, idx, nh, qop)
+                rows.append({"min_hits": mh, "window_scale": sc, "max_candidates_per_layer": C,
+                             "events_per_s": batch.n_events / (md + mc) * 1e3,
+                             "tracking_only_events_per_s": batch.n_events / mc * 1e3,
+                             "ms_decode": md, "ms_compass": mc, "efficiency": m["efficiency"],
+                             "ghost_rate": m["ghost_rate"], "charge_ok": m["charge_ok"],
+                             "four_hit_fraction": m["four_hit_fraction"], "n_tracklets": m["n_tracklets"],
+                             "n_reconstructible": m["n_reconstructible"],
+                             "status_word": (int(hits.status.item()) | int(tracks.status.item())) & 0xFFFFFFFF})
+    base = next(r for r in rows if (r["min_hits"], r["window_scale"], r["max_candidates_per_layer"]) == (3, 1.0, 16))
+    line = {"metric": METRIC, "value": base["events_per_s"], "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": 3,
+            "ms_per_step": base["ms_decode"] + base["ms_compass"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "events_per_gpu": batch.n_events, "velo_tracks": batch.n_velo_total,
+                       "l2": "flushed (256 MiB memset) between timed steps",
+                       "note": "value = the (min_hits 3, scale 1.0, C 16) row; efficiency / ghost rate against the "
+                               "generator truth (PAPER.md:199-215); absolute values are not comparable with the "
+                               "paper's Table 3 (synthetic events)"},
+            "gpu_launches": 2 * steps * len(rows), "sweep": rows}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -189,6 +261,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args, local_rank)
         return
 
     import synth
