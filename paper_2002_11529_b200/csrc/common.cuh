@@ -121,6 +121,9 @@ struct Carver {
 
 #endif  // __CUDACC__
 
+#ifdef __CUDACC__
+__host__ __device__
+#endif
 inline size_t align16(size_t v) { return (v + 15) & ~size_t(15); }
 
 }  // namespace utc

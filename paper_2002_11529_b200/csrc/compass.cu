@@ -256,27 +256,41 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
                                               int dir) {
   const int LA = dir ? 3 : 0, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
   const bool min3 = a.c.min_hits == 3;
+  // (b) compatible hits of every seed as bit masks: 4 lanes share one seed (8 seeds per round), each lane
+  //     tests every 4th hit of the two other layers; the masks end up in lane = seed index
   uint32_t pk = 0, mC = 0, mD = 0, k = 0;
+  if (lane < cnt) pk = wa.seedq[(qhead + lane) & (kSeedQ - 1)].x;
+  const int sub = lane & 3;
+  for (int r0 = 0; r0 < cnt; r0 += 8) {
+    const int q = r0 + (lane >> 2);
+    uint32_t pC = 0, pD = 0;
+    if (q < cnt) {
+      const uint2 sd = wa.seedq[(qhead + q) & (kSeedQ - 1)];
+      const float bs = __uint_as_float(sd.y);
+      const int j4 = (int)(sd.x >> 10) * 4, ia = (sd.x >> 5) & 31;
+      const float da = wa.cd[ia * 32 + j4 + LA];
+      const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + j4 + LA] & 0xFFFFu));
+      const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
+      for (int i = sub; i < nC; i += 4) {
+        const float dc = wa.cd[i * 32 + j4 + LC];
+        const float zc = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LC] & 0xFFFFu));
+        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
+        if (fabsf(__fsub_rn(dc, pred)) <= a.c.seed_tol) pC |= 1u << i;
+      }
+      for (int i = sub; i < nD; i += 4) {
+        const float dd = wa.cd[i * 32 + j4 + LD];
+        const float zd = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LD] & 0xFFFFu));
+        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
+        if (fabsf(__fsub_rn(dd, pred)) <= a.c.seed_tol) pD |= 1u << i;
+      }
+    }
+    pC |= __shfl_xor_sync(0xFFFFFFFFu, pC, 1); pC |= __shfl_xor_sync(0xFFFFFFFFu, pC, 2);
+    pD |= __shfl_xor_sync(0xFFFFFFFFu, pD, 1); pD |= __shfl_xor_sync(0xFFFFFFFFu, pD, 2);
+    const int src = ((lane - r0) & 7) * 4;               // lanes r0 .. r0+7 pick up the masks of their seed
+    const uint32_t gC = __shfl_sync(0xFFFFFFFFu, pC, src), gD = __shfl_sync(0xFFFFFFFFu, pD, src);
+    if (lane >= r0 && lane < r0 + 8) { mC = gC; mD = gD; }
+  }
   if (lane < cnt) {
-    const uint2 sd = wa.seedq[(qhead + lane) & (kSeedQ - 1)];
-    pk = sd.x;
-    const float bs = __uint_as_float(sd.y);
-    const int j4 = (int)(pk >> 10) * 4, ia = (pk >> 5) & 31;
-    const float da = wa.cd[ia * 32 + j4 + LA];
-    const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + j4 + LA] & 0xFFFFu));
-    const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
-    for (int i = 0; i < nC; ++i) {
-      const float dc = wa.cd[i * 32 + j4 + LC];
-      const float zc = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LC] & 0xFFFFu));
-      const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
-      if (fabsf(__fsub_rn(dc, pred)) <= a.c.seed_tol) mC |= 1u << i;
-    }
-    for (int i = 0; i < nD; ++i) {
-      const float dd = wa.cd[i * 32 + j4 + LD];
-      const float zd = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LD] & 0xFFFFu));
-      const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
-      if (fabsf(__fsub_rn(dd, pred)) <= a.c.seed_tol) mD |= 1u << i;
-    }
     const uint32_t pc = __popc(mC), pd = __popc(mD);
     k = min3 ? (pc + 1) * (pd + 1) - 1 : pc * pd;   // (c or none) x (d or none) with >= min_hits hits in total
   }
@@ -362,8 +376,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     for (int dir = 0; dir < 2 && todo; ++dir) {   // forward seeds (L0, L2), then backward (L3, L1)
       const int LA = dir ? 3 : 0, LB = dir ? 1 : 2;
       const uint32_t nA = wa.n[4 * j + LA], nB = wa.n[4 * j + LB];
-      const uint32_t P = (lane < kTPW && ((todo >> j) & 1u)) ? nA * nB : 0u;
-      const uint32_t rcpB = nB ? (65536u + nB - 1u) / nB : 0u;     // r / nB == (r * rcpB) >> 16 for r < 1024
+      // rows (track, hit a) of the batch, one per lane; the lane walks the partner hits b of its row
+      const uint32_t P = (lane < kTPW && ((todo >> j) & 1u) && nB > 0u) ? nA : 0u;
       const uint32_t incl = warp_incl_scan(P, lane), excl = incl - P;
       const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
       int qn = 0, qhead = 0;
@@ -375,33 +389,41 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
           const uint32_t e = __shfl_sync(0xFFFFFFFFu, excl, jj + step);
           if (e <= i) jj += step;
         }
-        const uint32_t r = i - __shfl_sync(0xFFFFFFFFu, excl, jj);
-        const uint32_t nBj = __shfl_sync(0xFFFFFFFFu, nB, jj), rcp = __shfl_sync(0xFFFFFFFFu, rcpB, jj);
-        bool pass = false;
-        uint32_t ia = 0, ib = 0;
-        float bs = 0.f;
+        const uint32_t ia = i - __shfl_sync(0xFFFFFFFFu, excl, jj);
+        int nBj = (int)__shfl_sync(0xFFFFFFFFu, nB, jj);
+        const int sA = jj * 4 + LA, sB = jj * 4 + LB;
+        float da = 0.f, za = 0.f, zam = 0.f;
         if (i < total) {
-          ia = (r * rcp) >> 16;
-          ib = r - ia * nBj;
-          const int sA = jj * 4 + LA, sB = jj * 4 + LB;
-          const float da = wa.cd[ia * 32 + sA], db = wa.cd[ib * 32 + sB];
-          const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + sA] & 0xFFFFu));
-          const float zb = __ldg(a.sec_z + (wa.chs[ib * 32 + sB] & 0xFFFFu));
-          bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
-          const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, a.c.z_mag)));
-          pass = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
+          da = wa.cd[ia * 32 + sA];
+          za = __ldg(a.sec_z + (wa.chs[ia * 32 + sA] & 0xFFFFu));
+          zam = __fsub_rn(za, a.c.z_mag);
+        } else {
+          nBj = 0;
         }
-        const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
-        if (pass)
-          wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] =
-              make_uint2(((uint32_t)jj << 10) | (ia << 5) | ib, __float_as_uint(bs));
-        qn += __popc(m);
-        __syncwarp();
-        if (qn >= 32) {
-          process_seeds(a, wa, lane, 32, qhead, dir);
-          qhead += 32;
-          qn -= 32;
+        const int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+        for (int ib = 0; ib < maxB; ++ib) {
+          bool pass = false;
+          float bs = 0.f;
+          if (ib < nBj) {
+            const float db = wa.cd[ib * 32 + sB];
+            const float zb = __ldg(a.sec_z + (wa.chs[ib * 32 + sB] & 0xFFFFu));
+            bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
+            const float a0 = __fsub_rn(da, __fmul_rn(bs, zam));
+            pass = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
+          }
+          const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
+          if (m == 0u) continue;
+          if (pass)
+            wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] =
+                make_uint2(((uint32_t)jj << 10) | (ia << 5) | (uint32_t)ib, __float_as_uint(bs));
+          qn += __popc(m);
           __syncwarp();
+          if (qn >= 32) {
+            process_seeds(a, wa, lane, 32, qhead, dir);
+            qhead += 32;
+            qn -= 32;
+            __syncwarp();
+          }
         }
       }
       if (qn > 0) process_seeds(a, wa, lane, qn, qhead, dir);
@@ -527,6 +549,49 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       for (uint32_t g = warp; g < ng; g += nwarps) {
         const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
         const uint32_t sa = s_gB[g].y & 0xFFFFu, sb = s_gB[g].y >> 16;
+        if (g == ng - 1 && lane == 0) s_off[ns] = (uint16_t)n;
+        if (gb - ga <= 64u && sb - sa <= 32u) {
+          // one pass, <= 2 hits per lane: rank among the lanes of the same sector (match.any keeps the x
+          // order), per-sector counts through shared memory, exclusive scan over the group's sectors
+          uint32_t* cntA = s_cnt;
+          uint32_t* cntB = s_cnt + ns;
+          if (sa + lane < sb) { cntA[sa + lane] = 0; cntB[sa + lane] = 0; }
+          const uint32_t i0 = ga + lane, i1 = i0 + 32u;
+          uint32_t sec0 = kInvalid, sec1 = kInvalid;
+          float x0 = 0.f, x1 = 0.f;
+          if (i0 < gb) {
+            const uint32_t rid = __ldg(a.hid + h0 + i0) >> 9;
+            sec0 = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+            if (!(sec0 >= sa && sec0 < sb)) { sec0 = kInvalid; bad_id = true; }
+            x0 = __ldg(a.hx + h0 + i0);
+          }
+          if (i1 < gb) {
+            const uint32_t rid = __ldg(a.hid + h0 + i1) >> 9;
+            sec1 = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+            if (!(sec1 >= sa && sec1 < sb)) { sec1 = kInvalid; bad_id = true; }
+            x1 = __ldg(a.hx + h0 + i1);
+          }
+          const uint32_t peers0 = __match_any_sync(0xFFFFFFFFu, sec0);
+          const uint32_t rank0 = __popc(peers0 & lt_mask);
+          const bool two = gb - ga > 32u;                       // warp-uniform
+          uint32_t peers1 = 0, rank1 = 0;
+          if (two) { peers1 = __match_any_sync(0xFFFFFFFFu, sec1); rank1 = __popc(peers1 & lt_mask); }
+          __syncwarp();
+          if (sec0 != kInvalid && rank0 == 0) cntA[sec0] = __popc(peers0);
+          if (sec1 != kInvalid && rank1 == 0) cntB[sec1] = __popc(peers1);
+          __syncwarp();
+          const uint32_t cA = sa + lane < sb ? cntA[sa + lane] : 0u;
+          const uint32_t cB = sa + lane < sb ? cntB[sa + lane] : 0u;
+          const uint32_t excl = warp_incl_scan(cA + cB, lane) - (cA + cB);
+          if (sa + lane < sb) s_off[sa + lane] = (uint16_t)(ga + excl);
+          const uint32_t b0 = __shfl_sync(0xFFFFFFFFu, excl, sec0 == kInvalid ? 0 : (int)(sec0 - sa));
+          const int src1 = sec1 == kInvalid ? 0 : (int)(sec1 - sa);
+          const uint32_t b1 = __shfl_sync(0xFFFFFFFFu, excl, src1) + __shfl_sync(0xFFFFFFFFu, cA, src1);
+          if (sec0 != kInvalid) { s_hx[ga + b0 + rank0] = x0; s_hh[ga + b0 + rank0] = (uint16_t)i0; }
+          if (sec1 != kInvalid) { s_hx[ga + b1 + rank1] = x1; s_hh[ga + b1 + rank1] = (uint16_t)i1; }
+          __syncwarp();                                          // cntA / cntB are reused by the next group
+          continue;
+        }
         for (uint32_t s = sa + lane; s < sb; s += 32) s_cnt[s] = 0;
         __syncwarp();
         for (uint32_t i = ga + lane; i < gb; i += 32) {
@@ -543,7 +608,6 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
           if (s < sb) { s_off[s] = (uint16_t)(run + incl - c); s_cnt[s] = run + incl - c; }
           run += __shfl_sync(0xFFFFFFFFu, incl, 31);
         }
-        if (g == ng - 1 && lane == 0) s_off[ns] = (uint16_t)n;
         __syncwarp();
         for (uint32_t i0 = ga; i0 < gb; i0 += 32) {
           const uint32_t i = i0 + lane;
@@ -585,7 +649,7 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, i
   size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + align16((size_t)ns * 8);
   b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
   b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
-  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)), align16((size_t)ns * 4));
+  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)), align16((size_t)ns * 8));
   return b;
 }
 
