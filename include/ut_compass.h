@@ -63,7 +63,8 @@ typedef void* ut_stream_t;
  * numbered layer-major, so `sector_group` is non-decreasing; group g belongs to layer
  * g / (n_groups / n_layers).  A sector group is a region of unique X.
  * Contract checked by ut_geometry_upload: n_layers == 4; n_groups % 4 == 0; every group non-empty;
- * dxdy constant inside a group; group_xmin and group_xmax non-decreasing inside a layer;
+ * at most 32 sectors per group; dxdy constant inside a group; group_xmin and group_xmax
+ * non-decreasing inside a layer;
  * pitch > 0; every x a sector can produce lies in [group_xmin, group_xmax] of its group. */
 typedef struct {
   uint32_t n_layers, n_sectors, n_groups;
@@ -77,6 +78,8 @@ typedef struct {
   /* filled by ut_geometry_upload (device, library-owned until ut_geometry_free) */
   const uint32_t* group_first_sector; /* [n_groups + 1] */
   const float* group_inv_span;        /* [n_groups] 1 / (group_xmax - group_xmin) */
+  const void* sector_rows;            /* [n_sectors] 32-byte rows {z, y_begin, y_end, dxdy | weight, raw id, x0,
+                                         pitch}: the table row a decoded hit copies, packed for 128-bit loads */
   uint32_t flags;                     /* UT_GEOM_* properties found by ut_geometry_upload */
   void* owner;                        /* opaque allocation handle, NULL for caller-owned tables */
 } ut_geometry;

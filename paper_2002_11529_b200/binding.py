@@ -34,7 +34,8 @@ class ut_geometry(C.Structure):
                 ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
                 ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
                 ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
-                ("group_first_sector", C.c_void_p), ("group_inv_span", C.c_void_p), ("flags", C.c_uint32),
+                ("group_first_sector", C.c_void_p), ("group_inv_span", C.c_void_p), ("sector_rows", C.c_void_p),
+                ("flags", C.c_uint32),
                 ("owner", C.c_void_p)]
 
 

@@ -71,6 +71,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
     }
     for (uint32_t g = 0; g < ng; ++g) {
       if (cnt[g] == 0) return UT_ERR_GEOMETRY;
+      if (cnt[g] > 32) return UT_ERR_LIMIT;                                // a warp holds a group's sector table
       first[g + 1] = first[g] + cnt[g];
       for (uint32_t s = first[g]; s < first[g + 1]; ++s) {
         if (h->dxdy[s] != h->dxdy[first[g]]) return UT_ERR_GEOMETRY;      // one stereo angle per group
@@ -86,7 +87,8 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   // ---- one device block, 256-byte aligned sub-tables ----
   auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
   const size_t sz_id = up(h->id_table_size * 4), sz_s = up(ns * 4), sz_g = up((ng + 1) * 4);
-  const size_t total = sz_id + 9 * sz_s + 4 * sz_g;
+  const size_t sz_rows = up((size_t)ns * 32);
+  const size_t total = sz_id + 9 * sz_s + 4 * sz_g + sz_rows;
   unsigned char* dev = nullptr;
   if (cudaMalloc(&dev, total) != cudaSuccess) return UT_ERR_CUDA;
   std::vector<unsigned char> host(total, 0);
@@ -113,6 +115,15 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   out->group_xmax = (const float*)put(h->group_xmax, ng * 4, sz_g);
   out->group_first_sector = (const uint32_t*)put(first.data(), (ng + 1) * 4, sz_g);
   out->group_inv_span = (const float*)put(inv.data(), ng * 4, sz_g);
+  {
+    std::vector<float> rows((size_t)ns * 8);
+    for (uint32_t s = 0; s < ns; ++s) {
+      float* r = rows.data() + (size_t)s * 8;
+      r[0] = h->z[s]; r[1] = h->y_begin[s]; r[2] = h->y_end[s]; r[3] = h->dxdy[s];
+      r[4] = h->weight[s]; memcpy(&r[5], &h->sector_raw_id[s], 4); r[6] = h->x0[s]; r[7] = h->pitch[s];
+    }
+    out->sector_rows = put(rows.data(), (size_t)ns * 32, sz_rows);
+  }
   if (cudaMemcpy(dev, host.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaFree(dev);
     return UT_ERR_CUDA;
@@ -151,7 +162,8 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
   launch_info().kernels_launched = 0;
   if (!bank_offsets || !geometry || !hits_out || !hit_offsets_out) return UT_ERR_NULL;
   if (n_events < 0) return UT_ERR_ARG;
-  if (!geometry->group_first_sector || !geometry->group_inv_span) return UT_ERR_GEOMETRY;   // not uploaded
+  if (!geometry->group_first_sector || !geometry->group_inv_span || !geometry->sector_rows)
+    return UT_ERR_GEOMETRY;                                                                  // not uploaded
   if (geometry->n_sectors > UT_MAX_SECTORS || geometry->n_groups > UT_MAX_GROUPS) return UT_ERR_LIMIT;
   if (!hits_out->x_at_y0 || !hits_out->z_at_y0 || !hits_out->y_begin || !hits_out->y_end || !hits_out->dxdy ||
       !hits_out->weight || !hits_out->id)

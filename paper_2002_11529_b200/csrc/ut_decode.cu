@@ -2,21 +2,25 @@
 //
 // The paper splits decoding into 7 launches (Table 1: count, 3-kernel Blelloch
 // scan with a host read-back of the total, pre-decode, find permutation, decode in order).  That
-// shape was made for sm_61/sm_70 and a batch of events that is tiny for a B200 (DESIGN.md section 5).
+// shape was made for sm_61/sm_70 and a batch of events that is tiny for a B200 (DESIGN.md section 6).
 // Here one CTA owns one event at a time (dynamic ticket), keeps the event on chip and touches HBM
 // once per byte:
 //
 //   ticket -> bank offsets (coalesced) -> raw banks of the event by ONE TMA bulk copy into smem
-//   -> per-bank header check, sector claim, count          (paper: "calculate number of hits")
-//   -> event total -> chained exclusive prefix over events by decoupled look-back (paper: prefix sum
-//      + host sync; here no sync, no second launch)
-//   -> bucket histogram of x inside every sector group (monotone fp32 -> bucket map), block scan,
-//      scatter, in-bucket rank by (x, sector, word)         (paper: pre-decode + find permutation)
-//   -> coalesced SoA store at base + rank                   (paper: decode raw banks in order)
+//   -> thread per bank: header check, sector claim, count   (paper: "calculate number of hits")
+//   -> event total published at once for the chained exclusive prefix over events (decoupled
+//      look-back by warp 0; paper: prefix sum + host sync; here no sync, no second launch); the
+//      event's base is only awaited in front of the first store
+//   -> warp per sector group (dynamic ticket inside the CTA): the lanes gather the group's words
+//      from its banks in fill order (sector, word), decode x, and rank them -- for <= 32 hits in
+//      registers with shuffles, else through a per-warp shared-memory buffer.  Lane order is the
+//      tie-break order, so the rank IS the stable sort by x   (paper: pre-decode + find permutation)
+//   -> SoA store at base + group start + rank; a group is one contiguous window of every array
+//                                                            (paper: decode raw banks in order)
 //
-// The bucket pass makes the stable in-group sort O(n) instead of the paper's insertion sort.
-// Events that do not fit the shared-memory staging sizes take a slower generic path with the same
-// results.  Arithmetic of x follows include/ut_compass.h exactly (__fmul_rn/__fadd_rn, never fused).
+// There is no block barrier after the count: warps run independently through the groups.
+// Events or groups that do not fit the staging sizes take slower generic code with the same results.
+// Arithmetic of x follows include/ut_compass.h exactly (__fmul_rn/__fadd_rn, never fused).
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -38,26 +42,13 @@ struct DecodeArgs {
   uint32_t* ctrl;               // [0] ticket, [1] CTAs done, [2] epoch
   unsigned long long* flags;    // [n_events] look-back words: epoch:30 | state:2 | value:32
   uint32_t raw_stage_bytes;     // multiple of 16
-  uint32_t hit_stage;           // elements
-  uint32_t log2_buckets;        // buckets per group = 1 << log2_buckets
+  uint32_t sort_buf;            // elements of the per-warp sort buffer (multiple of 32)
 };
 
 __device__ __forceinline__ float decode_x(uint32_t word, float x0, float pitch) {
   const uint32_t u = ((word & 0x1FFu) << 1) | ((word >> 9) & 1u);   // 2*strip + frac
   const float t = __fadd_rn(__fmul_rn((float)u, 0.5f), 0.25f);
   return __fadd_rn(x0, __fmul_rn(t, pitch));
-}
-
-// monotone non-decreasing map x -> bucket inside a group (equal x -> equal bucket)
-__device__ __forceinline__ uint32_t bucket_of(float x, float xmin, float inv_span, uint32_t nb) {
-  const float f = __fmul_rn(__fmul_rn(__fsub_rn(x, xmin), inv_span), (float)nb);
-  int b = (int)f;                                         // cvt.rzi saturates, NaN -> 0
-  b = b < 0 ? 0 : b;
-  return (uint32_t)b < nb ? (uint32_t)b : nb - 1;
-}
-
-__device__ __forceinline__ bool key_less(float xa, uint32_t ka, float xb, uint32_t kb) {
-  return xa < xb || (xa == xb && ka < kb);
 }
 
 // Chained exclusive prefix over events (decoupled look-back).  Called by warp 0.  Event e only waits
@@ -91,47 +82,61 @@ __device__ uint32_t event_base_lookback(unsigned long long* flags, int e, uint32
   return base;
 }
 
-__global__ void __launch_bounds__(1024) ut_decode_kernel(const DecodeArgs a) {
+__device__ __forceinline__ uint32_t ld_volatile_shared_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+  return v;
+}
+
+// stable order of the fill sequence: (x, position in the fill order)
+__device__ __forceinline__ uint32_t before(float xj, uint32_t j, float x, uint32_t i) {
+  return (xj < x || (xj == x && j < i)) ? 1u : 0u;
+}
+
+// Rank of this lane's x among the 32 lanes of the warp in the stable order (x, lane): lanes that hold no
+// element pass +inf and are never counted.  32 unrolled shuffles for "smaller", one match.any for the ties.
+__device__ __forceinline__ uint32_t warp_rank(float x, uint32_t lt_mask) {
+  uint32_t rank = 0;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) rank += __shfl_sync(0xFFFFFFFFu, x, j) < x ? 1u : 0u;
+  const uint32_t ties = __match_any_sync(0xFFFFFFFFu, __float_as_uint(x + 0.0f));      // -0 == +0
+  return rank + __popc(ties & lt_mask);
+}
+
+__global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t ns = a.g.n_sectors, ng = a.g.n_groups;
-  const uint32_t nbk = 1u << a.log2_buckets, NB = ng << a.log2_buckets;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
+  const uint32_t idn = min(a.g.id_table_size, 2048u);
 
   Carver cv(smem_raw);
   unsigned char* s_rawstage = cv.take<unsigned char>(a.raw_stage_bytes);
-  float* g_x0 = cv.take<float>(ns);
-  float* g_pitch = cv.take<float>(ns);
-  float* g_z = cv.take<float>(ns);
-  float* g_yb = cv.take<float>(ns);
-  float* g_ye = cv.take<float>(ns);
-  float* g_dxdy = cv.take<float>(ns);
-  float* g_w = cv.take<float>(ns);
-  uint32_t* g_rawid = cv.take<uint32_t>(ns);
+  float2* g_x0p = cv.take<float2>(ns);            // (x0, pitch) per sector
+  uint16_t* g_idtab = cv.take<uint16_t>(idn);     // raw id -> dense sector, 0xFFFF = invalid
   uint16_t* g_group = cv.take<uint16_t>(ns);
-  float* g_gxmin = cv.take<float>(ng);
-  float* g_ginv = cv.take<float>(ng);
-  uint32_t* g_gfirst = cv.take<uint32_t>(ng + 1);
+  uint16_t* g_gfirst = cv.take<uint16_t>(ng + 1);
   uint32_t* s_off = cv.take<uint32_t>(ns + 4);
   uint32_t* s_cnt = cv.take<uint32_t>(ns);
   uint32_t* s_wpos = cv.take<uint32_t>(ns);
-  uint32_t* s_gstart = cv.take<uint32_t>(ng + 1);
-  uint32_t* s_bucket = cv.take<uint32_t>(NB);
-  float* t_x = cv.take<float>(a.hit_stage);
-  uint32_t* t_key = cv.take<uint32_t>(a.hit_stage);
+  uint32_t* s_gcnt = cv.take<uint32_t>(ng);
+  float* s_xbuf = cv.take<float>((size_t)nwarps * a.sort_buf);
+  uint32_t* s_wbuf = cv.take<uint32_t>((size_t)nwarps * a.sort_buf);
 
   __shared__ uint64_t s_bar;
   __shared__ int s_event;
-  __shared__ uint32_t s_epoch, s_status, s_base, s_tot;
+  __shared__ uint32_t s_epoch, s_status, s_base, s_ready, s_gticket;
   __shared__ uint32_t s_warp[32];
 
   // geometry tables: staged once per CTA, reused for every event this CTA takes
   for (uint32_t i = tid; i < ns; i += nt) {
-    g_x0[i] = a.g.x0[i]; g_pitch[i] = a.g.pitch[i]; g_z[i] = a.g.z[i]; g_yb[i] = a.g.y_begin[i];
-    g_ye[i] = a.g.y_end[i]; g_dxdy[i] = a.g.dxdy[i]; g_w[i] = a.g.weight[i];
-    g_rawid[i] = a.g.sector_raw_id[i]; g_group[i] = (uint16_t)a.g.sector_group[i];
+    g_x0p[i] = make_float2(a.g.x0[i], a.g.pitch[i]);
+    g_group[i] = (uint16_t)a.g.sector_group[i];
   }
-  for (uint32_t i = tid; i < ng; i += nt) { g_gxmin[i] = a.g.group_xmin[i]; g_ginv[i] = a.g.group_inv_span[i]; }
-  for (uint32_t i = tid; i <= ng; i += nt) g_gfirst[i] = a.g.group_first_sector[i];
+  for (uint32_t i = tid; i < idn; i += nt) {
+    const uint32_t s = a.g.id_to_sector[i];
+    g_idtab[i] = s < ns ? (uint16_t)s : (uint16_t)0xFFFFu;
+  }
+  for (uint32_t i = tid; i <= ng; i += nt) g_gfirst[i] = (uint16_t)a.g.group_first_sector[i];
   if (tid == 0) {
     mbar_init(&s_bar, 1);
     fence_mbar_init();
@@ -140,10 +145,13 @@ __global__ void __launch_bounds__(1024) ut_decode_kernel(const DecodeArgs a) {
   }
   __syncthreads();
   uint32_t bar_phase = 0;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  float* xbuf = s_xbuf + (size_t)warp * a.sort_buf;
+  uint32_t* wbuf = s_wbuf + (size_t)warp * a.sort_buf;
 
   for (;;) {
     if (tid == 0) s_event = (int)atomicAdd(a.ctrl, 1u);
-    __syncthreads();
+    __syncthreads();                     // also: every warp is done with the previous event's tables
     const int e = s_event;
     if (e >= a.n_events) break;
 
@@ -151,7 +159,8 @@ __global__ void __launch_bounds__(1024) ut_decode_kernel(const DecodeArgs a) {
     const uint32_t* bo = a.bank_offsets + (size_t)e * ns;
     for (uint32_t i = tid; i <= ns; i += nt) s_off[i] = __ldg(bo + i);
     for (uint32_t i = tid; i < ns; i += nt) { s_cnt[i] = 0; s_wpos[i] = kInvalid; }
-    for (uint32_t i = tid; i < NB; i += nt) s_bucket[i] = 0;
+    for (uint32_t i = tid; i < ng; i += nt) s_gcnt[i] = 0;
+    if (tid == 0) { s_ready = 0; s_gticket = 0; }
     __syncthreads();
 
     const uint32_t b0 = s_off[0], b1 = s_off[ns];
@@ -179,139 +188,187 @@ __global__ void __launch_bounds__(1024) ut_decode_kernel(const DecodeArgs a) {
         const uint32_t rel = o0 - b0a;
         const uint32_t rid = *reinterpret_cast<const uint32_t*>(rawp + rel);
         const uint32_t cnt = *reinterpret_cast<const uint32_t*>(rawp + rel + 4) & 0xFFFFu;
-        const uint32_t s = rid < a.g.id_table_size ? __ldg(a.g.id_to_sector + rid) : kInvalid;
+        uint32_t s = kInvalid;
+        if (rid < idn) { s = g_idtab[rid]; if (s == 0xFFFFu) s = kInvalid; }
+        else if (rid < a.g.id_table_size) s = __ldg(a.g.id_to_sector + rid);
         if (s >= ns) { st |= UT_STATUS_UNKNOWN_SECTOR; continue; }
         if (o1 - o0 != ((6u + 2u * cnt + 3u) & ~3u)) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
         if (atomicCAS(&s_wpos[s], kInvalid, rel + 6u) != kInvalid) { st |= UT_STATUS_DUPLICATE_SECTOR; continue; }
         s_cnt[s] = cnt;
+        if (cnt) atomicAdd(&s_gcnt[g_group[s]], cnt);
         local += cnt;
       }
     }
     if (st) atomicOr(&s_status, st);
     local = warp_sum(local);
     if (lane == 0) s_warp[warp] = local;
-    __syncthreads();
+    __syncthreads();                     // last block barrier of the event: warps run on their own from here
 
-    // ---- event total, chained prefix over events, group starts ---------------------------------------
+    uint32_t tot = warp_sum(lane < nwarps ? s_warp[lane] : 0u);
+    // exclusive scan of the group counts, 4 groups per lane (ng <= 128), kept in registers by every warp
+    uint32_t gc[4], gs[4];
+    {
+      uint32_t run = 0;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint32_t g = lane * 4 + q;
+        gc[q] = g < ng ? s_gcnt[g] : 0u;
+        run += gc[q];
+      }
+      uint32_t ex = warp_incl_scan(run, lane) - run;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) { gs[q] = ex; ex += gc[q]; }
+    }
+
+    // ---- event base: warp 0 publishes the total and resolves the chained prefix over events -----------
+    uint32_t base = 0;
+    bool have_base = false;
     if (warp == 0) {
-      uint32_t v = lane < nwarps ? s_warp[lane] : 0u;
-      v = warp_sum(v);
-      const uint32_t base = event_base_lookback(a.flags, e, v, s_epoch, lane);
-      if (lane == 0) { s_tot = v; s_base = base; }
-    } else if (warp == 1) {
-      // exclusive scan of the per-group counts (groups = runs of sectors), ng <= 128
-      uint32_t c[4], run = 0;
+      base = event_base_lookback(a.flags, e, tot, s_epoch, lane);
+      have_base = true;
+      if (lane == 0) {
+        s_base = base;
+        __threadfence_block();
+        *reinterpret_cast<volatile uint32_t*>(&s_ready) = 1u;
+        if ((unsigned long long)base + tot > a.capacity) atomicOr(&s_status, (uint32_t)UT_STATUS_CAPACITY);
+        if (e == a.n_events - 1) a.hit_offsets[(size_t)a.n_events * ng] = base + tot;
+      }
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const uint32_t g = lane * 4 + q;
-        uint32_t v = 0;
-        if (g < ng) for (uint32_t s = g_gfirst[g]; s < g_gfirst[g + 1]; ++s) v += s_cnt[s];
-        c[q] = v; run += v;
+        if (g < ng) a.hit_offsets[(size_t)e * ng + g] = base + gs[q];
       }
-      const uint32_t incl = warp_incl_scan(run, lane);
-      uint32_t ex = incl - run;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const uint32_t g = lane * 4 + q;
-        if (g < ng) s_gstart[g] = ex;
-        ex += c[q];
-      }
-      if (lane == 31) s_gstart[ng] = incl;
     }
-    __syncthreads();
-    const uint32_t tot = s_tot, base = s_base;
-    for (uint32_t g = tid; g < ng; g += nt) a.hit_offsets[(size_t)e * ng + g] = base + s_gstart[g];
-    if (e == a.n_events - 1 && tid == 0) a.hit_offsets[(size_t)a.n_events * ng] = base + tot;
-    const bool fits = (unsigned long long)base + tot <= a.capacity;
-    if (!fits && tid == 0) atomicOr(&s_status, (uint32_t)UT_STATUS_CAPACITY);
+    if (tot == 0) continue;
 
-    if (fits && tot > 0 && tot <= a.hit_stage) {
-      // ---- fast path: O(n) bucket ordering on chip ----------------------------------------------------
-      for (uint32_t s = tid; s < ns; s += nt) {                      // pass 1: bucket histogram
-        const uint32_t cnt = s_cnt[s];
-        if (!cnt) continue;
-        const uint16_t* w16 = reinterpret_cast<const uint16_t*>(rawp + s_wpos[s]);
-        const uint32_t g = g_group[s];
-        const float x0 = g_x0[s], pitch = g_pitch[s], xmin = g_gxmin[g], inv = g_ginv[g];
-        for (uint32_t k = 0; k < cnt; ++k) {
-          const float x = decode_x(w16[k], x0, pitch);
-          atomicAdd(&s_bucket[(g << a.log2_buckets) + bucket_of(x, xmin, inv, nbk)], 1u);
+    // ---- warp per sector group (ticket inside the CTA) --------------------------------------------------
+    for (;;) {
+      uint32_t g = 0;
+      if (lane == 0) g = atomicAdd(&s_gticket, 1u);
+      g = __shfl_sync(0xFFFFFFFFu, g, 0);
+      if (g >= ng) break;
+      const uint32_t q4 = g & 3u;                       // warp-uniform: pick the register, then the lane
+      const uint32_t n = __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gc[0] : q4 == 1 ? gc[1] : q4 == 2 ? gc[2] : gc[3], (int)(g >> 2));
+      const uint32_t gstart =
+          __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gs[0] : q4 == 1 ? gs[1] : q4 == 2 ? gs[2] : gs[3], (int)(g >> 2));
+      if (n == 0) continue;
+      const uint32_t sa = g_gfirst[g], nsec = g_gfirst[g + 1] - sa;      // nsec <= 32 (ut_geometry_upload)
+      // the group's banks: word count and word position per sector, exclusive prefix = fill order
+      const uint32_t cnt_r = (uint32_t)lane < nsec ? s_cnt[sa + lane] : 0u;
+      const uint32_t wpos_r = (uint32_t)lane < nsec ? s_wpos[sa + lane] : 0u;
+      const uint32_t e_incl = warp_incl_scan(cnt_r, lane);
+      const uint32_t e_r = (uint32_t)lane < nsec ? e_incl - cnt_r : n;   // lanes past the group: never selected
+      const bool in_regs = n <= 32u, in_buf = n <= a.sort_buf;
+
+      // gather: element i of the fill order -> (sector r, word k), decode x
+      float x = 0.f;
+      uint32_t rw = 0;                                  // (sector-in-group << 16) | raw word
+      for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+        const uint32_t i = c0 + lane;
+        int r = 0;                                      // largest r with e_r <= i
+#pragma unroll
+        for (int step = 16; step > 0; step >>= 1) {
+          const uint32_t ev = __shfl_sync(0xFFFFFFFFu, e_r, r + step);
+          if (ev <= i) r += step;
         }
-      }
-      __syncthreads();
-      {                                                               // exclusive scan over NB buckets
-        const uint32_t ipt = (NB + nt - 1) / nt;
-        const uint32_t c0 = min(NB, tid * ipt), c1 = min(NB, c0 + ipt);
-        uint32_t sum = 0;
-        for (uint32_t i = c0; i < c1; ++i) sum += s_bucket[i];
-        const uint32_t incl = warp_incl_scan(sum, lane);
-        if (lane == 31) s_warp[warp] = incl;
-        __syncthreads();
-        if (warp == 0) {
-          const uint32_t v = lane < nwarps ? s_warp[lane] : 0u;
-          const uint32_t iv = warp_incl_scan(v, lane);
-          s_warp[lane] = iv - v;
+        const uint32_t k = i - __shfl_sync(0xFFFFFFFFu, e_r, r);
+        const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
+        if (i < n) {
+          const uint32_t word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
+          const float2 xp = g_x0p[sa + r];
+          x = decode_x(word, xp.x, xp.y);
+          rw = ((uint32_t)r << 16) | word;
+          if (!in_regs && in_buf) { xbuf[i] = x; wbuf[i] = rw; }
         }
-        __syncthreads();
-        uint32_t ex = s_warp[warp] + incl - sum;
-        for (uint32_t i = c0; i < c1; ++i) { const uint32_t v = s_bucket[i]; s_bucket[i] = ex; ex += v; }
+        if (!in_buf) break;                             // generic path gathers again below
       }
-      __syncthreads();
-      for (uint32_t s = tid; s < ns; s += nt) {                      // pass 2: scatter into buckets
-        const uint32_t cnt = s_cnt[s];
-        if (!cnt) continue;
-        const uint16_t* w16 = reinterpret_cast<const uint16_t*>(rawp + s_wpos[s]);
-        const uint32_t g = g_group[s];
-        const float x0 = g_x0[s], pitch = g_pitch[s], xmin = g_gxmin[g], inv = g_ginv[g];
-        for (uint32_t k = 0; k < cnt; ++k) {
-          const float x = decode_x(w16[k], x0, pitch);
-          const uint32_t pos = atomicAdd(&s_bucket[(g << a.log2_buckets) + bucket_of(x, xmin, inv, nbk)], 1u);
-          t_x[pos] = x;
-          t_key[pos] = (s << 16) | k;
+
+      if (!have_base) {                                 // the event's base is needed from here on
+        while (ld_volatile_shared_u32(&s_ready) == 0u) {}
+        __threadfence_block();
+        base = *reinterpret_cast<volatile uint32_t*>(&s_base);
+        have_base = true;
+      }
+      if ((unsigned long long)base + tot > a.capacity) continue;        // flagged by warp 0; offsets stay exact
+      const size_t P0 = (size_t)base + gstart;
+
+      if (in_regs) {
+        // ---- <= 32 hits: rank in registers, lane order = fill order --------------------------------------
+        const uint32_t rank = warp_rank((uint32_t)lane < n ? x : __int_as_float(0x7F800000), lt_mask);
+        if ((uint32_t)lane < n) {
+          const uint32_t s = sa + (rw >> 16);
+          const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
+          const size_t P = P0 + rank;
+          a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
+          a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
         }
-      }
-      __syncthreads();                                               // now s_bucket[b] = end of bucket b
-      for (uint32_t q = tid; q < tot; q += nt) {                     // pass 3: rank inside bucket, store
-        const float x = t_x[q];
-        const uint32_t key = t_key[q];
-        const uint32_t s = key >> 16, k = key & 0xFFFFu;
-        const uint32_t g = g_group[s];
-        const uint32_t gb = (g << a.log2_buckets) + bucket_of(x, g_gxmin[g], g_ginv[g], nbk);
-        const uint32_t lo = gb ? s_bucket[gb - 1] : 0u, hi = s_bucket[gb];
-        uint32_t rank = lo;
-        for (uint32_t j = lo; j < hi; ++j) rank += key_less(t_x[j], t_key[j], x, key) ? 1u : 0u;
-        const uint32_t word = reinterpret_cast<const uint16_t*>(rawp + s_wpos[s])[k];
-        const size_t P = (size_t)base + rank;
-        a.x[P] = x; a.z[P] = g_z[s]; a.yb[P] = g_yb[s]; a.ye[P] = g_ye[s];
-        a.dxdy[P] = g_dxdy[s]; a.w[P] = g_w[s]; a.id[P] = (g_rawid[s] << 9) | (word & 0x1FFu);
-      }
-    } else if (fits && tot > 0) {
-      // ---- generic path (event larger than the staging sizes): rank by recomputation, O(n^2) per group ----
-      for (uint32_t s = 0; s < ns; ++s) {
-        const uint32_t cnt = s_cnt[s];
-        if (!cnt) continue;
-        const uint32_t g = g_group[s];
-        const uint16_t* w16 = reinterpret_cast<const uint16_t*>(rawp + s_wpos[s]);
-        for (uint32_t k = tid; k < cnt; k += nt) {
-          const uint32_t word = w16[k];
-          const float x = decode_x(word, g_x0[s], g_pitch[s]);
-          const uint32_t key = (s << 16) | k;
-          uint32_t rank = 0;
-          for (uint32_t s2 = g_gfirst[g]; s2 < g_gfirst[g + 1]; ++s2) {
-            const uint32_t c2 = s_cnt[s2];
-            if (!c2) continue;
-            const uint16_t* v16 = reinterpret_cast<const uint16_t*>(rawp + s_wpos[s2]);
-            const float x02 = g_x0[s2], p2 = g_pitch[s2];
-            for (uint32_t k2 = 0; k2 < c2; ++k2)
-              rank += key_less(decode_x(v16[k2], x02, p2), (s2 << 16) | k2, x, key) ? 1u : 0u;
+      } else if (in_buf) {
+        // ---- <= sort_buf hits: rank against the warp's shared-memory copy -----------------------------------
+        const uint32_t npad = (n + 3u) & ~3u;          // pad the tail of the buffer with +inf (never "smaller")
+        if (n + lane < npad) xbuf[n + lane] = __int_as_float(0x7F800000);
+        __syncwarp();
+        for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+          const uint32_t i = c0 + lane;
+          const bool valid = i < n;
+          const float xi = valid ? xbuf[i] : __int_as_float(0x7F800000);
+          // elements of earlier chunks come first on ties, later chunks never; this chunk: warp_rank
+          uint32_t rank = warp_rank(xi, lt_mask);
+          for (uint32_t j = 0; j < c0; j += 4u) {
+            const float4 v = *reinterpret_cast<const float4*>(xbuf + j);
+            rank += (v.x <= xi ? 1u : 0u) + (v.y <= xi ? 1u : 0u) + (v.z <= xi ? 1u : 0u) + (v.w <= xi ? 1u : 0u);
           }
-          const size_t P = (size_t)base + s_gstart[g] + rank;
-          a.x[P] = x; a.z[P] = g_z[s]; a.yb[P] = g_yb[s]; a.ye[P] = g_ye[s];
-          a.dxdy[P] = g_dxdy[s]; a.w[P] = g_w[s]; a.id[P] = (g_rawid[s] << 9) | (word & 0x1FFu);
+          for (uint32_t j = c0 + 32u; j < npad; j += 4u) {
+            const float4 v = *reinterpret_cast<const float4*>(xbuf + j);
+            rank += (v.x < xi ? 1u : 0u) + (v.y < xi ? 1u : 0u) + (v.z < xi ? 1u : 0u) + (v.w < xi ? 1u : 0u);
+          }
+          if (valid) {
+            const uint32_t rwi = wbuf[i];
+            const uint32_t s = sa + (rwi >> 16);
+            const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
+            const size_t P = P0 + rank;
+            a.x[P] = xi; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
+            a.id[P] = (__float_as_uint(B.y) << 9) | (rwi & 0x1FFu);
+          }
+        }
+        __syncwarp();                                   // the buffer is reused by the warp's next group
+      } else {
+        // ---- generic path (group larger than the sort buffer): rank by recomputation, O(n^2) --------------
+        for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+          const uint32_t i = c0 + lane;
+          int r = 0;
+#pragma unroll
+          for (int step = 16; step > 0; step >>= 1) {
+            const uint32_t ev = __shfl_sync(0xFFFFFFFFu, e_r, r + step);
+            if (ev <= i) r += step;
+          }
+          const uint32_t k = i - __shfl_sync(0xFFFFFFFFu, e_r, r);
+          const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
+          const bool valid = i < n;
+          uint32_t word = 0;
+          float xi = 0.f;
+          if (valid) {
+            word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
+            const float2 xp = g_x0p[sa + r];
+            xi = decode_x(word, xp.x, xp.y);
+          }
+          uint32_t rank = 0, j = 0;
+          for (uint32_t r2 = 0; r2 < nsec; ++r2) {      // warp-uniform walk over the fill order
+            const uint32_t c2 = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)r2);
+            const uint32_t w2 = __shfl_sync(0xFFFFFFFFu, wpos_r, (int)r2);
+            const float2 xp2 = g_x0p[sa + r2];
+            for (uint32_t k2 = 0; k2 < c2; ++k2, ++j)
+              rank += before(decode_x(*reinterpret_cast<const uint16_t*>(rawp + w2 + 2u * k2), xp2.x, xp2.y), j, xi, i);
+          }
+          if (valid) {
+            const uint32_t s = sa + (uint32_t)r;
+            const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
+            const size_t P = P0 + rank;
+            a.x[P] = xi; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
+            a.id[P] = (__float_as_uint(B.y) << 9) | (word & 0x1FFu);
+          }
         }
       }
     }
-    __syncthreads();      // everything of this event is consumed before the tables are reset
   }
 
   if (tid == 0) {
@@ -332,13 +389,11 @@ static int env_int(const char* name, int dflt) {
   return v && *v ? atoi(v) : dflt;
 }
 
-size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, uint32_t hit_stage, uint32_t log2b) {
+static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t idn, uint32_t raw_stage, uint32_t sort_buf, int block) {
   size_t b = align16(raw_stage);
-  b += 8 * align16(ns * 4) + align16(ns * 2);
-  b += 2 * align16(ng * 4) + align16((ng + 1) * 4);
-  b += align16((ns + 4) * 4) + 2 * align16(ns * 4) + align16((ng + 1) * 4);
-  b += align16((size_t)(ng << log2b) * 4);
-  b += 2 * align16((size_t)hit_stage * 4);
+  b += align16((size_t)ns * 8) + align16((size_t)idn * 2) + align16((size_t)ns * 2) + align16((size_t)(ng + 1) * 2);
+  b += align16((size_t)(ns + 4) * 4) + 2 * align16((size_t)ns * 4) + align16((size_t)ng * 4);
+  b += 2 * align16((size_t)(block / 32) * sort_buf * 4);
   return b;
 }
 
@@ -366,27 +421,30 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
 
   // staging sizes from the only size the host knows without a sync: capacity / n_events
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
+  const uint32_t idn = std::min<uint32_t>(geom->id_table_size, 2048u);
   const unsigned long long avg = hits->capacity / (unsigned long long)n_events + 1;
-  uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
-  hit_stage = (uint32_t)env_int("UT_DECODE_HIT_STAGE", (int)hit_stage);
-  uint32_t log2b = 3;
-  while (log2b < 8 && (1.4142f * (float)(1u << log2b)) < (float)avg / (float)ng) ++log2b;
-  log2b = (uint32_t)env_int("UT_DECODE_LOG2_BUCKETS", (int)log2b);
-  uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * hit_stage + 32u);
+  const unsigned long long stage_hits = std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
+  uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * stage_hits + 32u);
   raw_stage = (uint32_t)env_int("UT_DECODE_RAW_STAGE", (int)raw_stage) & ~15u;
-  size_t smem = decode_smem_bytes(ns, ng, raw_stage, hit_stage, log2b);
+  // per-warp sort buffer: twice the mean group size, at least 64, a multiple of 32
+  uint32_t sort_buf = (uint32_t)std::min<unsigned long long>(((2 * avg / ng + 31) / 32) * 32 + 32, 1024);
+  sort_buf = std::max(64u, sort_buf);
+  sort_buf = ((uint32_t)env_int("UT_DECODE_SORT_BUF", (int)sort_buf) + 31u) & ~31u;
+  int block = env_int("UT_DECODE_BLOCK", 256);
+  block = std::max(64, std::min(512, (block / 32) * 32));
+  size_t smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
   const size_t budget = (size_t)max_smem;
-  while (smem > budget && hit_stage > 256) {           // shrink until it fits; oversize events take the generic path
-    hit_stage /= 2;
-    raw_stage = (uint32_t)align16(8u * ns + 2u * hit_stage + 32u);
-    if (log2b > 3) --log2b;
-    smem = decode_smem_bytes(ns, ng, raw_stage, hit_stage, log2b);
+  while (smem > budget && raw_stage > 4096) {            // oversize events read their banks from global memory
+    raw_stage = (raw_stage / 2) & ~15u;
+    smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
+  }
+  while (smem > budget && sort_buf > 32) {
+    sort_buf -= 32;
+    smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
-  a.raw_stage_bytes = raw_stage; a.hit_stage = hit_stage; a.log2_buckets = log2b;
+  a.raw_stage_bytes = raw_stage; a.sort_buf = sort_buf;
 
-  int block = env_int("UT_DECODE_BLOCK", 512);
-  block = std::max(64, std::min(1024, (block / 32) * 32));
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ut_decode_kernel, block, smem));
   if (per_sm < 1) return cuda_fail("decode kernel does not fit on an SM", cudaErrorInvalidConfiguration);
@@ -396,7 +454,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   UTC_CUDA(cudaGetLastError());
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.decode_grid = grid; li.decode_block = block; li.decode_smem_bytes = (int)smem;
-  li.decode_buckets_per_group = 1 << log2b; li.decode_hit_stage = (int)hit_stage;
+  li.decode_buckets_per_group = 0; li.decode_hit_stage = (int)sort_buf;
   return UT_OK;
 }
 

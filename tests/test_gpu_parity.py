@@ -185,7 +185,7 @@ def test_repeated_calls_reuse_workspace(gpu, wl):
 def test_small_staging_takes_generic_paths(gpu, wl, monkeypatch):
     """Force the events through the non-staged decode path and the global-memory Compass path."""
     geom, b, p = wl(2, 12)
-    monkeypatch.setenv("UT_DECODE_HIT_STAGE", "256")
+    monkeypatch.setenv("UT_DECODE_SORT_BUF", "32")
     monkeypatch.setenv("UT_DECODE_RAW_STAGE", "4096")
     monkeypatch.setenv("UT_COMPASS_HIT_STAGE", "512")
     check_batch(gpu, geom, b, p)
