@@ -32,6 +32,13 @@ if ROOT not in sys.path:
 METRIC = "ut_decode_compass_events_per_s"
 UNIT = "events/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
+# profiles/ (config 3; taken with the bench's own L2 flush between steps).  Keyed by workload, then kernel.
+NCU_DRAM_TRAFFIC = {
+    "config3_throughput1000": {"compass_kernel": 18.6e6, "ut_decode_kernel": 17.6e6,
+                               "source": "profiles/r1c_decode_warp_per_group.md"},
+}
+
 
 def parse_args():
     ap = argparse.ArgumentParser()
@@ -416,7 +423,9 @@ def main():
     }
     dom = "ut_decode_kernel" if md >= mc else "compass_kernel"
     roof = {"kernel": dom, "bound": "hbm", "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
-            "frac": kern[dom]["frac_hbm"], "traffic": None, "peak_source": peak_src,
+            "frac": kern[dom]["frac_hbm"],
+            "traffic": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get(dom) if batch.n_events == cfg.n_events else None,
+            "traffic_source": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get("source"), "peak_source": peak_src,
             "algorithmic_bytes_per_launch": kern[dom]["bytes"],
             "end_to_end": {"bytes": abytes["e2e"], "gbs": abytes["e2e"] / ms / 1e6,
                            "frac": abytes["e2e"] / ms / 1e6 / hbm_peak, "frac_of_8TBs": abytes["e2e"] / ms / 1e6 / 8000.0}}

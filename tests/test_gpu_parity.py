@@ -60,6 +60,47 @@ def test_config4_subset(gpu, wl):
     assert (t.cand_n > p.max_candidates_per_layer).any()      # the candidate cap path runs on the GPU too
 
 
+def test_config3_full_size_bench_launch(gpu, wl):
+    """BASELINE.json configs[2] at its full size, in the launch configuration bench.py times (defaults of the
+    library for a 1000-event batch): every output element against the oracle."""
+    geom, b, p = wl(3)
+    assert b.n_events == 1000
+    check_batch(gpu, geom, b, p)
+    li = gpu.B.last_launch_info()
+    assert li["kernels_launched"] == 1 and li["compass_grid"] >= 148
+
+
+def test_config4_full_size(gpu, wl):
+    """configs[3] at its full size (1000 events, ~8000 hits, C = 32)."""
+    geom, b, p = wl(4)
+    assert b.n_events == 1000
+    h, t = check_batch(gpu, geom, b, p)
+    assert (t.cand_n > p.max_candidates_per_layer).sum() > 1000
+
+
+def test_config5_first_1000_events_all_settings(gpu, wl):
+    """configs[4]: the 18 sweep settings on the first 1000 events of the 10000-event stream (events are
+    generated independently of the batch size, so these are the sweep's own first 1000 events)."""
+    from gpu_helpers import compare_tracks
+    from synth.configs import SWEEP_MIN_HITS, SWEEP_SCALE, SWEEP_CANDIDATES
+    geom, b, _ = wl(5, 1000)
+    hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+    h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+    got, off, st = gpu.hits_numpy(hits, b.n_events)
+    from gpu_helpers import compare_decode
+    compare_decode(h_ref, got, off, st)
+    for mh in SWEEP_MIN_HITS:
+        for sc in SWEEP_SCALE:
+            for C in SWEEP_CANDIDATES:
+                p = synth.CONFIGS[5].compass_params(min_hits=mh, window_scale=sc, max_candidates_per_layer=C)
+                t_ref = oracle.compass(h_ref, b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z, b.velo_offsets,
+                                       b.n_events, geom, p)
+                trk = gpu.compass(hits, b, p)
+                n_diff, _ = compare_tracks(t_ref, trk)
+                assert n_diff == 0, (mh, sc, C)
+                assert np.array_equal(trk["chi2"].view(np.uint32), t_ref.chi2.view(np.uint32)), (mh, sc, C)
+
+
 @pytest.mark.parametrize("min_hits", [3, 4])
 @pytest.mark.parametrize("scale", [0.5, 1.0, 2.0])
 @pytest.mark.parametrize("C", [8, 16, 32])
