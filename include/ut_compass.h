@@ -105,7 +105,10 @@ typedef struct {
   const ut_geometry* geom;    /* HOST pointer to the device-table descriptor used to decode */
   uint32_t* status;           /* device word, OR-ed with UT_STATUS_* (caller zeroes it) */
   void* workspace;            /* device, ut_decode_workspace_bytes() bytes, zeroed once by
-                                 ut_decode_workspace_init(); reusable across calls on one stream */
+                                 ut_decode_workspace_init(); reusable across calls on one stream.
+                                 compass_track keeps its event ticket here too: calls that share one
+                                 ut_hits must be ordered on one stream.  May be NULL for a container that
+                                 ut_decode did not fill (compass_track then assigns events statically). */
 } ut_hits;
 
 size_t ut_decode_workspace_bytes(int32_t max_events);

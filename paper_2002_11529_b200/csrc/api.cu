@@ -147,7 +147,7 @@ int32_t ut_geometry_free(ut_geometry* g) {
 }
 
 size_t ut_decode_workspace_bytes(int32_t max_events) {
-  return 16 + 8 * (size_t)(max_events > 0 ? max_events : 0) + 8;
+  return 32 + 8 * (size_t)(max_events > 0 ? max_events : 0) + 8;   // 8 control words, then one look-back word per event
 }
 
 int32_t ut_decode_workspace_init(void* workspace, int32_t max_events, ut_stream_t stream) {

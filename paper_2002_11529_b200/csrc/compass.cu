@@ -59,6 +59,7 @@ struct CompassArgs {
   float *out_qop, *out_chi2;
   uint32_t* status;
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
+  uint32_t* ticket;                    // [0] next event, [1] CTAs done (in the hit container's workspace) or null
 };
 
 struct FitResult { float chi2, b; bool valid; };
@@ -514,8 +515,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   }
   const uint32_t T = __ldg(a.velo_offsets + a.n_events);
 
-  for (int e = blockIdx.x; e < a.n_events; e += gridDim.x) {
+  __shared__ int s_event[2];                       // double-buffered: a slow thread still reads the previous ticket
+  for (int k = 0;; ++k) {
+    // events are dealt out dynamically (CTAs that finish early take more), statically without a workspace
+    if (tid == 0) s_event[k & 1] = a.ticket ? (int)atomicAdd(a.ticket, 1u) : (int)(blockIdx.x + (unsigned)k * gridDim.x);
     __syncthreads();                               // tables staged / previous event fully consumed
+    const int e = s_event[k & 1];
+    if (e >= a.n_events) break;
     const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
     const uint32_t* go = a.hit_offsets + (size_t)e * ng;
     const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
@@ -638,6 +644,10 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       track_loop<false>(a, wa, S, &s_ticket, h0, t0, t1, T);
     }
   }
+  if (tid == 0 && a.ticket) {                 // last CTA out re-arms the ticket for the next call
+    __threadfence();
+    if (atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1) { a.ticket[0] = 0; a.ticket[1] = 0; __threadfence(); }
+  }
 }
 
 static int env_int(const char* name, int dflt) {
@@ -688,6 +698,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
+  a.ticket = hits->workspace ? reinterpret_cast<uint32_t*>(hits->workspace) + 4 : nullptr;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 
   const int C = cfg->max_candidates_per_layer;

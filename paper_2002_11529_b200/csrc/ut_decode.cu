@@ -39,7 +39,7 @@ struct DecodeArgs {
   unsigned long long capacity;
   uint32_t* status;
   uint32_t* hit_offsets;
-  uint32_t* ctrl;               // [0] ticket, [1] CTAs done, [2] epoch
+  uint32_t* ctrl;               // [0] ticket, [1] CTAs done, [2] epoch   ([4], [5]: compass_track's event ticket)
   unsigned long long* flags;    // [n_events] look-back words: epoch:30 | state:2 | value:32
   uint32_t raw_stage_bytes;     // multiple of 16
   uint32_t sort_buf;            // elements of the per-warp sort buffer (multiple of 32)
@@ -417,7 +417,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   a.w = hits->weight; a.id = hits->id; a.capacity = hits->capacity; a.status = hits->status;
   a.hit_offsets = hit_offsets;
   a.ctrl = reinterpret_cast<uint32_t*>(hits->workspace);
-  a.flags = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hits->workspace) + 16);
+  a.flags = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hits->workspace) + 32);
 
   // staging sizes from the only size the host knows without a sync: capacity / n_events
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
