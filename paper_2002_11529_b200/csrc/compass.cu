@@ -215,17 +215,19 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t p1 = S.off[s + 1];
         for (uint32_t p = S.off[s]; p < p1; ++p) {
           const float d = __fsub_rn(__fadd_rn(S.hx[p], syg), x_e);
-          if (fabsf(d) <= D) {
-            const uint32_t hs = ((uint32_t)S.hh[p] << 16) | (uint32_t)s;
-            if (n < C && (n == 0 || last < hs)) {   // hits arrive in ascending index almost always: append
-              wa.cd[n * 32 + slot] = d;
-              wa.chs[n * 32 + slot] = hs;
-              last = hs;
-              ++n;
-            } else {
-              cand_insert(wa, slot, n, C, d, hs);
-              last = wa.chs[(n - 1) * 32 + slot];
-            }
+          if (d > D) break;                         // x-sorted inside the sector: d only grows
+          const bool acc = d >= negD;
+          const uint32_t hs = ((uint32_t)S.hh[p] << 16) | (uint32_t)s;
+          if (acc && (n >= C || (n > 0 && hs <= last))) {   // rare: cap reached or out of hit order
+            cand_insert(wa, slot, n, C, d, hs);
+            last = wa.chs[(n - 1) * 32 + slot];
+            continue;
+          }
+          if (acc) {                                // hits arrive in ascending index almost always: append
+            wa.cd[n * 32 + slot] = d;
+            wa.chs[n * 32 + slot] = hs;
+            last = hs;
+            ++n;
           }
         }
       }
