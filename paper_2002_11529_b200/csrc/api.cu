@@ -10,10 +10,10 @@
 
 namespace utc {
 int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
-                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream);
+                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in);
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream);
+                       cudaStream_t stream, uint32_t idx_stride);
 
 ut_launch_info& launch_info() {
   static thread_local ut_launch_info info = {};
@@ -176,7 +176,8 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
   if (n_events == 0)      // the offsets array still has its single entry
     return cudaMemsetAsync(hit_offsets_out, 0, 4, (cudaStream_t)stream) == cudaSuccess ? UT_OK : UT_ERR_CUDA;
   if (!raw_banks) return UT_ERR_NULL;
-  return launch_decode(raw_banks, bank_offsets, n_events, geometry, hits_out, hit_offsets_out, (cudaStream_t)stream);
+  return launch_decode(raw_banks, bank_offsets, n_events, geometry, hits_out, hit_offsets_out, (cudaStream_t)stream,
+                       nullptr);
 }
 
 int32_t compass_config_default(float p_min_mev, float window_scale, int32_t min_hits, int32_t max_candidates_per_layer,
@@ -212,7 +213,7 @@ int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const ve
       !velo->tx || !velo->ty)
     return UT_ERR_NULL;
   if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
-  return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream);
+  return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream, 0u);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -230,6 +231,9 @@ struct ut_pipeline {
   float *vx, *vy, *vtx, *vty;
   ut_hits hits;
   ut_tracks tracks;
+  // chunked overlap of copies and kernels: copy-in stream, copy-out stream, per-chunk events
+  cudaStream_t s_in, s_out;
+  cudaEvent_t ev_start, ev_out, ev_in[4], ev_done[4];
 };
 
 int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_raw_bytes, uint64_t max_hits,
@@ -263,12 +267,25 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   p->tracks.n_hits = (int32_t*)take(s_v); p->tracks.qop = (float*)take(s_v); p->tracks.chi2 = (float*)take(s_v);
   p->tracks.status = p->status + 1;
   if (cudaMemset(p->block, 0, total) != cudaSuccess) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
+  bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&p->ev_out, cudaEventDisableTiming) == cudaSuccess;
+  for (int k = 0; k < 4 && ok; ++k)
+    ok = cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&p->ev_done[k], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
   *out = p;
   return UT_OK;
 }
 
 int32_t ut_pipeline_destroy(ut_pipeline* p) {
   if (!p) return UT_ERR_NULL;
+  cudaStreamSynchronize(p->s_in);
+  cudaStreamSynchronize(p->s_out);
+  for (int k = 0; k < 4; ++k) { cudaEventDestroy(p->ev_in[k]); cudaEventDestroy(p->ev_done[k]); }
+  cudaEventDestroy(p->ev_start); cudaEventDestroy(p->ev_out);
+  cudaStreamDestroy(p->s_in); cudaStreamDestroy(p->s_out);
   cudaFree(p->block);
   delete p;
   return UT_OK;
@@ -283,25 +300,64 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   if (n_events > 0 && !raw_h) return UT_ERR_NULL;
   cudaStream_t s = (cudaStream_t)stream_;
   const ut_geometry* g = &p->geom;
-  auto h2d = [&](void* d, const void* h, size_t n) { return n == 0 || cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, s) == cudaSuccess; };
-  auto d2h = [&](void* h, const void* d, size_t n) { return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, s) == cudaSuccess; };
-  bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess;
-  ok = ok && h2d(p->raw, raw_h, raw_bytes) && h2d(p->bank_offsets, bo_h, ((size_t)n_events * g->n_sectors + 1) * 4) &&
-       h2d(p->velo_offsets, vo_h, ((size_t)n_events + 1) * 4) && h2d(p->vx, velo_h->x, (size_t)n_velo * 4) &&
-       h2d(p->vy, velo_h->y, (size_t)n_velo * 4) && h2d(p->vtx, velo_h->tx, (size_t)n_velo * 4) &&
-       h2d(p->vty, velo_h->ty, (size_t)n_velo * 4);
+  const uint32_t ns = g->n_sectors, ng = g->n_groups;
+  // The batch is cut into up to 4 chunks of events: chunk k+1 is copied in while chunk k is decoded and
+  // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
+  // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
+  static const int kChunkEvents = [] { const char* v = getenv("UT_PIPELINE_CHUNK_EVENTS"); return v && *v ? atoi(v) : 500; }();
+  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
+  K = K < 1 ? 1 : (K > 4 ? 4 : K);
+  bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
+            cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&
+            cudaStreamWaitEvent(p->s_out, p->ev_start, 0) == cudaSuccess;
   if (!ok) return UT_ERR_CUDA;
-  int32_t rc = ut_decode(p->raw, p->bank_offsets, n_events, g, &p->hits, p->hit_offsets, stream_);
-  if (rc) return rc;
-  int launched = launch_info().kernels_launched;
+  if (n_events == 0) {
+    ok = cudaMemsetAsync(p->hit_offsets, 0, 4, s) == cudaSuccess;
+    if (status_h) ok = ok && cudaMemcpyAsync(status_h, p->status, 8, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (n_hits_h) ok = ok && cudaMemcpyAsync(n_hits_h, p->hit_offsets, 4, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    return ok ? UT_OK : UT_ERR_CUDA;
+  }
+  if (!p->hits.geom->group_first_sector || !p->hits.geom->sector_rows) return UT_ERR_GEOMETRY;
+  if (const int32_t rc = check_config(config)) return rc;
+  auto h2d = [&](void* d, const void* h, size_t n) {
+    return n == 0 || cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
+  };
+  auto d2h = [&](void* h, const void* d, size_t n) {
+    return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
+  };
   velo_states vd = {p->vx, p->vy, p->vtx, p->vty, velo_h->z};
-  rc = compass_track(&p->hits, p->hit_offsets, &vd, p->velo_offsets, n_events, config, &p->tracks, stream_);
-  if (rc) return rc;
-  launch_info().kernels_launched += launched;
-  ok = d2h(tracks_h->hit_idx, p->tracks.hit_idx, (size_t)n_velo * 16) && d2h(tracks_h->n_hits, p->tracks.n_hits, (size_t)n_velo * 4) &&
-       d2h(tracks_h->qop, p->tracks.qop, (size_t)n_velo * 4) && d2h(tracks_h->chi2, p->tracks.chi2, (size_t)n_velo * 4);
+  int launched = 0;
+  for (int k = 0; k < K; ++k) {
+    const int e0 = (int)((long long)n_events * k / K), e1 = (int)((long long)n_events * (k + 1) / K), ne = e1 - e0;
+    const size_t r0 = k == 0 ? 0 : bo_h[(size_t)e0 * ns], r1 = k == K - 1 ? raw_bytes : bo_h[(size_t)e1 * ns];
+    const uint32_t v0 = vo_h[e0], v1 = vo_h[e1];
+    if (r1 < r0 || r1 > raw_bytes || v1 < v0 || v1 > n_velo) return UT_ERR_ARG;
+    ok = h2d(p->raw + r0, raw_h + r0, r1 - r0) &&
+         h2d(p->bank_offsets + (size_t)e0 * ns, bo_h + (size_t)e0 * ns, ((size_t)ne * ns + 1) * 4) &&
+         h2d(p->velo_offsets + e0, vo_h + e0, ((size_t)ne + 1) * 4) &&
+         h2d(p->vx + v0, velo_h->x + v0, (size_t)(v1 - v0) * 4) && h2d(p->vy + v0, velo_h->y + v0, (size_t)(v1 - v0) * 4) &&
+         h2d(p->vtx + v0, velo_h->tx + v0, (size_t)(v1 - v0) * 4) && h2d(p->vty + v0, velo_h->ty + v0, (size_t)(v1 - v0) * 4) &&
+         cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess;
+    if (!ok) return UT_ERR_CUDA;
+    uint32_t* ho = p->hit_offsets + (size_t)e0 * ng;
+    int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &p->hits, ho, s, k == 0 ? nullptr : ho);
+    if (rc) return rc;
+    launched += launch_info().kernels_launched;
+    rc = launch_compass(&p->hits, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo);
+    if (rc) return rc;
+    launched += launch_info().kernels_launched;
+    ok = cudaEventRecord(p->ev_done[k], s) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess;
+    for (int l = 0; l < 4 && ok; ++l)
+      ok = d2h(tracks_h->hit_idx + (size_t)l * n_velo + v0, p->tracks.hit_idx + (size_t)l * n_velo + v0, (size_t)(v1 - v0) * 4);
+    ok = ok && d2h(tracks_h->n_hits + v0, p->tracks.n_hits + v0, (size_t)(v1 - v0) * 4) &&
+         d2h(tracks_h->qop + v0, p->tracks.qop + v0, (size_t)(v1 - v0) * 4) &&
+         d2h(tracks_h->chi2 + v0, p->tracks.chi2 + v0, (size_t)(v1 - v0) * 4);
+    if (!ok) return UT_ERR_CUDA;
+  }
+  launch_info().kernels_launched = launched;
   if (status_h) ok = ok && d2h(status_h, p->status, 8);
-  if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * g->n_groups, 4);
+  if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * ng, 4);
+  ok = ok && cudaEventRecord(p->ev_out, p->s_out) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_out, 0) == cudaSuccess;
   return ok ? UT_OK : UT_ERR_CUDA;
 }
 

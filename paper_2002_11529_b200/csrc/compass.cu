@@ -59,6 +59,7 @@ struct CompassArgs {
   float *out_qop, *out_chi2;
   uint32_t* status;
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
+  uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
   uint32_t* ticket;                    // [0] next event, [1] CTAs done (in the hit container's workspace) or null
 };
 
@@ -515,7 +516,8 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     wa.best = reinterpret_cast<unsigned long long*>(p + (size_t)C * 32 * 8 + kSeedQ * 8);
     wa.n = reinterpret_cast<int*>(p + (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8);
   }
-  const uint32_t T = __ldg(a.velo_offsets + a.n_events);
+  const uint32_t Tend = __ldg(a.velo_offsets + a.n_events);
+  const uint32_t T = a.idx_stride ? a.idx_stride : Tend;
 
   __shared__ int s_event[2];                       // double-buffered: a slow thread still reads the previous ticket
   for (int k = 0;; ++k) {
@@ -527,7 +529,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
     const uint32_t* go = a.hit_offsets + (size_t)e * ng;
     const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
-    if (t1 < t0 || t1 > T) {                       // inconsistent VELO offsets: nothing can be written safely
+    if (t1 < t0 || t1 > Tend) {                       // inconsistent VELO offsets: nothing can be written safely
       if (tid == 0) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_OFFSETS);
       continue;
     }
@@ -672,7 +674,7 @@ static const void* const kKernelLarge = reinterpret_cast<const void*>(&compass_k
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream) {
+                       cudaStream_t stream, uint32_t idx_stride) {
   static int max_smem = 0, n_sm = 0, sm_smem = 0;     // max_smem = largest dynamic size a CTA may ask for
   if (!max_smem) {
     int dev = 0, optin = 0;
@@ -700,6 +702,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
+  a.idx_stride = idx_stride;
   a.ticket = hits->workspace ? reinterpret_cast<uint32_t*>(hits->workspace) + 4 : nullptr;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 

@@ -43,6 +43,7 @@ struct DecodeArgs {
   unsigned long long* flags;    // [n_events] look-back words: epoch:30 | state:2 | value:32
   uint32_t raw_stage_bytes;     // multiple of 16
   uint32_t sort_buf;            // elements of the per-warp sort buffer (multiple of 32)
+  const uint32_t* carry_in;     // hits in front of event 0 (chunked pipeline) or null
 };
 
 __device__ __forceinline__ float decode_x(uint32_t word, float x0, float pitch) {
@@ -53,11 +54,13 @@ __device__ __forceinline__ float decode_x(uint32_t word, float x0, float pitch) 
 
 // Chained exclusive prefix over events (decoupled look-back).  Called by warp 0.  Event e only waits
 // for events with a smaller ticket, which are running or finished, so it always makes progress.
-__device__ uint32_t event_base_lookback(unsigned long long* flags, int e, uint32_t tot, uint32_t epoch, int lane) {
+__device__ uint32_t event_base_lookback(unsigned long long* flags, int e, uint32_t tot, uint32_t epoch, int lane,
+                                        const uint32_t* carry_in) {
   const unsigned long long tag = (unsigned long long)(epoch & 0x3FFFFFFFu) << 34;
   if (e == 0) {
-    if (lane == 0) st_volatile_u64(&flags[0], tag | (2ull << 32) | tot);
-    return 0;
+    const uint32_t carry = carry_in ? ld_volatile_u32(carry_in) : 0u;
+    if (lane == 0) st_volatile_u64(&flags[0], tag | (2ull << 32) | (unsigned long long)(carry + tot));
+    return carry;
   }
   if (lane == 0) st_volatile_u64(&flags[e], tag | (1ull << 32) | tot);
   uint32_t base = 0;
@@ -224,7 +227,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
     uint32_t base = 0;
     bool have_base = false;
     if (warp == 0) {
-      base = event_base_lookback(a.flags, e, tot, s_epoch, lane);
+      base = event_base_lookback(a.flags, e, tot, s_epoch, lane, a.carry_in);
       have_base = true;
       if (lane == 0) {
         s_base = base;
@@ -398,7 +401,7 @@ static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t idn, uint32_t
 }
 
 int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
-                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream) {
+                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in) {
   static int n_sm = 0, max_smem = 0;     // max_smem = largest dynamic size this kernel may ask for
   if (!n_sm) {
     int dev = 0, optin = 0;
@@ -416,6 +419,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   a.x = hits->x_at_y0; a.z = hits->z_at_y0; a.yb = hits->y_begin; a.ye = hits->y_end; a.dxdy = hits->dxdy;
   a.w = hits->weight; a.id = hits->id; a.capacity = hits->capacity; a.status = hits->status;
   a.hit_offsets = hit_offsets;
+  a.carry_in = carry_in;
   a.ctrl = reinterpret_cast<uint32_t*>(hits->workspace);
   a.flags = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hits->workspace) + 32);
 

@@ -255,3 +255,36 @@ def test_invalid_arguments(gpu, wl):
             B.compass_track(hits, hits.hit_offsets, velo, vo, 1, B.make_config(bad), tracks)
     with pytest.raises(B.UTError):
         B.ut_decode(B.to_device_raw(b.raw), B.to_device_u32(b.bank_offsets), -1, gpu.geom, hits)
+
+
+@pytest.mark.parametrize("n_events", [1000, 37])
+def test_host_pipeline_matches_oracle(gpu, wl, n_events):
+    """ut_pipeline_run_host (HOST buffers in, HOST track SoA out; the call bench.py's e2e figure times).
+    1000 events run as overlapped chunks, 37 events as one: both must equal the oracle element by element."""
+    import torch
+    geom, b, p = wl(3, n_events)
+    h_ref, t_ref = oracle_run(b, geom, p)
+    B = gpu.B
+    T = b.n_velo_total
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    raw_h = pin(np.concatenate([b.raw, np.zeros(32, np.uint8)]))
+    bo_h, vo_h = pin(b.bank_offsets.view(np.int32)), pin(b.velo_offsets.view(np.int32))
+    velo_h = [pin(v) for v in (b.velo_x, b.velo_y, b.velo_tx, b.velo_ty)]
+    out_h = {"hit_idx": torch.full((4 * T,), -7, dtype=torch.int32).pin_memory(),
+             "n_hits": torch.full((T,), -7, dtype=torch.int32).pin_memory(),
+             "qop": torch.zeros(T, dtype=torch.float32).pin_memory(),
+             "chi2": torch.zeros(T, dtype=torch.float32).pin_memory(),
+             "status": torch.full((2,), -1, dtype=torch.int32).pin_memory(),
+             "n_hits_total": torch.zeros(1, dtype=torch.int32).pin_memory()}
+    pipe = B.Pipeline(gpu.geom, b.n_events, int(b.raw.size) + 32, b.hit_capacity, T)
+    for _ in range(2):                                   # second run: workspace and events are reused
+        pipe.run_host(raw_h, int(b.raw.size), bo_h, velo_h, b.velo_z, vo_h, T, b.n_events, B.make_config(p), out_h)
+        torch.cuda.synchronize()
+        assert int(out_h["n_hits_total"][0]) == h_ref.n_hits
+        assert out_h["status"].tolist() == [0, 0]
+        assert np.array_equal(out_h["hit_idx"].numpy().reshape(4, T), t_ref.hit_idx)
+        assert np.array_equal(out_h["n_hits"].numpy(), t_ref.n_hits)
+        assert np.array_equal(out_h["chi2"].numpy().view(np.uint32), t_ref.chi2.view(np.uint32))
+        assert np.array_equal(out_h["qop"].numpy().view(np.uint32), t_ref.qop.view(np.uint32))
+        out_h["n_hits"].fill_(-7)
+    pipe.destroy()
