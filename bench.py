@@ -354,6 +354,21 @@ def main():
         events_all = float(batch.n_events)
     clocks = sampler.stop() if sampler else None
 
+    # ---- SURVEY.md 8(f) row 1 (not part of the step): compacted track output, timed on its own ----
+    compact = B.CompactTracks(batch.n_velo_total, batch.n_velo_total, batch.n_events)
+    evc = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(min(args.steps, 50))]
+    for _ in range(3):
+        B.compass_consolidate(tracks, vo_d, batch.n_events, compact)
+    for a_, b_ in evc:
+        flush.zero_()
+        a_.record(stream)
+        B.compass_consolidate(tracks, vo_d, batch.n_events, compact)
+        b_.record(stream)
+    torch.cuda.synchronize()
+    t_cons = statistics.mean(a_.elapsed_time(b_) for a_, b_ in evc)
+    n_compact = int(compact.track_offsets[batch.n_events].item())
+    cons_bytes = 28 * batch.n_velo_total + 4 * (batch.n_events + 1) + 32 * n_compact + 4 * (batch.n_events + 1)
+
     # ---- end to end through the host-buffer C-ABI call (H2D + kernels + D2H inside the timed region) ----
     e2e = None
     if not args.no_e2e:
@@ -444,6 +459,10 @@ def main():
         "median_ms": {"decode": statistics.median(t_dec), "compass": statistics.median(t_cmp),
                       "step": statistics.median(t_step), "step_min": min(t_step)},
         "wall_events_per_s_incl_flush": batch.n_events * args.steps / t_wall,
+        "next_rows": {"compass_consolidate": {"ms": t_cons, "tracklets": n_compact, "bytes": int(cons_bytes),
+                                               "gbs": cons_bytes / t_cons / 1e6,
+                                               "frac_hbm": cons_bytes / t_cons / 1e6 / hbm_peak,
+                                               "note": "SURVEY.md 8(f) row 1, timed alone, not part of the step"}},
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(batch, geom_t, params)

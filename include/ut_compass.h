@@ -175,6 +175,35 @@ int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const ve
                       const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
                       ut_tracks* tracks_out, ut_stream_t stream);
 
+/* Compacted VELO+UT track container ("a prefix sum and a consolidation of the tracks", which
+ * replaces the atomicAdd slot allocation of PAPER.md:348): only the VELO tracks that got a tracklet, events
+ * ascending and the VELO order inside an event kept, so the result is unique.  Arrays have `capacity`
+ * elements (n_velo_total is always enough); hit_idx has row stride `capacity`. */
+typedef struct {
+  uint32_t* velo_index; /* [capacity] global VELO track index of the tracklet */
+  int32_t* hit_idx;     /* [4][capacity] */
+  int32_t* n_hits;      /* [capacity] 3 or 4 */
+  float* qop;           /* [capacity] */
+  float* chi2;          /* [capacity] */
+  uint64_t capacity;
+  uint32_t* status;     /* device word; UT_STATUS_CAPACITY if the tracklets do not fit (nothing past capacity
+                           is written, track_offsets_out stays exact) */
+  void* workspace;      /* device, compass_consolidate_workspace_bytes(max_velo_total) bytes, zeroed once;
+                           reusable across calls on one stream */
+  uint32_t max_velo_total; /* what the workspace was sized for; n_velo_total above it sets UT_STATUS_BAD_OFFSETS
+                              and nothing is written */
+} ut_compact_tracks;
+
+size_t compass_consolidate_workspace_bytes(uint32_t max_velo_total);
+
+/* compass_consolidate -- PAPER.md:460.  One launch: tiles of 1024 VELO tracks by atomic ticket, block scan of
+ * the "has a tracklet" flags, chained exclusive prefix over tiles (decoupled look-back), coalesced stores.
+ * tracks, velo_offsets : as given to / filled by compass_track (n_velo_total = velo_offsets[n_events], read on
+ *                        the device; the row stride of tracks->hit_idx is n_velo_total).
+ * track_offsets_out    : device u32 [n_events + 1]: event e owns compact tracks [off[e], off[e+1]). */
+int32_t compass_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events,
+                            ut_compact_tracks* out, uint32_t* track_offsets_out, ut_stream_t stream);
+
 /* End-to-end convenience for HOST buffers (bench.py "e2e"): H2D of raw banks, offsets and VELO
  * states, ut_decode, compass_track, D2H of the track SoA, all asynchronous on `stream`.
  * The arena holds the device staging buffers (library-owned). Host buffers should be pinned. */

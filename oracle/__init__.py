@@ -66,6 +66,7 @@ def _load():
             lib.oracle_decode.restype = C.c_int32
             lib.oracle_compass.restype = C.c_int32
             lib.oracle_fit.restype = C.c_int32
+            lib.oracle_consolidate.restype = C.c_int32
             _lib = lib
     return _lib
 
@@ -205,3 +206,35 @@ def run_batch(batch, geom, params, mode: int = 0):
     t = compass(h, batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z, batch.velo_offsets,
                 batch.n_events, geom, params, mode)
     return h, t
+
+
+@dataclass
+class CompactTracks:
+    velo_index: np.ndarray       # u32 [K]
+    hit_idx: np.ndarray          # i32 [4, K]
+    n_hits: np.ndarray           # i32 [K]
+    qop: np.ndarray              # f32 [K]
+    chi2: np.ndarray             # f32 [K]
+    track_offsets: np.ndarray    # u32 [n_events + 1]
+    status: int
+
+
+def consolidate(hit_idx, n_hits, qop, chi2, velo_offsets, n_events: int, capacity: int | None = None) -> CompactTracks:
+    """PAPER.md:460 as the plain definition: keep the tracks with a tracklet, in order."""
+    lib = _load()
+    T = int(velo_offsets[n_events])
+    cap = T if capacity is None else int(capacity)
+    hit_idx = np.ascontiguousarray(hit_idx, np.int32).reshape(4, T)
+    n_hits, qop, chi2 = (np.ascontiguousarray(n_hits, np.int32), np.ascontiguousarray(qop, np.float32),
+                         np.ascontiguousarray(chi2, np.float32))
+    vo = np.ascontiguousarray(velo_offsets, np.uint32)
+    o_v = np.zeros(max(cap, 1), np.uint32); o_i = np.full((4, max(cap, 1)), -1, np.int32)
+    o_n = np.zeros(max(cap, 1), np.int32); o_q = np.zeros(max(cap, 1), np.float32); o_c = np.zeros(max(cap, 1), np.float32)
+    off = np.zeros(n_events + 1, np.uint32)
+    st = C.c_uint32(0)
+    rc = lib.oracle_consolidate(_p(hit_idx), _p(n_hits), _p(qop), _p(chi2), _p(vo), C.c_int32(n_events), _p(o_v),
+                                _p(o_i), _p(o_n), _p(o_q), _p(o_c), C.c_uint64(cap), _p(off), C.byref(st))
+    if rc != 0:
+        raise RuntimeError(f"oracle_consolidate rc={rc}")
+    K = min(int(off[-1]), cap)
+    return CompactTracks(o_v[:K], o_i[:, :K] if cap else o_i[:, :0], o_n[:K], o_q[:K], o_c[:K], off, int(st.value))

@@ -426,4 +426,34 @@ int32_t oracle_fit(int32_t n, const float* d, const float* z, const float* w, co
   return 0;
 }
 
+// Compacted VELO+UT tracks: the plain definition.  Walk the events in
+// order and the VELO tracks of each event in order; every track with a tracklet (n_hits > 0) is appended.
+// track_offsets[e] = number of tracklets in front of event e.  Nothing past `capacity` is written (status 8),
+// the offsets stay exact.  hit_idx in has row stride T, hit_idx_out row stride `capacity`.
+int32_t oracle_consolidate(const int32_t* hit_idx, const int32_t* n_hits, const float* qop, const float* chi2,
+                           const uint32_t* velo_offsets, int32_t n_events, uint32_t* velo_index_out,
+                           int32_t* hit_idx_out, int32_t* n_hits_out, float* qop_out, float* chi2_out,
+                           uint64_t capacity, uint32_t* track_offsets, uint32_t* status) {
+  const uint64_t T = velo_offsets[n_events];
+  uint64_t k = 0;
+  for (int32_t e = 0; e < n_events; ++e) {
+    track_offsets[e] = (uint32_t)k;
+    for (uint64_t t = velo_offsets[e]; t < velo_offsets[e + 1]; ++t) {
+      if (n_hits[t] <= 0) continue;
+      if (k < capacity) {
+        velo_index_out[k] = (uint32_t)t;
+        for (int l = 0; l < 4; ++l) hit_idx_out[(uint64_t)l * capacity + k] = hit_idx[(uint64_t)l * T + t];
+        n_hits_out[k] = n_hits[t];
+        qop_out[k] = qop[t];
+        chi2_out[k] = chi2[t];
+      } else {
+        *status |= 8u;
+      }
+      ++k;
+    }
+  }
+  track_offsets[n_events] = (uint32_t)k;
+  return 0;
+}
+
 }  // extern "C"

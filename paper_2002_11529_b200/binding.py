@@ -61,6 +61,12 @@ class ut_tracks(C.Structure):
                 ("status", C.c_void_p)]
 
 
+class ut_compact_tracks(C.Structure):
+    _fields_ = [("velo_index", C.c_void_p), ("hit_idx", C.c_void_p), ("n_hits", C.c_void_p), ("qop", C.c_void_p),
+                ("chi2", C.c_void_p), ("capacity", C.c_uint64), ("status", C.c_void_p), ("workspace", C.c_void_p),
+                ("max_velo_total", C.c_uint32)]
+
+
 class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_buckets_per_group",
@@ -69,7 +75,7 @@ class ut_launch_info(C.Structure):
 
 EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
-           "compass_track", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
+           "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
            "ut_pipeline_device_hits"]
 
 _lib.ut_version.restype = C.c_char_p
@@ -85,6 +91,10 @@ _lib.compass_config_default.argtypes = [C.c_float, C.c_float, C.c_int32, C.c_int
                                         C.POINTER(compass_config)]
 _lib.compass_track.argtypes = [C.POINTER(ut_hits), C.c_void_p, C.POINTER(velo_states), C.c_void_p, C.c_int32,
                                C.POINTER(compass_config), C.POINTER(ut_tracks), C.c_void_p]
+_lib.compass_consolidate_workspace_bytes.restype = C.c_size_t
+_lib.compass_consolidate_workspace_bytes.argtypes = [C.c_uint32]
+_lib.compass_consolidate.argtypes = [C.POINTER(ut_tracks), C.c_void_p, C.c_int32, C.POINTER(ut_compact_tracks),
+                                     C.c_void_p, C.c_void_p]
 _lib.ut_pipeline_create.argtypes = [C.POINTER(ut_geometry), C.c_int32, C.c_size_t, C.c_uint64, C.c_uint32,
                                     C.POINTER(C.c_void_p)]
 _lib.ut_pipeline_destroy.argtypes = [C.c_void_p]
@@ -94,7 +104,8 @@ _lib.ut_pipeline_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_vo
 _lib.ut_pipeline_device_hits.argtypes = [C.c_void_p, C.POINTER(ut_hits), C.POINTER(C.c_void_p)]
 _lib.ut_last_launch_info.argtypes = [C.POINTER(ut_launch_info)]
 for _n in EXPORTS:
-    if _n not in ("ut_version", "ut_last_error", "ut_decode_workspace_bytes", "ut_last_launch_info"):
+    if _n not in ("ut_version", "ut_last_error", "ut_decode_workspace_bytes", "ut_last_launch_info",
+                  "compass_consolidate_workspace_bytes"):
         getattr(_lib, _n).restype = C.c_int32
 
 
@@ -195,6 +206,47 @@ class Tracks:
         n = self.n
         return (self.hit_idx[:4 * n].cpu().numpy().reshape(4, n), self.n_hits[:n].cpu().numpy(),
                 self.qop[:n].cpu().numpy(), self.chi2[:n].cpu().numpy())
+
+
+class CompactTracks:
+    """Caller-owned compacted track container (compass_consolidate) + the per-event offsets."""
+
+    def __init__(self, capacity: int, max_velo_total: int, max_events: int, device="cuda"):
+        n = max(int(capacity), 1)
+        self.capacity = int(capacity)
+        self.velo_index = torch.empty(n, dtype=torch.int32, device=device)
+        self.hit_idx = torch.empty(4 * n, dtype=torch.int32, device=device)
+        self.n_hits = torch.empty(n, dtype=torch.int32, device=device)
+        self.qop = torch.empty(n, dtype=torch.float32, device=device)
+        self.chi2 = torch.empty(n, dtype=torch.float32, device=device)
+        self.status = torch.zeros(1, dtype=torch.int32, device=device)
+        nbytes = int(_lib.compass_consolidate_workspace_bytes(int(max_velo_total)))
+        self.workspace = torch.zeros((nbytes + 15) // 16 * 2, dtype=torch.int64, device=device)   # zeroed once
+        self.track_offsets = torch.zeros(max_events + 1, dtype=torch.int32, device=device)
+        self.c = ut_compact_tracks(self.velo_index.data_ptr(), self.hit_idx.data_ptr(), self.n_hits.data_ptr(),
+                                   self.qop.data_ptr(), self.chi2.data_ptr(), self.capacity, self.status.data_ptr(),
+                                   self.workspace.data_ptr(), int(max_velo_total))
+
+    def numpy(self, n_events: int):
+        off = self.track_offsets[:n_events + 1].cpu().numpy().view(np.uint32)
+        k = min(int(off[-1]), self.capacity)
+        cap = max(self.capacity, 1)
+        return dict(velo_index=self.velo_index[:k].cpu().numpy().view(np.uint32),
+                    hit_idx=self.hit_idx.cpu().numpy().reshape(4, cap)[:, :k], n_hits=self.n_hits[:k].cpu().numpy(),
+                    qop=self.qop[:k].cpu().numpy(), chi2=self.chi2[:k].cpu().numpy(), track_offsets=off,
+                    status=int(self.status.item()) & 0xFFFFFFFF)
+
+
+def compass_consolidate(tracks: Tracks, velo_offsets: torch.Tensor, n_events: int, out: CompactTracks,
+                        stream=None) -> int:
+    rc = _lib.compass_consolidate(C.byref(tracks.c), velo_offsets.data_ptr(), n_events, C.byref(out.c),
+                                  out.track_offsets.data_ptr(), _stream_ptr(stream))
+    _check(rc, "compass_consolidate")
+    return rc
+
+
+def compass_consolidate_workspace_bytes(max_velo_total: int) -> int:
+    return int(_lib.compass_consolidate_workspace_bytes(int(max_velo_total)))
 
 
 def make_config(params) -> compass_config:

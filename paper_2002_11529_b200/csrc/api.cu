@@ -15,6 +15,10 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
                        cudaStream_t stream, uint32_t idx_stride);
 
+size_t consolidate_workspace_bytes(uint32_t max_velo);
+int32_t launch_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events, uint32_t n_velo_hint,
+                           ut_compact_tracks* out, uint32_t* track_offsets, cudaStream_t stream);
+
 ut_launch_info& launch_info() {
   static thread_local ut_launch_info info = {};
   return info;
@@ -219,6 +223,21 @@ int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const ve
 // ---------------------------------------------------------------------------------------------------
 // Host-buffer pipeline (bench.py "e2e"): one arena of device buffers, async copies around the two calls.
 // ---------------------------------------------------------------------------------------------------
+size_t compass_consolidate_workspace_bytes(uint32_t max_velo_total) { return consolidate_workspace_bytes(max_velo_total); }
+
+int32_t compass_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events,
+                            ut_compact_tracks* out, uint32_t* track_offsets_out, ut_stream_t stream) {
+  launch_info().kernels_launched = 0;
+  if (!tracks || !velo_offsets || !out || !track_offsets_out) return UT_ERR_NULL;
+  if (n_events < 0) return UT_ERR_ARG;
+  if (!out->status || !out->workspace) return UT_ERR_NULL;
+  if (reinterpret_cast<uintptr_t>(out->workspace) & 15u) return UT_ERR_ARG;
+  if (n_events == 0) return cudaMemsetAsync(track_offsets_out, 0, 4, (cudaStream_t)stream) == cudaSuccess ? UT_OK : UT_ERR_CUDA;
+  if (out->capacity > 0 && (!out->velo_index || !out->hit_idx || !out->n_hits || !out->qop || !out->chi2)) return UT_ERR_NULL;
+  if (out->max_velo_total > 0 && (!tracks->hit_idx || !tracks->n_hits || !tracks->qop || !tracks->chi2)) return UT_ERR_NULL;
+  return launch_consolidate(tracks, velo_offsets, n_events, out->max_velo_total, out, track_offsets_out, (cudaStream_t)stream);
+}
+
 struct ut_pipeline {
   ut_geometry geom;
   int32_t max_events;

@@ -109,6 +109,41 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
   return v;
 }
 
+// Chained exclusive prefix over work items handed out by an atomic ticket (decoupled look-back; the decode
+// chains events, the track consolidation chains tiles).  Called by one warp.  Item e only waits for items with a
+// smaller ticket, which are running or finished, so it always makes progress.  flags[e] = epoch:30 | state:2 |
+// value:32 with state 1 = the item's own total, 2 = inclusive prefix; the epoch makes the words reusable.
+__device__ inline uint32_t event_base_lookback(unsigned long long* flags, int e, uint32_t tot, uint32_t epoch, int lane,
+                                        const uint32_t* carry_in) {
+  const unsigned long long tag = (unsigned long long)(epoch & 0x3FFFFFFFu) << 34;
+  if (e == 0) {
+    const uint32_t carry = carry_in ? ld_volatile_u32(carry_in) : 0u;
+    if (lane == 0) st_volatile_u64(&flags[0], tag | (2ull << 32) | (unsigned long long)(carry + tot));
+    return carry;
+  }
+  if (lane == 0) st_volatile_u64(&flags[e], tag | (1ull << 32) | tot);
+  uint32_t base = 0;
+  int idx = e - 1 - lane;
+  for (;;) {
+    unsigned long long v = 0;
+    if (idx >= 0) {
+      do { v = ld_volatile_u64(&flags[idx]); } while ((v >> 34) != (tag >> 34) || ((v >> 32) & 3ull) == 0ull);
+    }
+    const bool incl = idx >= 0 && ((v >> 32) & 3ull) == 2ull;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, incl);
+    uint32_t val = idx >= 0 ? (uint32_t)v : 0u;
+    if (m) {
+      const int first = __ffs(m) - 1;                    // closest predecessor with an inclusive prefix
+      base += warp_sum(lane <= first ? val : 0u);
+      break;
+    }
+    base += warp_sum(val);
+    idx -= 32;
+  }
+  if (lane == 0) st_volatile_u64(&flags[e], tag | (2ull << 32) | (unsigned long long)(base + tot));
+  return base;
+}
+
 // bump allocator over dynamic shared memory, 16-byte granules
 struct Carver {
   unsigned char* p;

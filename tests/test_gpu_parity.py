@@ -288,3 +288,63 @@ def test_host_pipeline_matches_oracle(gpu, wl, n_events):
         assert np.array_equal(out_h["qop"].numpy().view(np.uint32), t_ref.qop.view(np.uint32))
         out_h["n_hits"].fill_(-7)
     pipe.destroy()
+
+
+def _consolidate_both(gpu, t_idx, t_n, t_qop, t_chi2, vo, n_events, capacity=None):
+    """compass_consolidate on device copies of a dense track SoA vs oracle.consolidate."""
+    import torch
+    B = gpu.B
+    T = int(vo[n_events])
+    cap = T if capacity is None else capacity
+    tr = B.Tracks(T)
+    if T:
+        tr.hit_idx[:4 * T] = torch.from_numpy(np.ascontiguousarray(t_idx, np.int32).reshape(-1)).cuda()
+        tr.n_hits[:T] = torch.from_numpy(np.ascontiguousarray(t_n)).cuda()
+        tr.qop[:T] = torch.from_numpy(np.ascontiguousarray(t_qop)).cuda()
+        tr.chi2[:T] = torch.from_numpy(np.ascontiguousarray(t_chi2)).cuda()
+    out = B.CompactTracks(cap, T, n_events)
+    vo_d = B.to_device_u32(vo)
+    for _ in range(2):                                   # the look-back workspace re-arms itself
+        out.track_offsets.fill_(-1)
+        B.compass_consolidate(tr, vo_d, n_events, out)
+        torch.cuda.synchronize()
+    got = out.numpy(n_events)
+    ref = oracle.consolidate(t_idx, t_n, t_qop, t_chi2, vo, n_events, cap)
+    assert got["status"] == ref.status
+    assert np.array_equal(got["track_offsets"], ref.track_offsets)
+    assert np.array_equal(got["velo_index"], ref.velo_index)
+    assert np.array_equal(got["hit_idx"], ref.hit_idx) and np.array_equal(got["n_hits"], ref.n_hits)
+    assert np.array_equal(got["qop"].view(np.uint32), ref.qop.view(np.uint32))
+    assert np.array_equal(got["chi2"].view(np.uint32), ref.chi2.view(np.uint32))
+    return ref
+
+
+def test_consolidate_full_size(gpu, wl):
+    """PAPER.md:460 on the Compass output of configs[2] and configs[3] at full size (147 / 586 tiles)."""
+    for c in (3, 4):
+        geom, b, p = wl(c)
+        _, t = oracle_run(b, geom, p)
+        ref = _consolidate_both(gpu, t.hit_idx, t.n_hits, t.qop, t.chi2, b.velo_offsets, b.n_events)
+        assert 0 < len(ref.velo_index) < b.n_velo_total
+
+
+def test_consolidate_edge_cases(gpu):
+    rng = np.random.default_rng(3)
+
+    def tracks(nt, p_keep):
+        vo = np.concatenate([[0], np.cumsum(nt)]).astype(np.uint32)
+        T = int(vo[-1])
+        n = np.where(rng.random(T) < p_keep, rng.integers(3, 5, T), 0).astype(np.int32)
+        idx = np.where(n[None, :] > 0, rng.integers(0, 10 ** 6, (4, T)), -1).astype(np.int32)
+        return idx, n, rng.normal(0, 1, T).astype(np.float32), rng.random(T).astype(np.float32), vo
+
+    for nt, pk in (([0, 0, 0], 0.5),                          # no VELO tracks at all
+                   ([2048, 0, 0, 2048, 1], 0.5),              # boundaries exactly on tile edges, empty events
+                   ([4096], 1.0), ([4095, 1], 0.0),           # everything / nothing kept
+                   ([5000, 3, 0, 7000, 1, 1, 1], 0.7),
+                   (rng.poisson(3, 3000), 0.9)):              # many events per tile
+        a = tracks(np.asarray(nt), pk)
+        _consolidate_both(gpu, *a, len(nt))
+    a = tracks(np.asarray([3000, 3000]), 1.0)
+    ref = _consolidate_both(gpu, *a, 2, capacity=4100)        # capacity: offsets stay exact, nothing past the end
+    assert ref.status == 8
