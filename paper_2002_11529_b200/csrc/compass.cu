@@ -214,7 +214,14 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
         if (!(y_e <= yr.y)) continue;
         const uint32_t p1 = S.off[s + 1];
-        for (uint32_t p = S.off[s]; p < p1; ++p) {
+        uint32_t p = S.off[s];
+        if (p1 - p > 6u) {                          // busy sector: lower bound of d >= -D
+          for (uint32_t cnt = p1 - p; cnt > 0;) {
+            const uint32_t half = cnt >> 1, mid = p + half;
+            if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= negD) cnt = half; else { p = mid + 1; cnt -= half + 1; }
+          }
+        }
+        for (; p < p1; ++p) {
           const float d = __fsub_rn(__fadd_rn(S.hx[p], syg), x_e);
           if (d > D) break;                         // x-sorted inside the sector: d only grows
           const bool acc = d >= negD;
