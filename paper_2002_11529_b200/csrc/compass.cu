@@ -59,6 +59,8 @@ struct CompassArgs {
   float *out_qop, *out_chi2;
   uint32_t* status;
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
+  unsigned long long capacity;         // elements of the hit arrays (bulk copies never read past it)
+  uint32_t bulk_ok;                    // hit arrays are 16-byte aligned: the event's x and id ranges come by TMA
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
   uint32_t* ticket;                    // [0] next event, [1] CTAs done (in the hit container's workspace) or null
 };
@@ -493,8 +495,14 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage);
   unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by s_cnt below
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp_areas);
+  // while staging, the same region also receives the event's id and x ranges by two bulk copies (TMA)
+  uint32_t* s_tmp_id = reinterpret_cast<uint32_t*>(s_warp_areas + align16((size_t)ns * 8));
+  float* s_tmp_x = reinterpret_cast<float*>(s_warp_areas + align16((size_t)ns * 8) + align16((size_t)(a.hit_stage + 8) * 4));
   __shared__ float2 s_lay[4];
   __shared__ int s_ticket;
+  __shared__ uint64_t s_bar;
+  uint32_t bar_phase = 0;
+  if (tid == 0) { mbar_init(&s_bar, 1); fence_mbar_init(); }
   const uint32_t lt_mask = (1u << lane) - 1u;
 
   // ---- geometry tables, once per CTA ---------------------------------------------------------------------
@@ -563,6 +571,23 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       // ---- stage: a warp re-buckets one sector group at a time, per sector, keeping the x order -----------
       // (count -> warp scan over the group's sectors -> ordered scatter with match.any; no block barrier)
       bool bad_id = false;
+      // the event's ids and x by two bulk copies over the 16-byte aligned superset of [h0, h1)
+      const uint32_t c0 = h0 & ~3u, c1 = (h1 + 3u) & ~3u;
+      const bool bulk = a.bulk_ok && (unsigned long long)c1 <= a.capacity && n > 0;
+      const uint32_t* idp = a.hid + h0;
+      const float* xp = a.hx + h0;
+      if (bulk) {
+        if (tid == 0) {
+          fence_proxy_async();               // earlier generic-proxy accesses of the region are done (barrier above)
+          mbar_expect_tx(&s_bar, 2u * (c1 - c0) * 4u);
+          bulk_g2s(s_tmp_id, a.hid + c0, (c1 - c0) * 4u, &s_bar);
+          bulk_g2s(s_tmp_x, a.hx + c0, (c1 - c0) * 4u, &s_bar);
+        }
+        mbar_wait(&s_bar, bar_phase);
+        bar_phase ^= 1u;
+        idp = s_tmp_id + (h0 - c0);
+        xp = s_tmp_x + (h0 - c0);
+      }
       for (uint32_t g = warp; g < ng; g += nwarps) {
         const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
         const uint32_t sa = s_gB[g].y & 0xFFFFu, sb = s_gB[g].y >> 16;
@@ -577,16 +602,16 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
           uint32_t sec0 = kInvalid, sec1 = kInvalid;
           float x0 = 0.f, x1 = 0.f;
           if (i0 < gb) {
-            const uint32_t rid = __ldg(a.hid + h0 + i0) >> 9;
+            const uint32_t rid = idp[i0] >> 9;
             sec0 = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
             if (!(sec0 >= sa && sec0 < sb)) { sec0 = kInvalid; bad_id = true; }
-            x0 = __ldg(a.hx + h0 + i0);
+            x0 = xp[i0];
           }
           if (i1 < gb) {
-            const uint32_t rid = __ldg(a.hid + h0 + i1) >> 9;
+            const uint32_t rid = idp[i1] >> 9;
             sec1 = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
             if (!(sec1 >= sa && sec1 < sb)) { sec1 = kInvalid; bad_id = true; }
-            x1 = __ldg(a.hx + h0 + i1);
+            x1 = xp[i1];
           }
           const uint32_t peers0 = __match_any_sync(0xFFFFFFFFu, sec0);
           const uint32_t rank0 = __popc(peers0 & lt_mask);
@@ -612,7 +637,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
         for (uint32_t s = sa + lane; s < sb; s += 32) s_cnt[s] = 0;
         __syncwarp();
         for (uint32_t i = ga + lane; i < gb; i += 32) {
-          const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+          const uint32_t rid = idp[i] >> 9;
           const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
           if (s >= sa && s < sb) atomicAdd(&s_cnt[s], 1u); else bad_id = true;
         }
@@ -631,10 +656,10 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
           uint32_t s = kInvalid;
           float x = 0.f;
           if (i < gb) {
-            const uint32_t rid = __ldg(a.hid + h0 + i) >> 9;
+            const uint32_t rid = idp[i] >> 9;
             s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
             if (!(s >= sa && s < sb)) s = kInvalid;
-            x = __ldg(a.hx + h0 + i);
+            x = xp[i];
           }
           const uint32_t peers = __match_any_sync(0xFFFFFFFFu, s);
           const uint32_t rank = __popc(peers & lt_mask);
@@ -670,7 +695,8 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, i
   size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + align16((size_t)ns * 8);
   b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
   b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
-  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)), align16((size_t)ns * 8));
+  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)),
+                align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4));   // staging scratch aliases the warp areas
   return b;
 }
 
@@ -710,6 +736,8 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
   a.idx_stride = idx_stride;
+  a.capacity = hits->capacity;
+  a.bulk_ok = ((reinterpret_cast<uintptr_t>(hits->x_at_y0) | reinterpret_cast<uintptr_t>(hits->id)) & 15u) == 0 ? 1u : 0u;
   a.ticket = hits->workspace ? reinterpret_cast<uint32_t*>(hits->workspace) + 4 : nullptr;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 
