@@ -81,11 +81,8 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
 
   Carver cv(smem_raw);
   unsigned char* s_rawstage = cv.take<unsigned char>(a.raw_stage_bytes);
-  float2* g_x0p = cv.take<float2>(ns);            // (x0, pitch) per sector
   uint16_t* g_idtab = cv.take<uint16_t>(idn);     // raw id -> dense sector, 0xFFFF = invalid
-  uint16_t* g_group = cv.take<uint16_t>(ns);
   uint16_t* g_gfirst = cv.take<uint16_t>(ng + 1);
-  uint32_t* s_off = cv.take<uint32_t>(ns + 4);
   uint32_t* s_cnt = cv.take<uint32_t>(ns);
   uint32_t* s_wpos = cv.take<uint32_t>(ns);
   uint32_t* s_gcnt = cv.take<uint32_t>(ng);
@@ -98,10 +95,6 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   __shared__ uint32_t s_warp[32];
 
   // geometry tables: staged once per CTA, reused for every event this CTA takes
-  for (uint32_t i = tid; i < ns; i += nt) {
-    g_x0p[i] = make_float2(a.g.x0[i], a.g.pitch[i]);
-    g_group[i] = (uint16_t)a.g.sector_group[i];
-  }
   for (uint32_t i = tid; i < idn; i += nt) {
     const uint32_t s = a.g.id_to_sector[i];
     g_idtab[i] = s < ns ? (uint16_t)s : (uint16_t)0xFFFFu;
@@ -127,13 +120,12 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
 
     // ---- bank offsets of the event, table reset -------------------------------------------------------
     const uint32_t* bo = a.bank_offsets + (size_t)e * ns;
-    for (uint32_t i = tid; i <= ns; i += nt) s_off[i] = __ldg(bo + i);
+    const uint32_t b0 = __ldg(bo), b1 = __ldg(bo + ns);          // first byte and end of the event's banks
     for (uint32_t i = tid; i < ns; i += nt) { s_cnt[i] = 0; s_wpos[i] = kInvalid; }
     for (uint32_t i = tid; i < ng; i += nt) s_gcnt[i] = 0;
     if (tid == 0) { s_ready = 0; s_gticket = 0; }
     __syncthreads();
 
-    const uint32_t b0 = s_off[0], b1 = s_off[ns];
     const uint32_t b0a = b0 & ~15u;
     const bool range_ok = b1 >= b0;
     const uint32_t span = range_ok ? (((b1 + 15u) & ~15u) - b0a) : 0u;
@@ -153,7 +145,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
     uint32_t local = 0, st = range_ok ? 0u : (uint32_t)UT_STATUS_BAD_BANK_SIZE;
     if (range_ok) {
       for (uint32_t j = tid; j < ns; j += nt) {
-        const uint32_t o0 = s_off[j], o1 = s_off[j + 1];
+        const uint32_t o0 = __ldg(bo + j), o1 = __ldg(bo + j + 1);
         if ((o0 & 3u) || o1 < o0 + 6u || o0 < b0 || o1 > b1) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
         const uint32_t rel = o0 - b0a;
         const uint32_t rid = *reinterpret_cast<const uint32_t*>(rawp + rel);
@@ -165,7 +157,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         if (o1 - o0 != ((6u + 2u * cnt + 3u) & ~3u)) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
         if (atomicCAS(&s_wpos[s], kInvalid, rel + 6u) != kInvalid) { st |= UT_STATUS_DUPLICATE_SECTOR; continue; }
         s_cnt[s] = cnt;
-        if (cnt) atomicAdd(&s_gcnt[g_group[s]], cnt);
+        if (cnt) atomicAdd(&s_gcnt[__ldg(a.g.sector_group + s)], cnt);
         local += cnt;
       }
     }
@@ -233,6 +225,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
       // gather: element i of the fill order -> (sector r, word k), decode x
       float x = 0.f;
       uint32_t rw = 0;                                  // (sector-in-group << 16) | raw word
+      float4 Brow = make_float4(0.f, 0.f, 0.f, 0.f);
       for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
         const uint32_t i = c0 + lane;
         int r = 0;                                      // largest r with e_r <= i
@@ -245,8 +238,8 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
         if (i < n) {
           const uint32_t word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
-          const float2 xp = g_x0p[sa + r];
-          x = decode_x(word, xp.x, xp.y);
+          Brow = __ldg(a.g.sector_rows + 2 * (sa + r) + 1);            // {weight, raw id, x0, pitch}
+          x = decode_x(word, Brow.z, Brow.w);
           rw = ((uint32_t)r << 16) | word;
           if (!in_regs && in_buf) { xbuf[i] = x; wbuf[i] = rw; }
         }
@@ -267,7 +260,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         const uint32_t rank = warp_rank((uint32_t)lane < n ? x : __int_as_float(0x7F800000), lt_mask);
         if ((uint32_t)lane < n) {
           const uint32_t s = sa + (rw >> 16);
-          const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
+          const float4 A = __ldg(a.g.sector_rows + 2 * s), B = Brow;
           const size_t P = P0 + rank;
           a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
           a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
@@ -318,14 +311,15 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
           float xi = 0.f;
           if (valid) {
             word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
-            const float2 xp = g_x0p[sa + r];
-            xi = decode_x(word, xp.x, xp.y);
+            const float4 Bx = __ldg(a.g.sector_rows + 2 * (sa + r) + 1);
+            xi = decode_x(word, Bx.z, Bx.w);
           }
           uint32_t rank = 0, j = 0;
           for (uint32_t r2 = 0; r2 < nsec; ++r2) {      // warp-uniform walk over the fill order
             const uint32_t c2 = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)r2);
             const uint32_t w2 = __shfl_sync(0xFFFFFFFFu, wpos_r, (int)r2);
-            const float2 xp2 = g_x0p[sa + r2];
+            const float4 Bx2 = __ldg(a.g.sector_rows + 2 * (sa + r2) + 1);
+            const float2 xp2 = make_float2(Bx2.z, Bx2.w);
             for (uint32_t k2 = 0; k2 < c2; ++k2, ++j)
               rank += before(decode_x(*reinterpret_cast<const uint16_t*>(rawp + w2 + 2u * k2), xp2.x, xp2.y), j, xi, i);
           }
@@ -361,8 +355,8 @@ static int env_int(const char* name, int dflt) {
 
 static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t idn, uint32_t raw_stage, uint32_t sort_buf, int block) {
   size_t b = align16(raw_stage);
-  b += align16((size_t)ns * 8) + align16((size_t)idn * 2) + align16((size_t)ns * 2) + align16((size_t)(ng + 1) * 2);
-  b += align16((size_t)(ns + 4) * 4) + 2 * align16((size_t)ns * 4) + align16((size_t)ng * 4);
+  b += align16((size_t)idn * 2) + align16((size_t)(ng + 1) * 2);
+  b += 2 * align16((size_t)ns * 4) + align16((size_t)ng * 4);
   b += 2 * align16((size_t)(block / 32) * sort_buf * 4);
   return b;
 }
@@ -401,7 +395,8 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   uint32_t sort_buf = (uint32_t)std::min<unsigned long long>(((2 * avg / ng + 31) / 32) * 32 + 32, 1024);
   sort_buf = std::max(64u, sort_buf);
   sort_buf = ((uint32_t)env_int("UT_DECODE_SORT_BUF", (int)sort_buf) + 31u) & ~31u;
-  int block = env_int("UT_DECODE_BLOCK", 256);
+  // 5-warp CTAs keep a 1000-event batch resident at once (7 per SM); busy events get 8 warps per event
+  int block = env_int("UT_DECODE_BLOCK", avg > 4096 ? 256 : 160);
   block = std::max(64, std::min(512, (block / 32) * 32));
   size_t smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
   const size_t budget = (size_t)max_smem;
