@@ -10,10 +10,11 @@
 
 namespace utc {
 int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
-                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in);
+                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in,
+                      unsigned long long hits_hint);
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream, uint32_t idx_stride);
+                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint);
 
 size_t consolidate_workspace_bytes(uint32_t max_velo);
 int32_t launch_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events, uint32_t n_velo_hint,
@@ -181,7 +182,7 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
     return cudaMemsetAsync(hit_offsets_out, 0, 4, (cudaStream_t)stream) == cudaSuccess ? UT_OK : UT_ERR_CUDA;
   if (!raw_banks) return UT_ERR_NULL;
   return launch_decode(raw_banks, bank_offsets, n_events, geometry, hits_out, hit_offsets_out, (cudaStream_t)stream,
-                       nullptr);
+                       nullptr, 0ull);
 }
 
 int32_t compass_config_default(float p_min_mev, float window_scale, int32_t min_hits, int32_t max_candidates_per_layer,
@@ -217,7 +218,7 @@ int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const ve
       !velo->tx || !velo->ty)
     return UT_ERR_NULL;
   if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
-  return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream, 0u);
+  return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream, 0u, 0ull);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -359,10 +360,13 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
          cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess;
     if (!ok) return UT_ERR_CUDA;
     uint32_t* ho = p->hit_offsets + (size_t)e0 * ng;
-    int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &p->hits, ho, s, k == 0 ? nullptr : ho);
+    // upper bound of this chunk's hits from its raw size alone (sizes the on-chip staging like a whole call)
+    const size_t hdr = 6 * (size_t)ne * ns;
+    const unsigned long long hint = r1 - r0 > hdr ? (r1 - r0 - hdr) / 2 : 1;
+    int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &p->hits, ho, s, k == 0 ? nullptr : ho, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
-    rc = launch_compass(&p->hits, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo);
+    rc = launch_compass(&p->hits, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
     ok = cudaEventRecord(p->ev_done[k], s) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess;

@@ -707,7 +707,7 @@ static const void* const kKernelLarge = reinterpret_cast<const void*>(&compass_k
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream, uint32_t idx_stride) {
+                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint) {
   static int max_smem = 0, n_sm = 0, sm_smem = 0;     // max_smem = largest dynamic size a CTA may ask for
   if (!max_smem) {
     int dev = 0, optin = 0;
@@ -743,7 +743,8 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
 
   const int C = cfg->max_candidates_per_layer;
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
-  const unsigned long long avg = hits->capacity / (unsigned long long)n_events + 1;
+  // hits per event as far as the host can tell without a sync: capacity (or the caller's bound for this call) / events
+  const unsigned long long avg = (hits_hint ? hits_hint : hits->capacity) / (unsigned long long)n_events + 1;
   uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 127) / 128) * 128 + 128, 65536ull);
   hit_stage = (uint32_t)env_int("UT_COMPASS_HIT_STAGE", (int)hit_stage);
   const size_t budget = (size_t)max_smem;

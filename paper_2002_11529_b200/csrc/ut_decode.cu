@@ -362,7 +362,8 @@ static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t idn, uint32_t
 }
 
 int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
-                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in) {
+                      ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in,
+                      unsigned long long hits_hint) {
   static int n_sm = 0, max_smem = 0;     // max_smem = largest dynamic size this kernel may ask for
   if (!n_sm) {
     int dev = 0, optin = 0;
@@ -387,7 +388,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   // staging sizes from the only size the host knows without a sync: capacity / n_events
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
   const uint32_t idn = std::min<uint32_t>(geom->id_table_size, 2048u);
-  const unsigned long long avg = hits->capacity / (unsigned long long)n_events + 1;
+  const unsigned long long avg = (hits_hint ? hits_hint : hits->capacity) / (unsigned long long)n_events + 1;
   const unsigned long long stage_hits = std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
   uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * stage_hits + 32u);
   raw_stage = (uint32_t)env_int("UT_DECODE_RAW_STAGE", (int)raw_stage) & ~15u;
