@@ -35,8 +35,8 @@ UNIT = "events/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
 # profiles/ (config 3; taken with the bench's own L2 flush between steps).  Keyed by workload, then kernel.
 NCU_DRAM_TRAFFIC = {
-    "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 17.70e6,
-                               "source": "profiles/r1c_decode_warp_per_group.md"},
+    "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 18.07e6,
+                               "source": "profiles/r1d_final_round1.md"},
 }
 
 
