@@ -38,6 +38,10 @@ NCU_DRAM_TRAFFIC = {
     "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 18.07e6,
                                "source": "profiles/r1d_final_round1.md"},
 }
+# smsp__inst_executed.sum per launch from the same captures: the kernels are bound by instruction issue, so the
+# line also carries achieved warp-instructions/s against 148 SMs x 4 schedulers x 1 inst/clk x sm_max_mhz
+NCU_WARP_INST = {"config3_throughput1000": {"compass_kernel": 78.95e6, "ut_decode_kernel": 39.77e6}}
+
 
 
 def parse_args():
@@ -442,8 +446,17 @@ def main():
             "traffic": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get(dom) if batch.n_events == cfg.n_events else None,
             "traffic_source": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get("source"), "peak_source": peak_src,
             "algorithmic_bytes_per_launch": kern[dom]["bytes"],
+            "issue": None,
             "end_to_end": {"bytes": abytes["e2e"], "gbs": abytes["e2e"] / ms / 1e6,
                            "frac": abytes["e2e"] / ms / 1e6 / hbm_peak, "frac_of_8TBs": abytes["e2e"] / ms / 1e6 / 8000.0}}
+    winst = NCU_WARP_INST.get(cfg.name, {}) if batch.n_events == cfg.n_events else {}
+    if winst:
+        issue_peak = 148 * 4 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6          # warp-inst / s
+        roof["issue"] = {k: {"warp_inst_per_launch": winst[k], "achieved_ginst_s": winst[k] / kern[k]["ms"] / 1e6,
+                             "peak_ginst_s": issue_peak / 1e9, "frac": winst[k] / (kern[k]["ms"] * 1e-3) / issue_peak}
+                         for k in kern if k in winst}
+        roof["issue"]["note"] = ("context: both kernels are issue / latency bound, not HBM bound; instruction counts from "
+                                 "the committed ncu captures")
     line = {
         "metric": METRIC, "value": events_all * args.steps / (total_ms * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
