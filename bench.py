@@ -318,7 +318,62 @@ def main():
     status = (int(hits.status.item()) | int(tracks.status.item())) & 0xFFFFFFFF
     abytes = algorithmic_bytes(batch, geom_t, n_hits)
 
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    if world > 1:
+        ne = torch.tensor([batch.n_events], dtype=torch.float64, device=dev)
+        dist.all_reduce(ne, op=dist.ReduceOp.SUM)
+        events_all = float(ne.item())
+    else:
+        events_all = float(batch.n_events)
+
+    # (measured before the nvidia-smi clock sampler starts: its polling was seen to slow the host copies)
+    # ---- end to end through the host-buffer C-ABI call (H2D + kernels + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        T = batch.n_velo_total
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        raw_h = pin(np.concatenate([batch.raw, np.zeros(32, np.uint8)]))
+        bo_h, vo_h = pin(batch.bank_offsets.view(np.int32)), pin(batch.velo_offsets.view(np.int32))
+        velo_h = [pin(v) for v in (batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty)]
+        out_h = {"hit_idx": torch.empty(4 * max(T, 1), dtype=torch.int32).pin_memory(),
+                 "n_hits": torch.empty(max(T, 1), dtype=torch.int32).pin_memory(),
+                 "qop": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
+                 "chi2": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
+                 "status": torch.zeros(2, dtype=torch.int32).pin_memory(),
+                 "n_hits_total": torch.zeros(1, dtype=torch.int32).pin_memory()}
+        pipe = B.Pipeline(geom, batch.n_events, int(batch.raw.size) + 32, batch.hit_capacity, max(T, 1))
+        run = lambda: pipe.run_host(raw_h, int(batch.raw.size), bo_h, velo_h, batch.velo_z, vo_h, T, batch.n_events,
+                                    config, out_h)
+        for _ in range(3):
+            run()
+        torch.cuda.synchronize()
+        k_e2e = max(10, min(args.steps, 100))
+        if world > 1:
+            dist.barrier()
+        # per step: flush L2 (outside the timed part), then H2D + kernels + D2H + sync through the C ABI
+        t_steps = []
+        for _ in range(k_e2e):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            run()
+            torch.cuda.synchronize()       # the step's result is on the host before the next one starts
+            t_steps.append(time.perf_counter() - t0)
+        t_e2e = float(sum(t_steps))
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        h2d = int(batch.raw.size) + 4 * (batch.bank_offsets.size + batch.velo_offsets.size) + 16 * T
+        e2e = {"value": events_all * k_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": 28 * T + 12, "steps": k_e2e,
+               "ms_per_step_mean": 1e3 * t_e2e / k_e2e, "ms_per_step_median": 1e3 * statistics.median(t_steps),
+               "ms_per_step_min": 1e3 * min(t_steps),
+               "api": "ut_pipeline_run_host (pinned host buffers in, host track SoA out, sync per step)"}
+        ok = np.array_equal(out_h["n_hits"][:T].numpy(), tracks.n_hits[:T].cpu().numpy())
+        e2e["matches_device_path"] = bool(ok)
+        pipe.destroy()
+
+    sampler = ClockSampler(local_rank) if rank == 0 and not os.environ.get("BENCH_NO_SAMPLER") else None
     for _ in range(max(args.warmup, 3)):
         flush.zero_()
         step()
@@ -351,11 +406,6 @@ def main():
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
-        ne = torch.tensor([batch.n_events], dtype=torch.float64, device=dev)
-        dist.all_reduce(ne, op=dist.ReduceOp.SUM)
-        events_all = float(ne.item())
-    else:
-        events_all = float(batch.n_events)
     clocks = sampler.stop() if sampler else None
 
     # ---- SURVEY.md 8(f) row 1 (not part of the step): compacted track output, timed on its own ----
@@ -372,52 +422,6 @@ def main():
     t_cons = statistics.mean(a_.elapsed_time(b_) for a_, b_ in evc)
     n_compact = int(compact.track_offsets[batch.n_events].item())
     cons_bytes = 28 * batch.n_velo_total + 4 * (batch.n_events + 1) + 32 * n_compact + 4 * (batch.n_events + 1)
-
-    # ---- end to end through the host-buffer C-ABI call (H2D + kernels + D2H inside the timed region) ----
-    e2e = None
-    if not args.no_e2e:
-        T = batch.n_velo_total
-        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        raw_h = pin(np.concatenate([batch.raw, np.zeros(32, np.uint8)]))
-        bo_h, vo_h = pin(batch.bank_offsets.view(np.int32)), pin(batch.velo_offsets.view(np.int32))
-        velo_h = [pin(v) for v in (batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty)]
-        out_h = {"hit_idx": torch.empty(4 * max(T, 1), dtype=torch.int32).pin_memory(),
-                 "n_hits": torch.empty(max(T, 1), dtype=torch.int32).pin_memory(),
-                 "qop": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
-                 "chi2": torch.empty(max(T, 1), dtype=torch.float32).pin_memory(),
-                 "status": torch.zeros(2, dtype=torch.int32).pin_memory(),
-                 "n_hits_total": torch.zeros(1, dtype=torch.int32).pin_memory()}
-        pipe = B.Pipeline(geom, batch.n_events, int(batch.raw.size) + 32, batch.hit_capacity, max(T, 1))
-        run = lambda: pipe.run_host(raw_h, int(batch.raw.size), bo_h, velo_h, batch.velo_z, vo_h, T, batch.n_events,
-                                    config, out_h)
-        for _ in range(3):
-            run()
-        torch.cuda.synchronize()
-        k_e2e = max(10, min(args.steps, 100))
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for _ in range(k_e2e):
-            flush.zero_()
-            run()
-            torch.cuda.synchronize()       # the step's result is on the host before the next one starts
-        t_e2e = time.perf_counter() - t0
-        t_flush0 = time.perf_counter()
-        for _ in range(k_e2e):
-            flush.zero_()
-            torch.cuda.synchronize()
-        t_e2e -= time.perf_counter() - t_flush0          # the flush is not part of the step
-        if world > 1:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
-        h2d = int(batch.raw.size) + 4 * (batch.bank_offsets.size + batch.velo_offsets.size) + 16 * T
-        e2e = {"value": events_all * k_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": 28 * T + 12, "steps": k_e2e,
-               "api": "ut_pipeline_run_host (pinned host buffers in, host track SoA out, sync per step)"}
-        ok = np.array_equal(out_h["n_hits"][:T].numpy(), tracks.n_hits[:T].cpu().numpy())
-        e2e["matches_device_path"] = bool(ok)
-        pipe.destroy()
 
     if rank != 0:
         if world > 1:

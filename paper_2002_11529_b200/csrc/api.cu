@@ -253,7 +253,7 @@ struct ut_pipeline {
   ut_tracks tracks;
   // chunked overlap of copies and kernels: copy-in stream, copy-out stream, per-chunk events
   cudaStream_t s_in, s_out;
-  cudaEvent_t ev_start, ev_out, ev_in[4], ev_done[4];
+  cudaEvent_t ev_start, ev_out, ev_in[4], ev_velo[4], ev_done[4];
 };
 
 int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_raw_bytes, uint64_t max_hits,
@@ -293,6 +293,7 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
             cudaEventCreateWithFlags(&p->ev_out, cudaEventDisableTiming) == cudaSuccess;
   for (int k = 0; k < 4 && ok; ++k)
     ok = cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&p->ev_velo[k], cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&p->ev_done[k], cudaEventDisableTiming) == cudaSuccess;
   if (!ok) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
   *out = p;
@@ -303,7 +304,7 @@ int32_t ut_pipeline_destroy(ut_pipeline* p) {
   if (!p) return UT_ERR_NULL;
   cudaStreamSynchronize(p->s_in);
   cudaStreamSynchronize(p->s_out);
-  for (int k = 0; k < 4; ++k) { cudaEventDestroy(p->ev_in[k]); cudaEventDestroy(p->ev_done[k]); }
+  for (int k = 0; k < 4; ++k) { cudaEventDestroy(p->ev_in[k]); cudaEventDestroy(p->ev_velo[k]); cudaEventDestroy(p->ev_done[k]); }
   cudaEventDestroy(p->ev_start); cudaEventDestroy(p->ev_out);
   cudaStreamDestroy(p->s_in); cudaStreamDestroy(p->s_out);
   cudaFree(p->block);
@@ -324,8 +325,9 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   // The batch is cut into up to 4 chunks of events: chunk k+1 is copied in while chunk k is decoded and
   // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
   // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
-  static const int kChunkEvents = [] { const char* v = getenv("UT_PIPELINE_CHUNK_EVENTS"); return v && *v ? atoi(v) : 500; }();
-  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
+  const char* chunk_env = getenv("UT_PIPELINE_CHUNK_EVENTS");
+  const int kChunkEvents = chunk_env && *chunk_env ? atoi(chunk_env) : 2000;
+  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 2000);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
   bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&
@@ -352,12 +354,14 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     const size_t r0 = k == 0 ? 0 : bo_h[(size_t)e0 * ns], r1 = k == K - 1 ? raw_bytes : bo_h[(size_t)e1 * ns];
     const uint32_t v0 = vo_h[e0], v1 = vo_h[e1];
     if (r1 < r0 || r1 > raw_bytes || v1 < v0 || v1 > n_velo) return UT_ERR_ARG;
+    // the decode only needs the banks and their offsets: the VELO states follow while it runs
     ok = h2d(p->raw + r0, raw_h + r0, r1 - r0) &&
          h2d(p->bank_offsets + (size_t)e0 * ns, bo_h + (size_t)e0 * ns, ((size_t)ne * ns + 1) * 4) &&
+         cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess &&
          h2d(p->velo_offsets + e0, vo_h + e0, ((size_t)ne + 1) * 4) &&
          h2d(p->vx + v0, velo_h->x + v0, (size_t)(v1 - v0) * 4) && h2d(p->vy + v0, velo_h->y + v0, (size_t)(v1 - v0) * 4) &&
          h2d(p->vtx + v0, velo_h->tx + v0, (size_t)(v1 - v0) * 4) && h2d(p->vty + v0, velo_h->ty + v0, (size_t)(v1 - v0) * 4) &&
-         cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess;
+         cudaEventRecord(p->ev_velo[k], p->s_in) == cudaSuccess;
     if (!ok) return UT_ERR_CUDA;
     uint32_t* ho = p->hit_offsets + (size_t)e0 * ng;
     // upper bound of this chunk's hits from its raw size alone (sizes the on-chip staging like a whole call)
@@ -366,6 +370,7 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &p->hits, ho, s, k == 0 ? nullptr : ho, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
+    if (cudaStreamWaitEvent(s, p->ev_velo[k], 0) != cudaSuccess) return UT_ERR_CUDA;
     rc = launch_compass(&p->hits, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
