@@ -350,3 +350,20 @@ def test_consolidate_edge_cases(gpu):
     a = tracks(np.asarray([3000, 3000]), 1.0)
     ref = _consolidate_both(gpu, *a, 2, capacity=4100)        # capacity: offsets stay exact, nothing past the end
     assert ref.status == 8
+
+
+@pytest.mark.parametrize("shuffle_rows", [False, True], ids=["rows_sorted", "rows_shuffled"])
+def test_non_uniform_geometry(shuffle_rows):
+    """SURVEY.md 8(f) row 3 (layout part): decode + Compass parity on the staggered geometry of synth/variant.py
+    (two pitches, narrow inner columns and rows, rows overlapping in y, per-sector z, 4096-entry id table,
+    optionally unsorted rows) -- nothing in the kernels may depend on the regular 16 x 14 layout."""
+    from gpu_helpers import GpuRunner
+    from synth import variant as V
+    geom = V.make_staggered_geometry(shuffle_rows=shuffle_rows)
+    b = V.generate_batch_tables(geom, EventModel(mean_tracks=150.0, efficiency=0.97, noise_mean=1500.0), seed=22,
+                                n_events=60)
+    runner = GpuRunner(geom)
+    for p in (synth.make_compass_params(), synth.make_compass_params(window_scale=2.0, max_candidates_per_layer=4),
+              synth.make_compass_params(min_hits=4, max_candidates_per_layer=32)):
+        h, t = check_batch(runner, geom, b, p)
+        assert (t.n_hits == 4).sum() > 500
