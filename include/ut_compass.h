@@ -150,6 +150,8 @@ typedef struct {
   float z_mag;                 /* kick plane [mm] */
   int32_t min_hits;            /* 3 or 4 */
   int32_t max_candidates_per_layer; /* 1 .. UT_MAX_CANDIDATES, closest-first in |d| */
+  int32_t both_directions;     /* 0: backward seeds (L3, L1) only for tracks where the forward seeds (L0, L2) gave no
+                                  valid tracklet (A11); 1: best of both directions */
 } compass_config;
 
 /* win_half[l] = window_scale * (kappa/p_min_mev) * (layer_z[l] - z_mag) + 0.5,

@@ -54,7 +54,7 @@ class _Config(C.Structure):
     _fields_ = [("win_half", C.c_float * 4), ("y_tol", C.c_float), ("max_slope", C.c_float),
                 ("kink_tol", C.c_float), ("seed_tol", C.c_float), ("w_velo", C.c_float),
                 ("max_chi2_ndf", C.c_float), ("kappa", C.c_float), ("z_mag", C.c_float),
-                ("min_hits", C.c_int32), ("max_candidates_per_layer", C.c_int32)]
+                ("min_hits", C.c_int32), ("max_candidates_per_layer", C.c_int32), ("both_directions", C.c_int32)]
 
 
 def _load():
@@ -91,6 +91,7 @@ def _config_struct(p):
     for n in ("y_tol", "max_slope", "kink_tol", "seed_tol", "w_velo", "max_chi2_ndf", "kappa", "z_mag",
               "min_hits", "max_candidates_per_layer"):
         setattr(c, n, getattr(p, n))
+    c.both_directions = int(getattr(p, "both_directions", 0))
     return c
 
 

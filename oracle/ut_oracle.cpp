@@ -53,6 +53,7 @@ struct oracle_config {              // same fields as synth.CompassParams
   float win_half[4];
   float y_tol, max_slope, kink_tol, seed_tol, w_velo, max_chi2_ndf, kappa, z_mag;
   int32_t min_hits, max_candidates_per_layer;
+  int32_t both_directions;          // 0: backward only if forward found nothing (A11); 1: best of forward and backward
 };
 
 // status bits (data-dependent errors), same meaning as include/ut_compass.h
@@ -274,6 +275,27 @@ struct Best {
   }
 };
 
+// step 7, choice between the directions.  Paper reading A11 (both == 0): forward's result if it has one, else
+// backward's.  SURVEY.md 8(f) row 4 (both == 1): the better of the two in the same total order; a tracklet both
+// directions found (same hits, same fit) counts once.
+static Best combine_directions(const Best& fwd, const Best& bwd, bool both) {
+  if (!both) { Best r = fwd.best.valid ? fwd : bwd; r.n_fits = fwd.n_fits + bwd.n_fits; return r; }
+  Best r;
+  if (!fwd.best.valid) r = bwd;
+  else if (!bwd.best.valid) r = fwd;
+  else {
+    bool same = true;
+    for (int l = 0; l < 4; ++l) same = same && fwd.best.h[l] == bwd.best.h[l];
+    const bool take_bwd = !same && better(bwd.best, fwd.best);
+    r = take_bwd ? bwd : fwd;
+    const Best& other = take_bwd ? fwd : bwd;
+    if (same) r.runner_chi2 = std::min(fwd.runner_chi2, bwd.runner_chi2);
+    else if (other.best.n == r.best.n) r.runner_chi2 = std::min(r.runner_chi2, other.best.chi2);
+  }
+  r.n_fits = fwd.n_fits + bwd.n_fits;
+  return r;
+}
+
 // seed predicates of step 5
 static inline bool seed_ok(const Cand& a, const Cand& b, const oracle_config* c, float* bs_out) {
   const float bs = (b.d - a.d) / (b.z - a.z);
@@ -355,16 +377,12 @@ int32_t oracle_compass(int32_t mode, const oracle_hits* hits, const uint32_t* hi
       int fits = 0;
       if (nonempty >= c->min_hits) {                        // step 4
         if (mode != 2) {
-          Best fwd;
+          Best fwd, bwd;
           search_direction(cand, 0, 2, 1, 3, c, fwd);       // forward seeds (L0, L2)
-          fits = fwd.n_fits;
-          if (fwd.best.valid) result = fwd;
-          else {                                            // A11: backward only if forward found nothing valid
-            Best bwd;
+          if (c->both_directions || !fwd.best.valid)        // A11: backward only if forward found nothing valid
             search_direction(cand, 3, 1, 2, 0, c, bwd);
-            fits += bwd.n_fits;
-            result = bwd;
-          }
+          result = combine_directions(fwd, bwd, c->both_directions != 0);
+          fits = result.n_fits;
         } else {
           // exhaustive: every combination, each tested against the predicates of its direction
           Best dir[2];
@@ -388,8 +406,8 @@ int32_t oracle_compass(int32_t mode, const oracle_hits* hits, const uint32_t* hi
                     dir[dct].offer(fit(hit, c));
                   }
                 }
-          result = dir[0].best.valid ? dir[0] : dir[1];
-          fits = dir[0].n_fits + dir[1].n_fits;
+          result = combine_directions(dir[0], dir[1], c->both_directions != 0);
+          fits = result.n_fits;
         }
       }
       const Tracklet& b = result.best;

@@ -195,12 +195,14 @@ int32_t compass_config_default(float p_min_mev, float window_scale, int32_t min_
   out->y_tol = 0.5f; out->max_slope = (float)(kick + 0.0015); out->kink_tol = 1.5f; out->seed_tol = 0.5f;
   out->w_velo = 100.0f; out->max_chi2_ndf = 9.0f; out->kappa = (float)kappa; out->z_mag = (float)z_mag;
   out->min_hits = min_hits; out->max_candidates_per_layer = max_candidates_per_layer;
+  out->both_directions = 0;
   return UT_OK;
 }
 
 static int32_t check_config(const compass_config* c) {
   if (c->min_hits != 3 && c->min_hits != 4) return UT_ERR_ARG;
   if (c->max_candidates_per_layer < 1 || c->max_candidates_per_layer > UT_MAX_CANDIDATES) return UT_ERR_ARG;
+  if (c->both_directions != 0 && c->both_directions != 1) return UT_ERR_ARG;
   for (int l = 0; l < UT_N_LAYERS; ++l) if (!(c->win_half[l] >= 0.f)) return UT_ERR_ARG;
   return UT_OK;
 }

@@ -441,7 +441,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       }
       if (qn > 0) process_seeds(a, wa, lane, qn, qhead, dir);
       __syncwarp();
-      todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);   // backward only if nothing valid (A11)
+      if (!a.c.both_directions)                   // backward only if nothing valid (A11); else best of both
+        todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);
     }
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {

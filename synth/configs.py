@@ -29,19 +29,21 @@ class CompassParams:
     z_mag: float               # mm
     min_hits: int              # 3 or 4
     max_candidates_per_layer: int
+    both_directions: int = 0   # 0: backward seeds only if forward found nothing (A11); 1: best of both directions
 
 
 def make_compass_params(p_min_gev: float = 2.0, window_scale: float = 1.0, min_hits: int = 3,
                         max_candidates_per_layer: int = 16, x_tol0: float = 0.5, y_tol: float = 0.5,
                         slope_tol: float = 0.0015, kink_tol: float = 1.5, seed_tol: float = 0.5,
-                        w_velo: float = 100.0, max_chi2_ndf: float = 9.0) -> CompassParams:
+                        w_velo: float = 100.0, max_chi2_ndf: float = 9.0, both_directions: int = 0) -> CompassParams:
     f = lambda v: float(np.float32(v))
     kick = window_scale * KAPPA / (p_min_gev * 1e3)          # max |slope change| at p_min, scaled
     win = tuple(f(kick * (z - Z_MAG) + x_tol0) for z in G.LAYER_Z)
     return CompassParams(
         win_half=win, y_tol=f(y_tol), max_slope=f(kick + slope_tol), kink_tol=f(kink_tol),
         seed_tol=f(seed_tol), w_velo=f(w_velo), max_chi2_ndf=f(max_chi2_ndf), kappa=f(KAPPA),
-        z_mag=f(Z_MAG), min_hits=int(min_hits), max_candidates_per_layer=int(max_candidates_per_layer))
+        z_mag=f(Z_MAG), min_hits=int(min_hits), max_candidates_per_layer=int(max_candidates_per_layer),
+        both_directions=int(both_directions))
 
 
 @dataclass(frozen=True)

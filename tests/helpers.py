@@ -86,5 +86,8 @@ def brute_force64(hits, lo, hi, geom, p, vx, vy, vtx, vty, vz=770.0):
             if best is None or key < best[0]:
                 best = (key, tuple(c[0] if c is not None else -1 for c in combo), n, chi2, sol[1] / p.kappa)
         res[direction] = best
-    best = res[0] if res[0] is not None else res[1]
+    if getattr(p, "both_directions", 0) and res[0] is not None and res[1] is not None:
+        best = min(res[0], res[1], key=lambda r: r[0])        # 8(f) row 4: best of both directions, same order
+    else:
+        best = res[0] if res[0] is not None else res[1]        # A11
     return None if best is None else best[1:]

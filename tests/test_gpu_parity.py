@@ -367,3 +367,20 @@ def test_non_uniform_geometry(shuffle_rows):
               synth.make_compass_params(min_hits=4, max_candidates_per_layer=32)):
         h, t = check_batch(runner, geom, b, p)
         assert (t.n_hits == 4).sum() > 500
+
+
+def test_both_directions_mode(gpu, wl):
+    """SURVEY.md 8(f) row 4 (selection part): best of forward and backward seeds, configs[1] and a busy subset."""
+    import dataclasses
+    for c, n in ((2, None), (4, 30)):
+        geom, b, p = wl(c, n)
+        _, t = check_batch(gpu, geom, b, dataclasses.replace(p, both_directions=1))
+        _, t0 = oracle_run(b, geom, p)
+        assert (t.hit_idx != t0.hit_idx).any()
+    B = gpu.B
+    with pytest.raises(B.UTError):
+        geom, b, p = wl(1)
+        hits, _ = gpu.run(b, p)
+        bad = B.make_config(p); bad.both_directions = 2
+        B.compass_track(hits, hits.hit_offsets, B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z),
+                        B.to_device_u32(b.velo_offsets), 1, bad, B.Tracks(20))

@@ -385,3 +385,49 @@ def test_golden_config1(wl):
             assert int(t.qop[k:k + 1].view(np.uint32)[0]) == int(f[7], 16)
             assert int(t.chi2[k:k + 1].view(np.uint32)[0]) == int(f[8], 16)
     assert nH == h.n_hits and nT == 20
+
+
+# ---- best of both seed directions ------------------------------------------------
+def test_both_directions_mode(geom):
+    """both_directions = 1: (a) equals the float64 brute force taking the better of the two directions,
+    (b) is never worse than the A11 result in (n, chi2), identical wherever forward alone decided and backward
+    has nothing better, (c) seeded search == exhaustive search (BF-2) in this mode too."""
+    import dataclasses
+    m = EventModel(fixed_tracks=8, efficiency=0.85, noise_mean=60.0)
+    b = generate_batch(geom, m, seed=41, n_events=15)
+    p0 = synth.make_compass_params(max_candidates_per_layer=64)
+    p1 = dataclasses.replace(p0, both_directions=1)
+    h, t0 = run(b, geom, p0, 0)
+    _, t1 = run(b, geom, p1, 0)
+    _, t1x = run(b, geom, p1, 2)
+    assert np.array_equal(t1.hit_idx, t1x.hit_idx) and np.array_equal(t1.chi2.view(np.uint32), t1x.chi2.view(np.uint32))
+    assert np.array_equal(t0.n_hits > 0, t1.n_hits > 0)
+    assert np.all(t1.n_hits >= t0.n_hits)
+    same_n = t1.n_hits == t0.n_hits
+    assert np.all(t1.chi2[same_n] <= t0.chi2[same_n])
+    n_cmp = 0
+    for e in range(b.n_events):
+        lo, hi = int(h.hit_offsets[e * 64]), int(h.hit_offsets[(e + 1) * 64])
+        for k in range(int(b.velo_offsets[e]), int(b.velo_offsets[e + 1])):
+            ref = brute_force64(h, lo, hi, geom, p1, float(b.velo_x[k]), float(b.velo_y[k]), float(b.velo_tx[k]),
+                                float(b.velo_ty[k]))
+            if ref is None:
+                assert t1.n_hits[k] == 0
+                continue
+            if np.isfinite(t1.runner_chi2[k]) and abs(t1.runner_chi2[k] - t1.chi2[k]) <= 1e-4 * t1.chi2[k]:
+                continue
+            assert tuple(t1.hit_idx[:, k]) == ref[0] and t1.n_hits[k] == ref[1]
+            n_cmp += 1
+    assert n_cmp >= 60
+
+
+def test_both_directions_changes_few_tracks(wl):
+    """On min-bias-like events the mode matters for a fraction of a per cent of the tracks, never lowers n_hits and
+    never finds fewer tracklets."""
+    import dataclasses
+    geom, b, p0 = wl(2, 30)
+    _, t0 = run(b, geom, p0, 0)
+    _, t1 = run(b, geom, dataclasses.replace(p0, both_directions=1), 0)
+    diff = (t1.hit_idx != t0.hit_idx).any(axis=0)
+    assert 0 < diff.sum() < 0.01 * diff.size
+    assert np.array_equal(t0.n_hits > 0, t1.n_hits > 0) and np.all(t1.n_hits >= t0.n_hits)
