@@ -557,7 +557,8 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     if (tid == 0) s_ticket = 0;
     const uint32_t n = h1 - h0;
-    const int flag = __syncthreads_or((bad ? 1 : 0) | ((!bad && n > 65535u) ? 2 : 0));
+    // (__syncthreads_or returns a truth value, not the OR of the arguments; n is the same in every thread)
+    const int flag = __syncthreads_or(bad ? 1 : 0) ? 1 : (n > 65535u ? 2 : 0);
     if (flag) {                                    // uniform: report and emit "no tracklet" for every track
       if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
                                            (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u));

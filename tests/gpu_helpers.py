@@ -55,10 +55,10 @@ def compare_decode(ref, got, off_got, status_got):
     assert np.array_equal(ref.id[:n], got["id"][:n])
 
 
-def compare_tracks(ref, got, rel=1e-5):
+def compare_tracks(ref, got, rel=1e-5, status=0):
     """ref: oracle.Tracks.  Hit indices exact except flagged near-ties (<= 1e-5 relative between the two
     best chi2 of the same n); q/p and chi2 within 1e-5 relative.  Returns the number of flagged tracks."""
-    assert got["status"] == 0
+    assert got["status"] == status
     near_tie = np.isfinite(ref.runner_chi2) & (np.abs(ref.runner_chi2 - ref.chi2) <= rel * np.abs(ref.chi2))
     same_idx = np.all(ref.hit_idx == got["hit_idx"], axis=0)
     bad = ~same_idx & ~near_tie

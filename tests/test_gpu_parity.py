@@ -384,3 +384,71 @@ def test_both_directions_mode(gpu, wl):
         bad = B.make_config(p); bad.both_directions = 2
         B.compass_track(hits, hits.hit_offsets, B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z),
                         B.to_device_u32(b.velo_offsets), 1, bad, B.Tracks(20))
+
+
+def test_compass_status_paths(gpu, geom):
+    """Data-dependent errors of compass_track (include/ut_compass.h): an event of more than 65535 hits (A19), hit
+    offsets that are not monotone, VELO offsets that run backwards.  The bad event gets "no tracklet" (or is
+    skipped), the status word says why, and every other event still equals the oracle."""
+    from synth.events import generate_event
+    B, torch = gpu.B, gpu.torch
+    small = EventModel(fixed_tracks=30, efficiency=0.97, noise_mean=300.0)
+    huge = EventModel(fixed_tracks=30, efficiency=0.97, noise_mean=80000.0)
+    b = assemble_batch(geom, [generate_event(geom, small, 5, 0), generate_event(geom, huge, 5, 1),
+                              generate_event(geom, small, 5, 2)])
+    p = synth.make_compass_params()
+    h_ref, t_ref = oracle_run(b, geom, p)
+    assert h_ref.hit_offsets[128] - h_ref.hit_offsets[64] > 65535
+    hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)      # the decode has no such limit
+    got, off, st = gpu.hits_numpy(hits, b.n_events)
+    from gpu_helpers import compare_decode
+    compare_decode(h_ref, got, off, st)
+    trk = gpu.compass(hits, b, p)
+    assert trk["status"] == B.UT_STATUS_EVENT_TOO_LARGE
+    ev = np.repeat(np.arange(3), np.diff(b.velo_offsets.astype(np.int64)))
+    ok = ev != 1
+    assert np.all(trk["n_hits"][~ok] == 0) and np.all(trk["hit_idx"][:, ~ok] == -1) and np.all(trk["chi2"][~ok] == 0)
+    assert np.array_equal(trk["hit_idx"][:, ok], t_ref.hit_idx[:, ok]) and (t_ref.n_hits[ok] > 0).sum() > 20
+    assert np.array_equal(trk["chi2"][ok].view(np.uint32), t_ref.chi2[ok].view(np.uint32))
+
+    # offsets of event 1 not monotone -> BAD_OFFSETS, that event empty, the others untouched
+    b3 = assemble_batch(geom, [generate_event(geom, small, 6, k) for k in range(3)])
+    h3, t3 = oracle_run(b3, geom, p)
+    hits = gpu.decode(b3.raw, b3.bank_offsets, 3, b3.hit_capacity)
+    o = hits.hit_offsets.clone()
+    hits.hit_offsets[64 + 10], hits.hit_offsets[64 + 11] = o[64 + 11] + 5, o[64 + 10]
+    trk = gpu.compass(hits, b3, p)
+    ev = np.repeat(np.arange(3), np.diff(b3.velo_offsets.astype(np.int64)))
+    assert trk["status"] == B.UT_STATUS_BAD_OFFSETS
+    assert np.all(trk["n_hits"][ev == 1] == 0)
+    assert np.array_equal(trk["hit_idx"][:, ev != 1], t3.hit_idx[:, ev != 1])
+
+    # VELO offsets running backwards for event 1: nothing can be written for it, status says so
+    hits.hit_offsets.copy_(o)
+    vo = b3.velo_offsets.copy()
+    vo[1], vo[2] = vo[2], vo[1]
+    velo = B.VeloStates(b3.velo_x, b3.velo_y, b3.velo_tx, b3.velo_ty, b3.velo_z)
+    tr = B.Tracks(b3.n_velo_total)
+    tr.n_hits.fill_(-9)
+    B.compass_track(hits, hits.hit_offsets, velo, B.to_device_u32(vo), 3, B.make_config(p), tr)
+    torch.cuda.synchronize()
+    assert int(tr.status.item()) & B.UT_STATUS_BAD_OFFSETS
+
+
+def test_compass_bad_hit_id(gpu, geom):
+    """A hit whose id names no sector of the geometry is ignored and reported (UT_STATUS_BAD_HIT_ID); events
+    without such a hit are untouched."""
+    from synth.events import generate_event
+    B = gpu.B
+    m = EventModel(fixed_tracks=30, efficiency=0.97, noise_mean=300.0)
+    b = assemble_batch(geom, [generate_event(geom, m, 8, k) for k in range(3)])
+    p = synth.make_compass_params()
+    _, t_ref = oracle_run(b, geom, p)
+    hits = gpu.decode(b.raw, b.bank_offsets, 3, b.hit_capacity)
+    k = int(hits.hit_offsets[64 + 3].item())                   # a hit of event 1
+    hits.id[k] = (1023 << 9) | 5                                # raw sector id 1023 is not in the table
+    trk = gpu.compass(hits, b, p)
+    assert trk["status"] == B.UT_STATUS_BAD_HIT_ID
+    ev = np.repeat(np.arange(3), np.diff(b.velo_offsets.astype(np.int64)))
+    assert np.array_equal(trk["hit_idx"][:, ev != 1], t_ref.hit_idx[:, ev != 1])
+    assert not (trk["hit_idx"][:, ev == 1] == k).any()
