@@ -452,3 +452,40 @@ def test_compass_bad_hit_id(gpu, geom):
     ev = np.repeat(np.arange(3), np.diff(b.velo_offsets.astype(np.int64)))
     assert np.array_equal(trk["hit_idx"][:, ev != 1], t_ref.hit_idx[:, ev != 1])
     assert not (trk["hit_idx"][:, ev == 1] == k).any()
+
+
+def test_consolidate_workspace_too_small(gpu):
+    """n_velo_total above what the workspace was sized for: reported, nothing written, the next call still works."""
+    B, torch = gpu.B, gpu.torch
+    T = 5000
+    tr = B.Tracks(T)
+    tr.n_hits.fill_(3); tr.hit_idx.fill_(7); tr.qop.fill_(1.0); tr.chi2.fill_(2.0)
+    vo = B.to_device_u32(np.array([0, 2000, T], np.uint32))
+    out = B.CompactTracks(T, 1000, 2)                  # workspace for 1000 tracks only
+    out.velo_index.fill_(-5)
+    B.compass_consolidate(tr, vo, 2, out)
+    torch.cuda.synchronize()
+    assert int(out.status.item()) == B.UT_STATUS_BAD_OFFSETS and int(out.velo_index[0].item()) == -5
+    out2 = B.CompactTracks(T, T, 2)
+    B.compass_consolidate(tr, vo, 2, out2)
+    torch.cuda.synchronize()
+    assert out2.numpy(2)["track_offsets"].tolist() == [0, 2000, T] and int(out2.status.item()) == 0
+
+
+def test_host_pipeline_empty_and_invalid(gpu, wl):
+    import torch
+    B = gpu.B
+    geom, b, p = wl(1)
+    pipe = B.Pipeline(gpu.geom, 4, 4096, 1024, 64)
+    z = lambda dt, n=1: torch.zeros(n, dtype=dt).pin_memory()
+    out_h = {"hit_idx": z(torch.int32, 4), "n_hits": z(torch.int32), "qop": z(torch.float32), "chi2": z(torch.float32),
+             "status": torch.full((2,), -1, dtype=torch.int32).pin_memory(),
+             "n_hits_total": torch.full((1,), -1, dtype=torch.int32).pin_memory()}
+    velo_h = [z(torch.float32) for _ in range(4)]
+    pipe.run_host(z(torch.uint8, 64), 0, z(torch.int32), velo_h, 770.0, z(torch.int32), 0, 0, B.make_config(p), out_h)
+    torch.cuda.synchronize()
+    assert out_h["status"].tolist() == [0, 0] and int(out_h["n_hits_total"][0]) == 0
+    with pytest.raises(B.UTError):                      # more events than the arena was created for
+        pipe.run_host(z(torch.uint8, 64), 0, z(torch.int32, 5 * 896 + 1), velo_h, 770.0, z(torch.int32, 6), 0, 5,
+                      B.make_config(p), out_h)
+    pipe.destroy()
