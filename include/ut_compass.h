@@ -77,7 +77,6 @@ typedef struct {
   float layer_z[UT_N_LAYERS], layer_dxdy[UT_N_LAYERS];           /* HOST values inside the struct */
   /* filled by ut_geometry_upload (device, library-owned until ut_geometry_free) */
   const uint32_t* group_first_sector; /* [n_groups + 1] */
-  const float* group_inv_span;        /* [n_groups] 1 / (group_xmax - group_xmin) */
   const void* sector_rows;            /* [n_sectors] 32-byte rows {z, y_begin, y_end, dxdy | weight, raw id, x0,
                                          pitch}: the table row a decoded hit copies, packed for 128-bit loads */
   uint32_t flags;                     /* UT_GEOM_* properties found by ut_geometry_upload */
@@ -226,7 +225,9 @@ int32_t ut_pipeline_device_hits(ut_pipeline* p, ut_hits* hits_out, const uint32_
 /* Launch statistics of the most recent call on this thread (host side, no sync). */
 typedef struct {
   int32_t kernels_launched;     /* kernels enqueued by the last hot-path call */
-  int32_t decode_grid, decode_block, decode_smem_bytes, decode_buckets_per_group, decode_hit_stage;
+  int32_t decode_grid, decode_block, decode_smem_bytes;
+  int32_t decode_raw_stage_bytes;   /* shared-memory staging of one event's raw banks (larger events read global memory) */
+  int32_t decode_sort_buf;          /* per-warp sort buffer, in hits (larger groups rank by recomputation) */
   int32_t compass_grid, compass_block, compass_smem_bytes, compass_hit_stage;
 } ut_launch_info;
 void ut_last_launch_info(ut_launch_info* out);

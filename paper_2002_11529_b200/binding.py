@@ -34,7 +34,7 @@ class ut_geometry(C.Structure):
                 ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
                 ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
                 ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
-                ("group_first_sector", C.c_void_p), ("group_inv_span", C.c_void_p), ("sector_rows", C.c_void_p),
+                ("group_first_sector", C.c_void_p), ("sector_rows", C.c_void_p),
                 ("flags", C.c_uint32),
                 ("owner", C.c_void_p)]
 
@@ -69,8 +69,8 @@ class ut_compact_tracks(C.Structure):
 
 class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
-                ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_buckets_per_group",
-                 "decode_hit_stage", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage")]
+                ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_raw_stage_bytes",
+                 "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage")]
 
 
 EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_geometry_upload", "ut_geometry_free",

@@ -61,7 +61,6 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   if (ns > UT_MAX_SECTORS || ng > UT_MAX_GROUPS || h->id_table_size == 0) return UT_ERR_LIMIT;
   // ---- container contract (include/ut_compass.h) ----
   std::vector<uint32_t> first(ng + 1, 0);
-  std::vector<float> inv(ng);
   bool rows_sorted = true;
   {
     uint32_t prev = 0;
@@ -84,7 +83,6 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
       }
       const float span = h->group_xmax[g] - h->group_xmin[g];
       if (!(span > 0.f)) return UT_ERR_GEOMETRY;
-      inv[g] = 1.0f / span;
       if (g % gpl != 0 && (h->group_xmin[g] < h->group_xmin[g - 1] || h->group_xmax[g] < h->group_xmax[g - 1]))
         return UT_ERR_GEOMETRY;                                           // bounds monotone inside a layer
     }
@@ -93,7 +91,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
   const size_t sz_id = up(h->id_table_size * 4), sz_s = up(ns * 4), sz_g = up((ng + 1) * 4);
   const size_t sz_rows = up((size_t)ns * 32);
-  const size_t total = sz_id + 9 * sz_s + 4 * sz_g + sz_rows;
+  const size_t total = sz_id + 9 * sz_s + 3 * sz_g + sz_rows;
   unsigned char* dev = nullptr;
   if (cudaMalloc(&dev, total) != cudaSuccess) return UT_ERR_CUDA;
   std::vector<unsigned char> host(total, 0);
@@ -119,7 +117,6 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   out->group_xmin = (const float*)put(h->group_xmin, ng * 4, sz_g);
   out->group_xmax = (const float*)put(h->group_xmax, ng * 4, sz_g);
   out->group_first_sector = (const uint32_t*)put(first.data(), (ng + 1) * 4, sz_g);
-  out->group_inv_span = (const float*)put(inv.data(), ng * 4, sz_g);
   {
     std::vector<float> rows((size_t)ns * 8);
     for (uint32_t s = 0; s < ns; ++s) {
@@ -167,7 +164,7 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
   launch_info().kernels_launched = 0;
   if (!bank_offsets || !geometry || !hits_out || !hit_offsets_out) return UT_ERR_NULL;
   if (n_events < 0) return UT_ERR_ARG;
-  if (!geometry->group_first_sector || !geometry->group_inv_span || !geometry->sector_rows)
+  if (!geometry->group_first_sector || !geometry->sector_rows)
     return UT_ERR_GEOMETRY;                                                                  // not uploaded
   if (geometry->n_sectors > UT_MAX_SECTORS || geometry->n_groups > UT_MAX_GROUPS) return UT_ERR_LIMIT;
   if (!hits_out->x_at_y0 || !hits_out->z_at_y0 || !hits_out->y_begin || !hits_out->y_end || !hits_out->dxdy ||

@@ -15,7 +15,7 @@ struct GeomDev {
   uint32_t n_sectors, n_groups, id_table_size, groups_per_layer;
   const uint32_t *id_to_sector, *sector_raw_id, *sector_group, *group_first_sector;
   const float *x0, *pitch, *dxdy, *z, *y_begin, *y_end, *weight;
-  const float *group_xmin, *group_xmax, *group_inv_span;
+  const float *group_xmin, *group_xmax;
   const float4* sector_rows;
   float layer_z[4], layer_dxdy[4];
 };
@@ -28,7 +28,6 @@ inline GeomDev make_geom_dev(const ut_geometry* g) {
   d.group_first_sector = g->group_first_sector;
   d.x0 = g->x0; d.pitch = g->pitch; d.dxdy = g->dxdy; d.z = g->z; d.y_begin = g->y_begin; d.y_end = g->y_end;
   d.weight = g->weight; d.group_xmin = g->group_xmin; d.group_xmax = g->group_xmax;
-  d.group_inv_span = g->group_inv_span;
   d.sector_rows = reinterpret_cast<const float4*>(g->sector_rows);
   for (int l = 0; l < 4; ++l) { d.layer_z[l] = g->layer_z[l]; d.layer_dxdy[l] = g->layer_dxdy[l]; }
   return d;

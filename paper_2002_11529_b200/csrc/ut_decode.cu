@@ -421,7 +421,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   UTC_CUDA(cudaGetLastError());
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.decode_grid = grid; li.decode_block = block; li.decode_smem_bytes = (int)smem;
-  li.decode_buckets_per_group = 0; li.decode_hit_stage = (int)sort_buf;
+  li.decode_raw_stage_bytes = (int)raw_stage; li.decode_sort_buf = (int)sort_buf;
   return UT_OK;
 }
 
