@@ -177,6 +177,25 @@ struct SmemView {
 // ---- phase 1: candidate list of one (track, layer) -------------------------------------
 // Group and sector row are found from a linear guess corrected against the tables (exact lower bound of
 // the same predicates the oracle's search uses; O(1) on a regular layout, any sorted layout works).
+#ifndef UT_COMPASS_YR_SMEM
+#define UT_COMPASS_YR_SMEM 0           // 1: the 7 KB table of toleranced y ranges lives in shared memory
+#endif
+// y range of a sector widened by y_tol (same two roundings wherever it is evaluated)
+__device__ __forceinline__ float yr_hi(const CompassArgs& a, const SmemView& S, int s) {
+#if UT_COMPASS_YR_SMEM
+  return S.yr[s].y;
+#else
+  return __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol);
+#endif
+}
+__device__ __forceinline__ float2 yr_of(const CompassArgs& a, const SmemView& S, int s) {
+#if UT_COMPASS_YR_SMEM
+  return S.yr[s];
+#else
+  return make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
+#endif
+}
+
 template <bool BUCKETED>
 __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
                                               int l, float x_e, float y_e, uint32_t h0) {
@@ -208,11 +227,11 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
       if (a.rows_sorted) {                          // first sector row with y_e <= y_end + y_tol
         const int guess = (int)ceilf((y_e - grp.w) * __uint_as_float(gi.x));
         s = sa + max(0, min(guess, sb - sa - 1));
-        while (s > sa && y_e <= S.yr[s - 1].y) --s;
-        while (s < sb && !(y_e <= S.yr[s].y)) ++s;
+        while (s > sa && y_e <= yr_hi(a, S, s - 1)) --s;
+        while (s < sb && !(y_e <= yr_hi(a, S, s))) ++s;
       }
       for (; s < sb; ++s) {
-        const float2 yr = S.yr[s];
+        const float2 yr = yr_of(a, S, s);
         if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
         if (!(y_e <= yr.y)) continue;
         const uint32_t p1 = S.off[s + 1];
@@ -489,7 +508,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   Carver cvr(smem_raw);
   float4* s_gA = cvr.take<float4>(ng);
   uint2* s_gB = cvr.take<uint2>(ng);
-  float2* s_yr = cvr.take<float2>(ns);
+  float2* s_yr = cvr.take<float2>(UT_COMPASS_YR_SMEM ? ns : 0);
   uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);
   uint16_t* s_off = cvr.take<uint16_t>(ns + 1);
   float* s_hx = cvr.take<float>(a.hit_stage);
@@ -507,7 +526,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t lt_mask = (1u << lane) - 1u;
 
   // ---- geometry tables, once per CTA ---------------------------------------------------------------------
-  for (uint32_t s = tid; s < ns; s += nt)
+  for (uint32_t s = tid; UT_COMPASS_YR_SMEM && s < ns; s += nt)
     s_yr[s] = make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
   for (uint32_t g = tid; g < ng; g += nt) {
     const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
@@ -694,7 +713,7 @@ static int env_int(const char* name, int dflt) {
 }
 
 static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block) {
-  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + align16((size_t)ns * 8);
+  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + (UT_COMPASS_YR_SMEM ? align16((size_t)ns * 8) : 0);
   b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
   b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
   b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)),
@@ -755,10 +774,10 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   int block = env_int("UT_COMPASS_BLOCK", 0);
   if (block <= 0) {
     int best_warps = -1;
-    for (int b = 192; b <= 768; b += 64) {
+    for (int b = 192; b <= 768; b += 32) {
       const size_t sm = compass_smem_bytes(ns, ng, hit_stage, C, b) + 1024;
       if (sm > budget) continue;
-      const int regs_warps = b <= 256 ? 24 : 21;
+      const int regs_warps = b <= 256 ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
       const int warps = ctas * (b / 32);
       if (warps > best_warps) { best_warps = warps; block = b; }
