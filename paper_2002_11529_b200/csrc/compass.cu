@@ -766,7 +766,9 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
   // hits per event as far as the host can tell without a sync: capacity (or the caller's bound for this call) / events
   const unsigned long long avg = (hits_hint ? hits_hint : hits->capacity) / (unsigned long long)n_events + 1;
-  uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((avg + 127) / 128) * 128 + 128, 65536ull);
+  // the capacity bound counts the pad half-word of every odd bank as a hit: about n_sectors / 2 per event
+  const unsigned long long est = avg > ns ? avg - ns / 2 : avg;
+  uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((est + est / 8 + 127) / 128) * 128 + 128, 65536ull);
   hit_stage = (uint32_t)env_int("UT_COMPASS_HIT_STAGE", (int)hit_stage);
   const size_t budget = (size_t)max_smem;
   // Block size: the one that keeps the most warps resident per SM (shared memory is the limit; about 24
