@@ -35,12 +35,12 @@ UNIT = "events/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
 # profiles/ (config 3; taken with the bench's own L2 flush between steps).  Keyed by workload, then kernel.
 NCU_DRAM_TRAFFIC = {
-    "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 18.07e6,
+    "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 18.20e6,
                                "source": "profiles/r1d_final_round1.md"},
 }
 # smsp__inst_executed.sum per launch from the same captures: the kernels are bound by instruction issue, so the
 # line also carries achieved warp-instructions/s against 148 SMs x 4 schedulers x 1 inst/clk x sm_max_mhz
-NCU_WARP_INST = {"config3_throughput1000": {"compass_kernel": 78.95e6, "ut_decode_kernel": 39.77e6}}
+NCU_WARP_INST = {"config3_throughput1000": {"compass_kernel": 81.16e6, "ut_decode_kernel": 40.10e6}}
 
 
 
