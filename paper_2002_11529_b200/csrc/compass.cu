@@ -3,28 +3,30 @@
 // The paper runs two kernels: "search UT windows" (2-D: 4 panels x tracks) writes
 // (first hit, size) ranges to global memory, then "tracklet finding" (thread per track)
 // reads them back through a shared-memory cache.  That shape leaves a B200 warp at
-// 7 of 32 lanes (profiles/r1a_first_path.md).  Here one CTA takes one event and keeps it on chip:
+// 7 of 32 lanes (profiles/r1a_first_path.md).  Here one CTA takes one event (atomic ticket) and keeps it on chip:
 //
-//   stage    the event's hits are re-bucketed PER SECTOR into shared memory (x and the hit index only;
-//            count -> block scan -> scatter).  A sector's y range, stereo slope, z and weight are rows of
-//            the geometry table, so the y test of the window search becomes a per-sector test: the scan
-//            touches the ~2 hits of the one sector row the track crosses instead of the ~20 hits of all
-//            14 rows of the column group.
+//   stage    the event's id and x ranges arrive by two TMA bulk copies into scratch that aliases the warp areas;
+//            a warp per sector group re-buckets them PER SECTOR into shared memory (x and the hit index only;
+//            one pass: match.any ranks, per-sector counts, warp scan).  A sector's y range, stereo slope, z and
+//            weight are rows of the geometry table, so the y test of the window search becomes a per-sector
+//            test: the scan touches the hits of the one sector row the track crosses instead of all 14 rows.
 //   phase 1  lane = (track, layer), 8 tracks per warp (the paper's 2-D window kernel shape):
-//            straight-line extrapolation, column groups by binary search on the group x bounds, sector
-//            row by binary search on the y bounds, |d| <= win test on the sector's hits; accepted hits go
-//            to the (track, layer) candidate list in shared memory, kept sorted by hit index and capped
-//            to the `max_candidates_per_layer` closest in |d|.
-//   phase 2  the nested loops of the tracklet search are flattened over the 32 lanes of the warp:
-//            (a) all seed pairs (a, b) of the 8 tracks, one pair per lane: slope + kink cuts; survivors are
-//                compacted (ballot) into a per-warp seed queue;
-//            (b) whenever 32 seeds are queued, one seed per lane: compatible hits in the other two layers
-//                as 32-bit masks, giving the number of 3/4-hit combinations of the seed;
-//            (c) all combinations of those 32 seeds, one fit per lane (linear chi2 fit with the VELO
-//                pseudo-point), packed (n, chi2, positions) key, atomicMin into the track's best key.
-//            Forward seeds first, backward only for tracks where forward found nothing valid (A11).
+//            straight-line extrapolation, column groups and sector row from a linear guess corrected against
+//            the tables (y ranges from L1), lower-bound search in busy sectors, |d| <= win test with early exit;
+//            accepted hits go to the (track, layer) candidate list in shared memory, kept sorted by hit index
+//            and capped to the `max_candidates_per_layer` closest in |d|.
+//   phase 2  the nested loops of the tracklet search are spread over the 32 lanes of the warp:
+//            (a) seed rows (track, hit a) of the 8 tracks, one row per lane walking the partner hits b: slope +
+//                kink cuts; survivors are compacted (ballot) into a per-warp seed queue;
+//            (b) the queued seeds, 4 lanes per seed: compatible hits in the other two layers as 32-bit masks,
+//                giving the number of 3/4-hit combinations of the seed;
+//            (c) all combinations of those seeds, one fit per lane (linear chi2 fit with the VELO pseudo-point),
+//                packed (n, chi2, positions) key, atomicMin into the track's best key.
+//            Forward seeds first, backward only for tracks where forward found nothing valid (A11), or both
+//            directions for every track (compass_config.both_directions).
 //   Candidate lists, queues and best keys never leave the SM; the phases of a warp are separated by
-//   __syncwarp only, and the warps of a CTA pull 8-track batches from a shared-memory ticket.
+//   __syncwarp only, and the 7 warps of a CTA pull 8-track batches from a shared-memory ticket (an event of up
+//   to 168 tracks is three rounds; the step at 1000 events is set by this latency, profiles/r1d_final_round1.md).
 //
 // Events that do not fit the staging buffer take the same phases with a group-level binary search on the
 // global x-sorted arrays (the plain definition of the window, per-hit y test).
