@@ -61,6 +61,7 @@ struct CompassArgs {
   float *out_qop, *out_chi2;
   uint32_t* status;
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
+  uint32_t trk_stage;                  // tracks of an event that can be ordered by radius (0: never)
   unsigned long long capacity;         // elements of the hit arrays (bulk copies never read past it)
   uint32_t bulk_ok;                    // hit arrays are 16-byte aligned: the event's x and id ranges come by TMA
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
@@ -379,7 +380,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 
 template <bool BUCKETED>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
-                                           uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T) {
+                                           uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T, const uint16_t* perm) {
   const int lane = threadIdx.x & 31;
   const int l = lane & 3;                         // layer of this lane in phase 1 and in the output
   const int j = lane & 7;                         // track-in-batch this lane does the bookkeeping for (lanes 0..7)
@@ -388,10 +389,10 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     int batch = 0;
     if (lane == 0) batch = atomicAdd(s_ticket, 1);
     batch = __shfl_sync(0xFFFFFFFFu, batch, 0);
-    const uint32_t tb = t0 + (uint32_t)batch * kTPW;
-    if (tb >= t1) break;
-    const uint32_t tg = tb + (uint32_t)(lane >> 2);
-    const bool active = tg < t1;
+    const uint32_t ti = (uint32_t)batch * kTPW + (uint32_t)(lane >> 2);      // track of the event, in batch order
+    if ((uint32_t)batch * kTPW >= t1 - t0) break;
+    const bool active = ti < t1 - t0;
+    const uint32_t tg = t0 + (active && perm ? (uint32_t)perm[ti] : ti);
     // ---------------- phase 1: window search, lane = (track, layer) ---------------------------------------
     int n_st = 0;
     if (active) {
@@ -515,6 +516,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   uint16_t* s_off = cvr.take<uint16_t>(ns + 1);
   float* s_hx = cvr.take<float>(a.hit_stage);
   uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage);
+  uint16_t* s_perm = cvr.take<uint16_t>(a.trk_stage);
   unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by s_cnt below
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp_areas);
   // while staging, the same region also receives the event's id and x ranges by two bulk copies (TMA)
@@ -590,7 +592,8 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       continue;
     }
     if (t1 == t0) continue;
-    if (n <= a.hit_stage) {
+    const bool staged = n <= a.hit_stage;
+    if (staged) {
       // ---- stage: a warp re-buckets one sector group at a time, per sector, keeping the x order -----------
       // (count -> warp scan over the group's sectors -> ordered scatter with match.any; no block barrier)
       bool bad_id = false;
@@ -698,9 +701,41 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       }
       if (bad_id) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_HIT_ID);
       __syncthreads();                             // s_cnt is dead from here on: the warp areas take its place
-      track_loop<true>(a, wa, S, &s_ticket, h0, t0, t1, T);
+    }
+    // ---- batch order: the tracks of the event by radius at the first layer, inner tracks first ---------------
+    // Inner tracks cross the busy sectors and have the long candidate lists; a batch costs what its heaviest
+    // track costs, so like goes with like and the heavy batches start first.  Results do not depend on the order.
+    const uint32_t nT = t1 - t0;
+    const uint16_t* perm = nullptr;
+    if (nT > (uint32_t)kTPW && nT <= a.trk_stage) {
+      float* keys = reinterpret_cast<float*>(s_warp_areas);    // scratch: the warp areas are idle here
+      const float dz0 = __fsub_rn(a.layer_z[0], a.vz);
+      for (uint32_t i = tid; i < ((nT + 3u) & ~3u); i += nt) {
+        float k = __int_as_float(0x7F800000);
+        if (i < nT) {
+          const float x = __ldg(a.vx + t0 + i) + __ldg(a.vtx + t0 + i) * dz0, y = __ldg(a.vy + t0 + i) + __ldg(a.vty + t0 + i) * dz0;
+          k = x * x + y * y;
+        }
+        keys[i] = k;
+      }
+      __syncthreads();
+      for (uint32_t i = tid; i < nT; i += nt) {
+        const float ki = keys[i];
+        uint32_t rank = 0;
+        for (uint32_t j = 0; j < nT; j += 4) {
+          const float4 v = *reinterpret_cast<const float4*>(keys + j);
+          rank += (v.x < ki || (v.x == ki && j < i)) + (v.y < ki || (v.y == ki && j + 1 < i)) +
+                  (v.z < ki || (v.z == ki && j + 2 < i)) + (v.w < ki || (v.w == ki && j + 3 < i));
+        }
+        s_perm[rank] = (uint16_t)i;
+      }
+      perm = s_perm;
+      __syncthreads();
+    }
+    if (staged) {
+      track_loop<true>(a, wa, S, &s_ticket, h0, t0, t1, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false>(a, wa, S, &s_ticket, h0, t0, t1, T);
+      track_loop<false>(a, wa, S, &s_ticket, h0, t0, t1, T, perm);
     }
   }
   if (tid == 0 && a.ticket) {                 // last CTA out re-arms the ticket for the next call
@@ -714,10 +749,10 @@ static int env_int(const char* name, int dflt) {
   return v && *v ? atoi(v) : dflt;
 }
 
-static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block) {
+static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block, uint32_t trk_stage = 0) {
   size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + (UT_COMPASS_YR_SMEM ? align16((size_t)ns * 8) : 0);
   b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
-  b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2);
+  b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2) + align16((size_t)trk_stage * 2);
   b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)),
                 align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4));   // staging scratch aliases the warp areas
   return b;
@@ -800,6 +835,16 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
+  // room for ordering up to 512 tracks per event, if it costs no resident CTA
+  a.trk_stage = 0;
+  {
+    const uint32_t want = (uint32_t)env_int("UT_COMPASS_TRK_STAGE", 512);
+    const size_t with = compass_smem_bytes(ns, ng, hit_stage, C, block, want);
+    if (want && with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
+      a.trk_stage = want;
+      smem = with;
+    }
+  }
   const void* kernel = block <= 256 ? kKernelSmall : kKernelLarge;
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
