@@ -835,14 +835,14 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  // room for ordering up to 512 tracks per event, if it costs no resident CTA
+  // room for ordering up to 2048 (else 1024, 512) tracks per event, if it costs no resident CTA
   a.trk_stage = 0;
-  {
-    const uint32_t want = (uint32_t)env_int("UT_COMPASS_TRK_STAGE", 512);
+  for (uint32_t want = (uint32_t)env_int("UT_COMPASS_TRK_STAGE", 2048); want >= 512; want /= 2) {
     const size_t with = compass_smem_bytes(ns, ng, hit_stage, C, block, want);
-    if (want && with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
+    if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
       a.trk_stage = want;
       smem = with;
+      break;
     }
   }
   const void* kernel = block <= 256 ? kKernelSmall : kKernelLarge;
