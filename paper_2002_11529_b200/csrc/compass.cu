@@ -10,6 +10,9 @@
 //            one pass: match.any ranks, per-sector counts, warp scan).  A sector's y range, stereo slope, z and
 //            weight are rows of the geometry table, so the y test of the window search becomes a per-sector
 //            test: the scan touches the hits of the one sector row the track crosses instead of all 14 rows.
+//   order    the tracks of the event are ranked by their radius at the first layer (counting rank in shared memory):
+//            a batch costs what its heaviest track costs and the inner tracks cross the busy sectors, so like goes
+//            with like and the heavy batches start first.  Results do not depend on the order.
 //   phase 1  lane = (track, layer), 8 tracks per warp (the paper's 2-D window kernel shape):
 //            straight-line extrapolation, column groups and sector row from a linear guess corrected against
 //            the tables (y ranges from L1), lower-bound search in busy sectors, |d| <= win test with early exit;
