@@ -325,8 +325,8 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
   // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
   const char* chunk_env = getenv("UT_PIPELINE_CHUNK_EVENTS");
-  const int kChunkEvents = chunk_env && *chunk_env ? atoi(chunk_env) : 2000;
-  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 2000);
+  const int kChunkEvents = chunk_env && *chunk_env ? atoi(chunk_env) : 500;
+  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
   bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&

@@ -260,7 +260,7 @@ def test_invalid_arguments(gpu, wl):
 @pytest.mark.parametrize("n_events", [1000, 37])
 def test_host_pipeline_matches_oracle(gpu, wl, n_events, monkeypatch):
     """ut_pipeline_run_host (HOST buffers in, HOST track SoA out; the call bench.py's e2e figure times).
-    1000 events run as 4 overlapped chunks of 250 (batches of >= 4000 events are chunked by default), 37 events as
+    1000 events run as 4 overlapped chunks of 250 (the default is chunks of >= 500 events), 37 events as
     one call: both must equal the oracle element by element."""
     import torch
     monkeypatch.setenv("UT_PIPELINE_CHUNK_EVENTS", "250")
