@@ -77,11 +77,9 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t ns = a.g.n_sectors, ng = a.g.n_groups;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
-  const uint32_t idn = min(a.g.id_table_size, 2048u);
 
   Carver cv(smem_raw);
   unsigned char* s_rawstage = cv.take<unsigned char>(a.raw_stage_bytes);
-  uint16_t* g_idtab = cv.take<uint16_t>(idn);     // raw id -> dense sector, 0xFFFF = invalid
   uint16_t* g_gfirst = cv.take<uint16_t>(ng + 1);
   uint32_t* s_cnt = cv.take<uint32_t>(ns);
   uint32_t* s_wpos = cv.take<uint32_t>(ns);
@@ -95,10 +93,6 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   __shared__ uint32_t s_warp[32];
 
   // geometry tables: staged once per CTA, reused for every event this CTA takes
-  for (uint32_t i = tid; i < idn; i += nt) {
-    const uint32_t s = a.g.id_to_sector[i];
-    g_idtab[i] = s < ns ? (uint16_t)s : (uint16_t)0xFFFFu;
-  }
   for (uint32_t i = tid; i <= ng; i += nt) g_gfirst[i] = (uint16_t)a.g.group_first_sector[i];
   if (tid == 0) {
     mbar_init(&s_bar, 1);
@@ -151,8 +145,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         const uint32_t rid = *reinterpret_cast<const uint32_t*>(rawp + rel);
         const uint32_t cnt = *reinterpret_cast<const uint32_t*>(rawp + rel + 4) & 0xFFFFu;
         uint32_t s = kInvalid;
-        if (rid < idn) { s = g_idtab[rid]; if (s == 0xFFFFu) s = kInvalid; }
-        else if (rid < a.g.id_table_size) s = __ldg(a.g.id_to_sector + rid);
+        if (rid < a.g.id_table_size) s = __ldg(a.g.id_to_sector + rid);   // 4 KB table, L1 / L2 resident
         if (s >= ns) { st |= UT_STATUS_UNKNOWN_SECTOR; continue; }
         if (o1 - o0 != ((6u + 2u * cnt + 3u) & ~3u)) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
         if (atomicCAS(&s_wpos[s], kInvalid, rel + 6u) != kInvalid) { st |= UT_STATUS_DUPLICATE_SECTOR; continue; }
@@ -353,9 +346,9 @@ static int env_int(const char* name, int dflt) {
   return v && *v ? atoi(v) : dflt;
 }
 
-static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t idn, uint32_t raw_stage, uint32_t sort_buf, int block) {
+static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, uint32_t sort_buf, int block) {
   size_t b = align16(raw_stage);
-  b += align16((size_t)idn * 2) + align16((size_t)(ng + 1) * 2);
+  b += align16((size_t)(ng + 1) * 2);
   b += 2 * align16((size_t)ns * 4) + align16((size_t)ng * 4);
   b += 2 * align16((size_t)(block / 32) * sort_buf * 4);
   return b;
@@ -387,7 +380,6 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
 
   // staging sizes from the only size the host knows without a sync: capacity / n_events
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
-  const uint32_t idn = std::min<uint32_t>(geom->id_table_size, 2048u);
   const unsigned long long avg = (hits_hint ? hits_hint : hits->capacity) / (unsigned long long)n_events + 1;
   const unsigned long long stage_hits = std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
   uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * stage_hits + 32u);
@@ -399,15 +391,15 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   // 5-warp CTAs keep a 1000-event batch resident at once (7 per SM); busy events get 8 warps per event
   int block = env_int("UT_DECODE_BLOCK", avg > 4096 ? 256 : 160);
   block = std::max(64, std::min(512, (block / 32) * 32));
-  size_t smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
+  size_t smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
   const size_t budget = (size_t)max_smem;
   while (smem > budget && raw_stage > 4096) {            // oversize events read their banks from global memory
     raw_stage = (raw_stage / 2) & ~15u;
-    smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
+    smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
   }
   while (smem > budget && sort_buf > 32) {
     sort_buf -= 32;
-    smem = decode_smem_bytes(ns, ng, idn, raw_stage, sort_buf, block);
+    smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.raw_stage_bytes = raw_stage; a.sort_buf = sort_buf;
