@@ -110,7 +110,10 @@ typedef struct {
                                  ut_decode did not fill (compass_track then assigns events statically). */
 } ut_hits;
 
-size_t ut_decode_workspace_bytes(int32_t max_events);
+/* Bytes of `workspace` for batches of up to `max_events` events decoded with `geometry` (control words and one
+ * look-back word per event; `geometry` may be NULL: the size does not depend on the tables today, the argument
+ * is SURVEY.md 8(b)'s and keeps the call stable if per-sector scratch moves here). */
+size_t ut_decode_workspace_bytes(int32_t max_events, const ut_geometry* geometry);
 int32_t ut_decode_workspace_init(void* workspace, int32_t max_events, ut_stream_t stream);
 
 /* ut_decode -- PAPER.md section IV.
@@ -231,6 +234,26 @@ typedef struct {
   int32_t compass_grid, compass_block, compass_smem_bytes, compass_hit_stage;
 } ut_launch_info;
 void ut_last_launch_info(ut_launch_info* out);
+
+/* Launch tuning, process-wide (HOST).  -1 = automatic.  The values are read ONCE from the environment when the
+ * library is first used (UT_DECODE_BLOCK, UT_DECODE_RAW_STAGE, UT_DECODE_SORT_BUF, UT_DECODE_MAX_CTAS_PER_SM,
+ * UT_COMPASS_BLOCK, UT_COMPASS_HIT_STAGE, UT_COMPASS_TRK_STAGE, UT_COMPASS_SPLIT, UT_PIPELINE_CHUNK_EVENTS); the
+ * hot-path calls never touch the environment.  ut_tuning_set replaces them (NULL: back to the environment's).
+ * Results never depend on these values, only launch shapes and which of the equivalent code paths run. */
+typedef struct {
+  int32_t decode_block;             /* threads per decode CTA */
+  int32_t decode_raw_stage_bytes;   /* shared-memory staging of an event's raw banks */
+  int32_t decode_sort_buf;          /* per-warp sort buffer, in hits */
+  int32_t decode_max_ctas_per_sm;
+  int32_t compass_block;            /* threads per Compass CTA */
+  int32_t compass_hit_stage;        /* hits of an event staged in shared memory; 0: window search on global memory */
+  int32_t compass_trk_stage;        /* tracks of an event that can be ordered by radius */
+  int32_t compass_split;            /* CTAs sharing one event's track batches (1, 2 or 4) */
+  int32_t pipeline_chunk_events;    /* ut_pipeline_run_host: events per overlapped chunk */
+  int32_t reserved[7];
+} ut_tuning;
+int32_t ut_tuning_get(ut_tuning* out);
+int32_t ut_tuning_set(const ut_tuning* in);
 
 const char* ut_version(void);
 /* Text of the last UT_ERR_CUDA on this thread ("<call>: <cuda error string>"), "" if none. */

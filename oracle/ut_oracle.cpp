@@ -90,9 +90,14 @@ int32_t oracle_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   std::vector<Hit> grp;
   for (int32_t e = 0; e < n_events; ++e) {
     for (auto& b : banks) b = Bank{nullptr, 0, false};
+    // the event's byte range: from its first bank offset to the first offset of the next event (or the end)
+    const uint64_t ev_begin = bank_offsets[(uint64_t)e * ns], ev_end = bank_offsets[(uint64_t)(e + 1) * ns];
     for (uint32_t j = 0; j < ns; ++j) {
       const uint64_t o0 = bank_offsets[(uint64_t)e * ns + j], o1 = bank_offsets[(uint64_t)e * ns + j + 1];
-      if (o1 < o0 + 6) { st |= ST_BAD_BANK_SIZE; continue; }
+      // DESIGN.md A22 (raw format of BASELINE.json configs[0] / SURVEY.md 8(d): banks are padded to 4 bytes and the
+      // banks of an event are contiguous): a bank that does not start on a 4-byte boundary, is shorter than its
+      // 6-byte header or does not lie inside [ev_begin, ev_end) is malformed -> ignored and flagged
+      if ((o0 & 3u) != 0 || o1 < o0 + 6 || o0 < ev_begin || o1 > ev_end) { st |= ST_BAD_BANK_SIZE; continue; }
       const uint32_t rid = rd32(raw + o0);
       const uint32_t cnt = rd16(raw + o0 + 4);
       const uint32_t s = rid < g->id_table_size ? g->id_to_sector[rid] : 0xFFFFFFFFu;

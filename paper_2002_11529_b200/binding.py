@@ -67,13 +67,20 @@ class ut_compact_tracks(C.Structure):
                 ("max_velo_total", C.c_uint32)]
 
 
+class ut_tuning(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("decode_block", "decode_raw_stage_bytes", "decode_sort_buf", "decode_max_ctas_per_sm", "compass_block",
+                 "compass_hit_stage", "compass_trk_stage", "compass_split", "pipeline_chunk_events")] + \
+               [("reserved", C.c_int32 * 7)]
+
+
 class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_raw_stage_bytes",
                  "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage")]
 
 
-EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_geometry_upload", "ut_geometry_free",
+EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
            "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
            "ut_pipeline_device_hits"]
@@ -81,7 +88,7 @@ EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_geometry_up
 _lib.ut_version.restype = C.c_char_p
 _lib.ut_last_error.restype = C.c_char_p
 _lib.ut_decode_workspace_bytes.restype = C.c_size_t
-_lib.ut_decode_workspace_bytes.argtypes = [C.c_int32]
+_lib.ut_decode_workspace_bytes.argtypes = [C.c_int32, C.c_void_p]
 _lib.ut_decode_workspace_init.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
 _lib.ut_geometry_upload.argtypes = [C.POINTER(ut_geometry), C.POINTER(ut_geometry)]
 _lib.ut_geometry_free.argtypes = [C.POINTER(ut_geometry)]
@@ -103,6 +110,8 @@ _lib.ut_pipeline_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_vo
                                       C.POINTER(ut_tracks), C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ut_pipeline_device_hits.argtypes = [C.c_void_p, C.POINTER(ut_hits), C.POINTER(C.c_void_p)]
 _lib.ut_last_launch_info.argtypes = [C.POINTER(ut_launch_info)]
+_lib.ut_tuning_get.argtypes = [C.POINTER(ut_tuning)]
+_lib.ut_tuning_set.argtypes = [C.POINTER(ut_tuning)]
 for _n in EXPORTS:
     if _n not in ("ut_version", "ut_last_error", "ut_decode_workspace_bytes", "ut_last_launch_info",
                   "compass_consolidate_workspace_bytes"):
@@ -166,8 +175,8 @@ def ut_geometry_upload(tables) -> Geometry:
     return Geometry(tables)
 
 
-def ut_decode_workspace_bytes(max_events: int) -> int:
-    return int(_lib.ut_decode_workspace_bytes(max_events))
+def ut_decode_workspace_bytes(max_events: int, geometry: "Geometry | None" = None) -> int:
+    return int(_lib.ut_decode_workspace_bytes(max_events, C.byref(geometry.c) if geometry is not None else None))
 
 
 class Hits:
@@ -181,7 +190,7 @@ class Hits:
             torch.empty(n, dtype=torch.float32, device=device) for _ in range(6))
         self.id = torch.empty(n, dtype=torch.int32, device=device)
         self.status = torch.zeros(1, dtype=torch.int32, device=device)
-        nbytes = ut_decode_workspace_bytes(max_events)
+        nbytes = ut_decode_workspace_bytes(max_events, geometry)
         self.workspace = torch.zeros((nbytes + 15) // 16 * 2, dtype=torch.int64, device=device)   # zeroed once
         self.hit_offsets = torch.zeros(max_events * geometry.n_groups + 1, dtype=torch.int32, device=device)
         self.geometry = geometry
@@ -306,6 +315,23 @@ def to_device_raw(raw: np.ndarray, device="cuda") -> torch.Tensor:
 
 def to_device_u32(a: np.ndarray, device="cuda") -> torch.Tensor:
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.uint32).view(np.int32)).to(device)
+
+
+def ut_tuning_get() -> ut_tuning:
+    t = ut_tuning()
+    _check(_lib.ut_tuning_get(C.byref(t)), "ut_tuning_get")
+    return t
+
+
+def ut_tuning_set(tuning: "ut_tuning | None" = None, **fields) -> None:
+    """Replace the process-wide launch tuning (None and no fields: back to the environment's values; fields given
+    by name override the current values).  Results never depend on it."""
+    if tuning is None and fields:
+        tuning = ut_tuning_get()
+    if tuning is not None:
+        for k, v in fields.items():
+            setattr(tuning, k, int(v))
+    _check(_lib.ut_tuning_set(C.byref(tuning) if tuning is not None else None), "ut_tuning_set")
 
 
 def last_launch_info() -> dict:

@@ -2,7 +2,9 @@
 // host, geometry upload, workspace, the two hot-path launches and the host-buffer pipeline.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -31,6 +33,85 @@ int32_t cuda_fail(const char* what, cudaError_t err) {
   return UT_ERR_CUDA;
 }
 
+namespace {
+constexpr int kMaxDevices = 64;
+struct DeviceEntry {
+  bool init = false;
+  DeviceInfo info = {};
+  bool opted[kNumKernelSlots] = {};
+  int max_dyn[kNumKernelSlots] = {};
+};
+std::mutex g_device_mu;
+DeviceEntry g_devices[kMaxDevices];
+
+std::mutex g_tuning_mu;
+bool g_tuning_init = false;
+ut_tuning g_tuning;
+
+int env_int(const char* name) {
+  const char* v = getenv(name);
+  return v && *v ? atoi(v) : -1;
+}
+void tuning_from_env(ut_tuning* t) {
+  for (int32_t* p = &t->decode_block; p <= &t->reserved[6]; ++p) *p = -1;
+  t->decode_block = env_int("UT_DECODE_BLOCK");
+  t->decode_raw_stage_bytes = env_int("UT_DECODE_RAW_STAGE");
+  t->decode_sort_buf = env_int("UT_DECODE_SORT_BUF");
+  t->decode_max_ctas_per_sm = env_int("UT_DECODE_MAX_CTAS_PER_SM");
+  t->compass_block = env_int("UT_COMPASS_BLOCK");
+  t->compass_hit_stage = env_int("UT_COMPASS_HIT_STAGE");
+  t->compass_trk_stage = env_int("UT_COMPASS_TRK_STAGE");
+  t->compass_split = env_int("UT_COMPASS_SPLIT");
+  t->pipeline_chunk_events = env_int("UT_PIPELINE_CHUNK_EVENTS");
+}
+}  // namespace
+
+ut_tuning tuning_snapshot() {
+  std::lock_guard<std::mutex> lock(g_tuning_mu);
+  if (!g_tuning_init) { tuning_from_env(&g_tuning); g_tuning_init = true; }
+  return g_tuning;
+}
+
+static int32_t device_entry(DeviceEntry** out) {
+  int dev = 0;
+  UTC_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return cuda_fail("device index above the library's table", cudaErrorInvalidDevice);
+  DeviceEntry& d = g_devices[dev];
+  if (!d.init) {
+    d.info.device = dev;
+    UTC_CUDA(cudaDeviceGetAttribute(&d.info.n_sm, cudaDevAttrMultiProcessorCount, dev));
+    UTC_CUDA(cudaDeviceGetAttribute(&d.info.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    UTC_CUDA(cudaDeviceGetAttribute(&d.info.smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    d.init = true;
+  }
+  *out = &d;
+  return UT_OK;
+}
+
+int32_t device_info(DeviceInfo* out) {
+  std::lock_guard<std::mutex> lock(g_device_mu);
+  DeviceEntry* d = nullptr;
+  if (const int32_t rc = device_entry(&d)) return rc;
+  *out = d->info;
+  return UT_OK;
+}
+
+int32_t kernel_max_dynamic_smem(const void* kernel, int slot, int* max_dyn) {
+  std::lock_guard<std::mutex> lock(g_device_mu);
+  DeviceEntry* d = nullptr;
+  if (const int32_t rc = device_entry(&d)) return rc;
+  if (!d->opted[slot]) {
+    cudaFuncAttributes fa;
+    UTC_CUDA(cudaFuncGetAttributes(&fa, kernel));
+    const int dyn = d->info.smem_optin - (int)fa.sharedSizeBytes;
+    UTC_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    d->max_dyn[slot] = dyn;
+    d->opted[slot] = true;
+  }
+  *max_dyn = d->max_dyn[slot];
+  return UT_OK;
+}
+
 struct GeomOwner {
   void* block = nullptr;     // one device allocation holding every table
 };
@@ -52,6 +133,19 @@ const char* ut_last_error(void) { return g_last_error; }
 
 void ut_last_launch_info(ut_launch_info* out) {
   if (out) *out = launch_info();
+}
+
+int32_t ut_tuning_get(ut_tuning* out) {
+  if (!out) return UT_ERR_NULL;
+  *out = tuning_snapshot();
+  return UT_OK;
+}
+
+int32_t ut_tuning_set(const ut_tuning* in) {
+  std::lock_guard<std::mutex> lock(g_tuning_mu);
+  if (in) g_tuning = *in; else tuning_from_env(&g_tuning);
+  g_tuning_init = true;
+  return UT_OK;
 }
 
 int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
@@ -148,14 +242,14 @@ int32_t ut_geometry_free(ut_geometry* g) {
   return UT_OK;
 }
 
-size_t ut_decode_workspace_bytes(int32_t max_events) {
+size_t ut_decode_workspace_bytes(int32_t max_events, const ut_geometry* /*geometry*/) {
   return 32 + 8 * (size_t)(max_events > 0 ? max_events : 0) + 8;   // 8 control words, then one look-back word per event
 }
 
 int32_t ut_decode_workspace_init(void* workspace, int32_t max_events, ut_stream_t stream) {
   if (!workspace) return UT_ERR_NULL;
   if (max_events < 0) return UT_ERR_ARG;
-  return cudaMemsetAsync(workspace, 0, ut_decode_workspace_bytes(max_events), (cudaStream_t)stream) == cudaSuccess
+  return cudaMemsetAsync(workspace, 0, ut_decode_workspace_bytes(max_events, nullptr), (cudaStream_t)stream) == cudaSuccess
              ? UT_OK : UT_ERR_CUDA;
 }
 
@@ -268,7 +362,7 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   const size_t s_raw = up(max_raw_bytes + 16), s_bo = up(((size_t)max_events * g->n_sectors + 1) * 4),
                s_ho = up(((size_t)max_events * g->n_groups + 1) * 4), s_vo = up(((size_t)max_events + 1) * 4),
                s_st = 256, s_v = up((size_t)max_velo * 4), s_h = up((size_t)max_hits * 4),
-               s_ws = up(ut_decode_workspace_bytes(max_events)), s_ti = up((size_t)max_velo * 16);
+               s_ws = up(ut_decode_workspace_bytes(max_events, g)), s_ti = up((size_t)max_velo * 16);
   const size_t total = s_raw + s_bo + s_ho + s_vo + s_st + 4 * s_v + 7 * s_h + s_ws + s_ti + 3 * s_v;
   if (cudaMalloc(&p->block, total) != cudaSuccess) { delete p; return UT_ERR_CUDA; }
   unsigned char* q = p->block;
@@ -324,8 +418,7 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   // The batch is cut into up to 4 chunks of events: chunk k+1 is copied in while chunk k is decoded and
   // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
   // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
-  const char* chunk_env = getenv("UT_PIPELINE_CHUNK_EVENTS");
-  const int kChunkEvents = chunk_env && *chunk_env ? atoi(chunk_env) : 500;
+  const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 500);
   int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
   bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&

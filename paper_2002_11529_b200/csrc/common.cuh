@@ -37,6 +37,19 @@ inline GeomDev make_geom_dev(const ut_geometry* g) {
 ut_launch_info& launch_info();
 // records "<what>: <cuda error string>" for ut_last_error(); returns UT_ERR_CUDA
 int32_t cuda_fail(const char* what, cudaError_t err);
+
+// Per-device facts and the dynamic shared-memory opt-in of the kernels.  cudaFuncAttributeMaxDynamicSharedMemorySize
+// is a per-DEVICE attribute: the table is keyed by the current device and filled under a mutex, so any number of
+// devices and host threads may call into the library.
+struct DeviceInfo { int device, n_sm, smem_optin, smem_per_sm; };
+enum KernelSlot { kSlotDecode = 0, kSlotCompassSmall, kSlotCompassLarge, kSlotWindows, kSlotTracklets, kNumKernelSlots = 8 };
+int32_t device_info(DeviceInfo* out);
+// largest dynamic shared-memory size `kernel` may ask for on the current device (opted in on its first use there)
+int32_t kernel_max_dynamic_smem(const void* kernel, int slot, int* max_dyn);
+// the process-wide tuning values (ut_tuning_get / ut_tuning_set), read from the environment once
+ut_tuning tuning_snapshot();
+inline int tuned(int32_t v, int dflt) { return v >= 0 ? (int)v : dflt; }
+
 #define UTC_CUDA(call)                                              \
   do {                                                              \
     const cudaError_t utc_err__ = (call);                           \

@@ -584,10 +584,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     if (tid == 0) s_ticket = 0;
     const uint32_t n = h1 - h0;
     // (__syncthreads_or returns a truth value, not the OR of the arguments; n is the same in every thread)
-    const int flag = __syncthreads_or(bad ? 1 : 0) ? 1 : (n > 65535u ? 2 : 0);
+    // an event whose hits end past `capacity` was not written by the decode (UT_STATUS_CAPACITY there): its range of
+    // the hit arrays must not be read
+    const int flag = __syncthreads_or(bad ? 1 : 0) ? 1 : ((unsigned long long)h1 > a.capacity ? 4 : (n > 65535u ? 2 : 0));
     if (flag) {                                    // uniform: report and emit "no tracklet" for every track
       if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
-                                           (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u));
+                                           (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u) |
+                                           (flag & 4 ? (uint32_t)UT_STATUS_CAPACITY : 0u));
       for (uint32_t t = t0 + tid; t < t1; t += nt) {
         for (int k = 0; k < 4; ++k) a.out_idx[(size_t)k * T + t] = -1;
         a.out_n[t] = 0; a.out_qop[t] = 0.f; a.out_chi2[t] = 0.f;
@@ -718,6 +721,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
         if (i < nT) {
           const float x = __ldg(a.vx + t0 + i) + __ldg(a.vtx + t0 + i) * dz0, y = __ldg(a.vy + t0 + i) + __ldg(a.vty + t0 + i) * dz0;
           k = x * x + y * y;
+          if (!(k == k)) k = __int_as_float(0x7F800000);       // NaN state: last, so that the rank stays a permutation
         }
         keys[i] = k;
       }
@@ -747,42 +751,33 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   }
 }
 
-static int env_int(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return v && *v ? atoi(v) : dflt;
-}
-
 static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block, uint32_t trk_stage = 0) {
   size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + (UT_COMPASS_YR_SMEM ? align16((size_t)ns * 8) : 0);
   b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
   b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2) + align16((size_t)trk_stage * 2);
-  b += std::max(align16((size_t)(block / 32) * warp_area_bytes(C)),
-                align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4));   // staging scratch aliases the warp areas
+  b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C)),
+                 align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4),   // staging scratch aliases the warp areas
+                 align16((size_t)trk_stage * 4)});                                      // and so do the ordering keys
   return b;
 }
 
-// Two register budgets: CTAs of <= 256 threads at >= 3 per SM, and larger CTAs (big events / C = 32,
+// Two register budgets: CTAs of <= 224 threads at 4 per SM (72 registers), and larger CTAs (big events / C = 32,
 // where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
-static const void* const kKernelSmall = reinterpret_cast<const void*>(&compass_kernel<256, 3>);
+constexpr int kSmallBlock = 224;
+static const void* const kKernelSmall = reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4>);
 static const void* const kKernelLarge = reinterpret_cast<const void*>(&compass_kernel<768, 1>);
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
                        cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint) {
-  static int max_smem = 0, n_sm = 0, sm_smem = 0;     // max_smem = largest dynamic size a CTA may ask for
-  if (!max_smem) {
-    int dev = 0, optin = 0;
-    UTC_CUDA(cudaGetDevice(&dev));
-    UTC_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    UTC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    UTC_CUDA(cudaDeviceGetAttribute(&sm_smem, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
-    cudaFuncAttributes fa;
-    UTC_CUDA(cudaFuncGetAttributes(&fa, kKernelSmall));
-    const int dyn = optin - (int)fa.sharedSizeBytes;
-    UTC_CUDA(cudaFuncSetAttribute(kKernelSmall, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-    UTC_CUDA(cudaFuncSetAttribute(kKernelLarge, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-    max_smem = dyn;
-  }
+  DeviceInfo dev;
+  int max_smem = 0, max_smem_large = 0;               // largest dynamic size a CTA may ask for on this device
+  if (const int32_t rc = device_info(&dev)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernelSmall, kSlotCompassSmall, &max_smem)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernelLarge, kSlotCompassLarge, &max_smem_large)) return rc;
+  max_smem = std::min(max_smem, max_smem_large);
+  const int n_sm = dev.n_sm, sm_smem = dev.smem_per_sm;
+  const ut_tuning tune = tuning_snapshot();
   const ut_geometry* geom = hits->geom;
   CompassArgs a;
   a.hx = hits->x_at_y0; a.hid = hits->id; a.hyb = hits->y_begin; a.hye = hits->y_end;
@@ -809,17 +804,17 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   // the capacity bound counts the pad half-word of every odd bank as a hit: about n_sectors / 2 per event
   const unsigned long long est = avg > ns ? avg - ns / 2 : avg;
   uint32_t hit_stage = (uint32_t)std::min<unsigned long long>(((est + est / 8 + 127) / 128) * 128 + 128, 65536ull);
-  hit_stage = (uint32_t)env_int("UT_COMPASS_HIT_STAGE", (int)hit_stage);
+  hit_stage = (uint32_t)tuned(tune.compass_hit_stage, (int)hit_stage);
   const size_t budget = (size_t)max_smem;
   // Block size: the one that keeps the most warps resident per SM (shared memory is the limit; about 24
   // warps per SM is what the register budget of the small variant allows).
-  int block = env_int("UT_COMPASS_BLOCK", 0);
+  int block = tuned(tune.compass_block, 0);
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= 768; b += 32) {
       const size_t sm = compass_smem_bytes(ns, ng, hit_stage, C, b) + 1024;
       if (sm > budget) continue;
-      const int regs_warps = b <= 256 ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
+      const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
       const int warps = ctas * (b / 32);
       if (warps > best_warps) { best_warps = warps; block = b; }
@@ -840,7 +835,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.hit_stage = hit_stage;
   // room for ordering up to 2048 (else 1024, 512) tracks per event, if it costs no resident CTA
   a.trk_stage = 0;
-  for (uint32_t want = (uint32_t)env_int("UT_COMPASS_TRK_STAGE", 2048); want >= 512; want /= 2) {
+  for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
     const size_t with = compass_smem_bytes(ns, ng, hit_stage, C, block, want);
     if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
       a.trk_stage = want;
@@ -848,7 +843,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
       break;
     }
   }
-  const void* kernel = block <= 256 ? kKernelSmall : kKernelLarge;
+  const void* kernel = block <= kSmallBlock ? kKernelSmall : kKernelLarge;
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
   if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);

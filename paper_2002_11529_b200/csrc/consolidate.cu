@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(kThreads) consolidate_kernel(const Consolidate
   const int n_tiles = too_many ? 0 : (int)((T + kTile - 1) / kTile);
   if (tid == 0) s_epoch = ld_volatile_u32(a.ctrl + 2);
   uint32_t st = too_many ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u;
-  if (n_tiles == 0 && blockIdx.x == 0)             // no VELO track at all: every event owns the empty range
+  if (n_tiles == 0 && !too_many && blockIdx.x == 0)   // no VELO track at all: every event owns the empty range
     for (int e = tid; e <= a.n_events; e += kThreads) a.track_offsets[e] = 0;
   for (;;) {
     __syncthreads();                               // previous tile fully consumed
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(kThreads) consolidate_kernel(const Consolidate
       const uint32_t r = s_excl[q];
       if (s_excl[q + 1] == r) continue;            // no tracklet
       const unsigned long long P = (unsigned long long)base + r;
-      if (P >= a.capacity) { st = UT_STATUS_CAPACITY; continue; }
+      if (P >= a.capacity) { st |= UT_STATUS_CAPACITY; continue; }
       a.o_velo[P] = t;
 #pragma unroll
       for (int l = 0; l < 4; ++l) a.o_idx[(size_t)l * a.capacity + P] = __ldg(a.idx + (size_t)l * T + t);
@@ -108,6 +108,7 @@ __global__ void __launch_bounds__(kThreads) consolidate_kernel(const Consolidate
       for (int e = lo_e + tid; e <= a.n_events; e += kThreads) {
         const uint32_t b = __ldg(a.velo_offsets + e);
         if (b > hi || (b == hi && hi != T)) break;   // boundary belongs to a later tile
+        if (b < t0) { st |= UT_STATUS_BAD_OFFSETS; continue; }   // offsets run backwards: nothing to look up
         a.track_offsets[e] = base + s_excl[b - t0];
       }
     }
@@ -129,12 +130,9 @@ size_t consolidate_workspace_bytes(uint32_t max_velo) {
 
 int32_t launch_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events, uint32_t n_velo_hint,
                            ut_compact_tracks* out, uint32_t* track_offsets, cudaStream_t stream) {
-  static int n_sm = 0;
-  if (!n_sm) {
-    int dev = 0;
-    UTC_CUDA(cudaGetDevice(&dev));
-    UTC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-  }
+  DeviceInfo dev;
+  if (const int32_t rc = device_info(&dev)) return rc;
+  const int n_sm = dev.n_sm;
   ConsolidateArgs a;
   a.idx = tracks->hit_idx; a.n = tracks->n_hits; a.qop = tracks->qop; a.chi2 = tracks->chi2;
   a.velo_offsets = velo_offsets; a.n_events = n_events;

@@ -341,11 +341,6 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   }
 }
 
-static int env_int(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return v && *v ? atoi(v) : dflt;
-}
-
 static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, uint32_t sort_buf, int block) {
   size_t b = align16(raw_stage);
   b += align16((size_t)(ng + 1) * 2);
@@ -357,18 +352,13 @@ static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, ui
 int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events, const ut_geometry* geom,
                       ut_hits* hits, uint32_t* hit_offsets, cudaStream_t stream, const uint32_t* carry_in,
                       unsigned long long hits_hint) {
-  static int n_sm = 0, max_smem = 0;     // max_smem = largest dynamic size this kernel may ask for
-  if (!n_sm) {
-    int dev = 0, optin = 0;
-    UTC_CUDA(cudaGetDevice(&dev));
-    UTC_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    cudaFuncAttributes fa;
-    UTC_CUDA(cudaFuncGetAttributes(&fa, ut_decode_kernel));
-    const int dyn = optin - (int)fa.sharedSizeBytes;
-    UTC_CUDA(cudaFuncSetAttribute(ut_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-    UTC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    max_smem = dyn;
-  }
+  DeviceInfo dev;
+  int max_smem = 0;                      // largest dynamic size this kernel may ask for on this device
+  if (const int32_t rc = device_info(&dev)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(reinterpret_cast<const void*>(&ut_decode_kernel), kSlotDecode, &max_smem))
+    return rc;
+  const int n_sm = dev.n_sm;
+  const ut_tuning tune = tuning_snapshot();
   DecodeArgs a;
   a.raw = raw; a.bank_offsets = bank_offsets; a.n_events = n_events; a.g = make_geom_dev(geom);
   a.x = hits->x_at_y0; a.z = hits->z_at_y0; a.yb = hits->y_begin; a.ye = hits->y_end; a.dxdy = hits->dxdy;
@@ -383,13 +373,13 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   const unsigned long long avg = (hits_hint ? hits_hint : hits->capacity) / (unsigned long long)n_events + 1;
   const unsigned long long stage_hits = std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
   uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * stage_hits + 32u);
-  raw_stage = (uint32_t)env_int("UT_DECODE_RAW_STAGE", (int)raw_stage) & ~15u;
+  raw_stage = (uint32_t)tuned(tune.decode_raw_stage_bytes, (int)raw_stage) & ~15u;
   // per-warp sort buffer: twice the mean group size, at least 64, a multiple of 32
   uint32_t sort_buf = (uint32_t)std::min<unsigned long long>(((2 * avg / ng + 31) / 32) * 32 + 32, 1024);
   sort_buf = std::max(64u, sort_buf);
-  sort_buf = ((uint32_t)env_int("UT_DECODE_SORT_BUF", (int)sort_buf) + 31u) & ~31u;
+  sort_buf = ((uint32_t)tuned(tune.decode_sort_buf, (int)sort_buf) + 31u) & ~31u;
   // 5-warp CTAs keep a 1000-event batch resident at once (7 per SM); busy events get 8 warps per event
-  int block = env_int("UT_DECODE_BLOCK", avg > 4096 ? 256 : 160);
+  int block = tuned(tune.decode_block, avg > 4096 ? 256 : 160);
   block = std::max(64, std::min(512, (block / 32) * 32));
   size_t smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
   const size_t budget = (size_t)max_smem;
@@ -407,7 +397,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ut_decode_kernel, block, smem));
   if (per_sm < 1) return cuda_fail("decode kernel does not fit on an SM", cudaErrorInvalidConfiguration);
-  per_sm = std::min(per_sm, env_int("UT_DECODE_MAX_CTAS_PER_SM", 8));
+  per_sm = std::min(per_sm, std::max(1, tuned(tune.decode_max_ctas_per_sm, 8)));
   const int grid = std::max(1, std::min(n_events, n_sm * per_sm));
   ut_decode_kernel<<<grid, block, smem, stream>>>(a);
   UTC_CUDA(cudaGetLastError());

@@ -201,3 +201,28 @@ def test_error_status(geom):
     h = oracle.decode(raw, offs, 1, geom, capacity=2)
     assert h.status & oracle.ST_CAPACITY and h.hit_offsets[-1] == 3
     assert oracle.decode(raw, offs, 1, geom).status == 0
+
+
+def test_bank_alignment_and_range_rule(geom):
+    """DESIGN.md A22: a bank off a 4-byte boundary, or outside its event's byte range, is ignored and flagged even
+    when its size field is consistent.  Expected hits come from the encoder inputs (which banks survive)."""
+    import malformed
+    raw, offs, want, j = malformed.misaligned_tail(geom)
+    h = oracle.decode(raw, offs, 1, geom)
+    assert h.status == oracle.ST_BAD_BANK_SIZE
+    assert sorted(h.id[:h.n_hits].astype(np.int64).tolist()) == want
+    # the same bytes with the cut undone decode completely: the rule, not the data, removed the tail
+    raw_ok = np.concatenate([raw[:int(offs[j + 1])], np.zeros(2, np.uint8), raw[int(offs[j + 1]):]])
+    offs_ok = offs.astype(np.int64); offs_ok[j + 1:] += 2
+    assert oracle.decode(raw_ok, offs_ok.astype(np.uint32), 1, geom).status == 0
+
+    raw, offs, want2 = malformed.foreign_bank(geom)
+    h = oracle.decode(raw, offs, 2, geom)
+    assert h.status == oracle.ST_BAD_BANK_SIZE               # in particular no DUPLICATE / foreign words
+    e0 = slice(0, int(h.hit_offsets[64])); e1 = slice(int(h.hit_offsets[64]), h.n_hits)
+    assert sorted(h.id[e0].astype(np.int64).tolist()) == want2[0]
+    assert sorted(h.id[e1].astype(np.int64).tolist()) == want2[1]
+    # an event whose end lies in front of its begin loses every bank
+    offs_bad = offs.copy(); offs_bad[896] = offs[2 * 896] + 4
+    h = oracle.decode(raw, offs_bad, 2, geom)
+    assert h.status & oracle.ST_BAD_BANK_SIZE and h.hit_offsets[64] <= len(want2[0])
