@@ -68,3 +68,85 @@ def compare_tracks(ref, got, rel=1e-5, status=0):
     assert np.allclose(got["qop"][ok], ref.qop[ok], rtol=rel, atol=0)
     assert np.allclose(got["chi2"][ok], ref.chi2[ok], rtol=rel, atol=0)
     return int((~same_idx).sum()), int(near_tie.sum())
+
+
+# ---- guard bands: every output array sits between two 4 KB canaries (the pool has no compute-sanitizer) -------
+GUARD = 1024                        # elements in front of and behind the array
+_CANARY = {"float32": -12345.678, "int32": -0x5A5A5A5B, "int64": -0x5A5A5A5A5A5A5A5B}
+
+
+def _guarded(n, dtype):
+    import torch
+    name = str(dtype).split(".")[-1]
+    full = torch.full((n + 2 * GUARD,), _CANARY[name], dtype=dtype, device="cuda")
+    return full, full[GUARD:GUARD + n]
+
+
+def check_guards(guards):
+    for name, full, n in guards:
+        c = _CANARY[str(full.dtype).split(".")[-1]]
+        front, back = full[:GUARD], full[GUARD + n:]
+        assert bool((front == c).all()) and bool((back == c).all()), f"canary of {name} overwritten"
+
+
+def guarded_hits(B, capacity, max_events, geometry):
+    """B.Hits whose arrays have EXACTLY `capacity` elements between canaries (hit_offsets, status, workspace too)."""
+    import torch
+    h = B.Hits(capacity, max_events, geometry)
+    guards = []
+    n = max(int(capacity), 1)
+    for f in h.FIELDS:
+        full, view = _guarded(n, torch.int32 if f == "id" else torch.float32)
+        setattr(h, f, view)
+        guards.append((f, full, n))
+    no = max_events * geometry.n_groups + 1
+    full, h.hit_offsets = _guarded(no, torch.int32)
+    guards.append(("hit_offsets", full, no))
+    full, h.status = _guarded(1, torch.int32)
+    h.status.zero_()
+    guards.append(("hits.status", full, 1))
+    nw = (B.ut_decode_workspace_bytes(max_events, geometry) + 7) // 8
+    full, h.workspace = _guarded(nw, torch.int64)
+    h.workspace.zero_()
+    guards.append(("workspace", full, nw))
+    h.c = B.ut_hits(h.x_at_y0.data_ptr(), h.z_at_y0.data_ptr(), h.y_begin.data_ptr(), h.y_end.data_ptr(),
+                    h.dxdy.data_ptr(), h.weight.data_ptr(), h.id.data_ptr(), int(capacity), h.c.geom,
+                    h.status.data_ptr(), h.workspace.data_ptr())
+    return h, guards
+
+
+def guarded_tracks(B, n_velo_total):
+    import torch
+    t = B.Tracks(n_velo_total)
+    n = max(int(n_velo_total), 1)
+    guards = []
+    for f, m, dt in (("hit_idx", 4 * n, torch.int32), ("n_hits", n, torch.int32), ("qop", n, torch.float32),
+                     ("chi2", n, torch.float32), ("status", 1, torch.int32)):
+        full, view = _guarded(m, dt)
+        setattr(t, f, view)
+        guards.append(("tracks." + f, full, m))
+    t.status.zero_()
+    t.c = B.ut_tracks(t.hit_idx.data_ptr(), t.n_hits.data_ptr(), t.qop.data_ptr(), t.chi2.data_ptr(), t.status.data_ptr())
+    return t, guards
+
+
+def guarded_compact(B, capacity, max_velo_total, max_events):
+    import torch
+    c = B.CompactTracks(capacity, max_velo_total, max_events)
+    n = max(int(capacity), 1)
+    guards = []
+    for f, m, dt in (("velo_index", n, torch.int32), ("hit_idx", 4 * n, torch.int32), ("n_hits", n, torch.int32),
+                     ("qop", n, torch.float32), ("chi2", n, torch.float32), ("status", 1, torch.int32),
+                     ("track_offsets", max_events + 1, torch.int32)):
+        full, view = _guarded(m, dt)
+        setattr(c, f, view)
+        guards.append(("compact." + f, full, m))
+    c.status.zero_()
+    nw = (B.compass_consolidate_workspace_bytes(int(max_velo_total)) + 7) // 8
+    full, c.workspace = _guarded(nw, torch.int64)
+    c.workspace.zero_()
+    guards.append(("compact.workspace", full, nw))
+    c.c = B.ut_compact_tracks(c.velo_index.data_ptr(), c.hit_idx.data_ptr(), c.n_hits.data_ptr(), c.qop.data_ptr(),
+                              c.chi2.data_ptr(), int(capacity), c.status.data_ptr(), c.workspace.data_ptr(),
+                              int(max_velo_total))
+    return c, guards

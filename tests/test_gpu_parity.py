@@ -223,13 +223,19 @@ def test_repeated_calls_reuse_workspace(gpu, wl):
     compare_decode(ref, got, off, st)
 
 
-def test_small_staging_takes_generic_paths(gpu, wl, monkeypatch):
-    """Force the events through the non-staged decode path and the global-memory Compass path."""
+def test_small_staging_takes_generic_paths(gpu, wl):
+    """Force the events through the non-staged decode path and the global-memory Compass path (ut_tuning_set:
+    the library reads its environment knobs once, so the launch shapes are set through the API)."""
     geom, b, p = wl(2, 12)
-    monkeypatch.setenv("UT_DECODE_SORT_BUF", "32")
-    monkeypatch.setenv("UT_DECODE_RAW_STAGE", "4096")
-    monkeypatch.setenv("UT_COMPASS_HIT_STAGE", "512")
-    check_batch(gpu, geom, b, p)
+    gpu.B.ut_tuning_set(decode_sort_buf=32, decode_raw_stage_bytes=4096, compass_hit_stage=512)
+    try:
+        t = gpu.B.ut_tuning_get()
+        assert (t.decode_sort_buf, t.decode_raw_stage_bytes, t.compass_hit_stage, t.compass_block) == (32, 4096, 512, -1)
+        check_batch(gpu, geom, b, p)
+        li = gpu.B.last_launch_info()
+        assert li["compass_hit_stage"] == 512
+    finally:
+        gpu.B.ut_tuning_set(None)
 
 
 def test_tracks_empty_cases(gpu, geom):
@@ -258,12 +264,12 @@ def test_invalid_arguments(gpu, wl):
 
 
 @pytest.mark.parametrize("n_events", [1000, 37])
-def test_host_pipeline_matches_oracle(gpu, wl, n_events, monkeypatch):
+def test_host_pipeline_matches_oracle(gpu, wl, n_events):
     """ut_pipeline_run_host (HOST buffers in, HOST track SoA out; the call bench.py's e2e figure times).
     1000 events run as 4 overlapped chunks of 250 (the default is chunks of >= 500 events), 37 events as
     one call: both must equal the oracle element by element."""
     import torch
-    monkeypatch.setenv("UT_PIPELINE_CHUNK_EVENTS", "250")
+    gpu.B.ut_tuning_set(pipeline_chunk_events=250)
     geom, b, p = wl(3, n_events)
     h_ref, t_ref = oracle_run(b, geom, p)
     B = gpu.B
@@ -290,6 +296,7 @@ def test_host_pipeline_matches_oracle(gpu, wl, n_events, monkeypatch):
         assert np.array_equal(out_h["qop"].numpy().view(np.uint32), t_ref.qop.view(np.uint32))
         out_h["n_hits"].fill_(-7)
     pipe.destroy()
+    gpu.B.ut_tuning_set(None)
 
 
 def _consolidate_both(gpu, t_idx, t_n, t_qop, t_chi2, vo, n_events, capacity=None):
