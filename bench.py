@@ -32,16 +32,36 @@ if ROOT not in sys.path:
 METRIC = "ut_decode_compass_events_per_s"
 UNIT = "events/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
-# profiles/ (config 3; taken with the bench's own L2 flush between steps).  Keyed by workload, then kernel.
-NCU_DRAM_TRAFFIC = {
-    "config3_throughput1000": {"compass_kernel": 18.63e6, "ut_decode_kernel": 18.20e6,
-                               "source": "profiles/r1d_final_round1.md"},
-}
-# smsp__inst_executed.sum per launch from the same captures: the kernels are bound by instruction issue, so the
-# line also carries achieved warp-instructions/s against 148 SMs x 4 schedulers x 1 inst/clk x sm_max_mhz
-NCU_WARP_INST = {"config3_throughput1000": {"compass_kernel": 81.74e6, "ut_decode_kernel": 40.10e6}}
+NCU_COUNTERS = os.path.join(ROOT, "profiles", "ncu_counters.json")
+CSRC = os.path.join(ROOT, "paper_2002_11529_b200", "csrc")
 
+
+def csrc_hash() -> str:
+    """sha256 over the kernel sources (names and contents): the key profiles/ncu_counters.json was captured at.
+    (The GPU box has no .git, so the tree hash is computed from the files themselves.)"""
+    import hashlib
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            h.update(open(os.path.join(CSRC, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_counters(workload: str):
+    """Per-launch ncu counters (DRAM bytes, warp instructions) of the committed `ncu --set full` capture, or
+    (None, reason) when the kernel sources changed since the capture: a stale figure is not reported."""
+    try:
+        doc = json.load(open(NCU_COUNTERS))
+    except Exception as exc:
+        return None, f"profiles/ncu_counters.json unreadable: {exc}"
+    if doc.get("csrc_sha256_16") != csrc_hash():
+        return None, (f"kernel sources changed since the capture (captured at {doc.get('csrc_sha256_16')} = commit "
+                      f"{doc.get('commit')}, now {csrc_hash()}): re-run the ncu capture named in {doc.get('source')}")
+    w = doc.get("workloads", {}).get(workload)
+    if not w:
+        return None, f"no ncu capture for workload {workload}"
+    return dict(w, source=doc.get("source"), commit=doc.get("commit")), None
 
 
 def parse_args():
@@ -54,6 +74,7 @@ def parse_args():
     ap.add_argument("--events", type=int, default=None, help="override the number of events per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (configs 1, 2, 4, 5)")
     ap.add_argument("--sweep", action="store_true", help="config 5: all 18 settings with efficiency / ghost rate")
     return ap.parse_args()
 
@@ -120,74 +141,107 @@ class ClockSampler:
 
 
 def oracle_chunked(batch, geom, params, lo, hi, threads):
-    """The oracle, as it stands, over disjoint event chunks on `threads` host threads (ctypes drops the GIL)."""
+    """The oracle, as it stands, over disjoint event chunks on `threads` host threads (ctypes drops the GIL).
+    Every thread decodes its chunk, waits for the others, then tracks it: returns the wall time of the decode
+    phase, of the tracking phase and of both (SURVEY.md 8(d) "oracle timed beside it": decode-only,
+    tracking-only, end to end)."""
     import oracle
     cuts = np.linspace(lo, hi, threads + 1).astype(int)
-    ns, ng = geom.n_sectors, geom.n_groups
+    ns = geom.n_sectors
+    gate = threading.Barrier(threads)
+    stamps = [0.0, 0.0, 0.0]
 
-    def work(a, b):
-        if b <= a:
-            return
+    def work(k, a, b):
         bo = batch.bank_offsets[a * ns:b * ns + 1]
-        cap = (int(bo[-1]) - int(bo[0]) - 6 * (b - a) * ns) // 2
-        h = oracle.decode(batch.raw, bo, b - a, geom, cap)
+        cap = max((int(bo[-1]) - int(bo[0]) - 6 * (b - a) * ns) // 2, 0)
         vo = batch.velo_offsets[a:b + 1]
         T = int(vo[-1]) - int(vo[0])
-        out = oracle.Tracks(np.full((4, T), -1, np.int32), np.zeros(T, np.int32), np.zeros(T, np.float32),
-                            np.zeros(T, np.float32), None, None, None, None)
-        v0 = int(vo[0])
-        sl = slice(v0, v0 + T)
-        oracle.compass_into(out, h, batch.velo_x[sl], batch.velo_y[sl], batch.velo_tx[sl], batch.velo_ty[sl],
-                            batch.velo_z, (vo - vo[0]).astype(np.uint32), b - a, geom, params, 0, extras=False)
+        out = oracle.Tracks(np.full((4, max(T, 1)), -1, np.int32), np.zeros(max(T, 1), np.int32),
+                            np.zeros(max(T, 1), np.float32), np.zeros(max(T, 1), np.float32), None, None, None, None)
+        sl = slice(int(vo[0]), int(vo[0]) + T)
+        v = [np.ascontiguousarray(x[sl]) for x in (batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty)]
+        vo0 = (vo - vo[0]).astype(np.uint32)
+        gate.wait()
+        if k == 0:
+            stamps[0] = time.perf_counter()
+        h = oracle.decode(batch.raw, bo, b - a, geom, cap) if b > a else None
+        gate.wait()
+        if k == 0:
+            stamps[1] = time.perf_counter()
+        if b > a and T > 0:
+            oracle.compass_into(out, h, v[0], v[1], v[2], v[3], batch.velo_z, vo0, b - a, geom, params, 0, extras=False)
+        gate.wait()
+        if k == 0:
+            stamps[2] = time.perf_counter()
 
-    ts = [threading.Thread(target=work, args=(int(a), int(b))) for a, b in zip(cuts[:-1], cuts[1:])]
-    t0 = time.perf_counter()
+    ts = [threading.Thread(target=work, args=(k, int(a), int(b))) for k, (a, b) in enumerate(zip(cuts[:-1], cuts[1:]))]
     for t in ts:
         t.start()
     for t in ts:
         t.join()
-    return time.perf_counter() - t0
+    return stamps[1] - stamps[0], stamps[2] - stamps[1], stamps[2] - stamps[0]
 
 
-def cpu_baseline(batch, geom, params, budget_s=4.0):
+def time_oracle(batch, geom, params, threads, budget_s, max_reps=50):
+    """events/s of the oracle on `threads` host threads over all events of `batch`: decode-only, tracking-only,
+    end to end (sums over whole passes; at least one pass)."""
+    n = batch.n_events
+    reps, td, tc, tb = 0, 0.0, 0.0, 0.0
+    while (tb < budget_s and reps < max_reps) or reps == 0:
+        d, c, both = oracle_chunked(batch, geom, params, 0, n, threads)
+        td, tc, tb, reps = td + d, tc + c, tb + both, reps + 1
+    return {"events_per_s": n * reps / tb, "decode_only_events_per_s": n * reps / td,
+            "tracking_only_events_per_s": n * reps / tc, "passes": reps, "wall_s": tb}
+
+
+def cpu_baseline(batch, geom, params, budget_s=6.0):
+    """The oracle as it stands on the GPU box's host cores: (i) one thread, (ii) all threads
+    over disjoint event chunks; decode-only / tracking-only / end to end each."""
     import oracle
     oracle.build()
     cores = os.cpu_count() or 1
     n = batch.n_events
-    oracle_chunked(batch, geom, params, 0, min(n, 4 * cores), cores)      # warm the library
-    reps, total = 0, 0.0
-    while total < budget_s and reps < 50:
-        total += oracle_chunked(batch, geom, params, 0, n, cores)
-        reps += 1
-    return {"value": n * reps / total, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"all {n} events of the workload x {reps} passes, oracle decode+compass on {cores} threads "
-                      f"over disjoint event chunks ({total:.1f} s wall)"}
+    oracle_chunked(batch, geom, params, 0, min(n, 4 * cores), min(cores, max(n, 1)))      # warm the library
+    many = time_oracle(batch, geom, params, min(cores, max(n, 1)), budget_s)
+    one = time_oracle(batch, geom, params, 1, budget_s / 2, max_reps=3)
+    return {"value": many["events_per_s"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"all {n} events of the workload x {many['passes']} passes, oracle decode + compass on {cores} "
+                      f"threads over disjoint event chunks ({many['wall_s']:.1f} s wall); one thread: {one['passes']} "
+                      f"pass(es) over the same {n} events ({one['wall_s']:.1f} s)",
+            "decode_only": many["decode_only_events_per_s"], "tracking_only": many["tracking_only_events_per_s"],
+            "one_thread": {"value": one["events_per_s"], "decode_only": one["decode_only_events_per_s"],
+                           "tracking_only": one["tracking_only_events_per_s"], "cores": 1}}
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the CPU oracle on the host cores, same metric / config."""
+    """--impl reference: the CPU oracle, as it stands, on the host cores: same metric, same config, the same
+    events per step as the GPU arm (rank 0 alone runs it)."""
     if rank != 0:
         return
     import synth
     cfg = synth.CONFIGS[args.config]
     cores = os.cpu_count() or 1
-    n = min(args.events or cfg.n_events, 250)        # bounded sample per step
+    n = args.events or cfg.n_events
     geom, batch, params = synth.make_workload(args.config, n_events=n, workers=min(8, cores))
     import oracle
     oracle.build()
-    for _ in range(max(args.warmup, 1)):
-        oracle_chunked(batch, geom, params, 0, min(n, 4 * cores), cores)
-    t = 0.0
+    threads = min(cores, max(n, 1))
+    for _ in range(max(min(args.warmup, 3), 1)):
+        oracle_chunked(batch, geom, params, 0, n, threads)
+    td = tc = t = 0.0
     for _ in range(args.steps):
-        t += oracle_chunked(batch, geom, params, 0, n, cores)
+        d, c, both = oracle_chunked(batch, geom, params, 0, n, threads)
+        td, tc, t = td + d, tc + c, t + both
     value = n * args.steps / t
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "impl": "reference",
-            "config": {"workload": cfg.name, "events_per_step": n, "note": "CPU oracle (oracle/ut_oracle.cpp), "
-                       f"bounded sample of {n} events per step on {cores} host threads"},
+            "config": {"workload": cfg.name, "events_per_step": n, "events_per_gpu": n,
+                       "note": f"CPU oracle (oracle/ut_oracle.cpp) as it stands: all {n} events of the workload per "
+                               f"step over disjoint event chunks on {threads} host threads"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"first {n} events of {cfg.name} per step"},
+                             "sample": f"all {n} events of {cfg.name} per step, {args.steps} steps",
+                             "decode_only": n * args.steps / td, "tracking_only": n * args.steps / tc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -265,6 +319,94 @@ def run_sweep(args, local_rank):
     print(json.dumps(line), flush=True)
 
 
+class DeviceWorkload:
+    """One synthetic batch resident on the device plus everything the two calls need."""
+
+    def __init__(self, B, geom_tables, batch, params):
+        self.B, self.tables, self.batch, self.params = B, geom_tables, batch, params
+        self.geom = B.ut_geometry_upload(geom_tables)
+        self.hits = B.Hits(batch.hit_capacity, batch.n_events, self.geom)
+        self.raw_d, self.bo_d = B.to_device_raw(batch.raw), B.to_device_u32(batch.bank_offsets)
+        self.velo = B.VeloStates(batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z)
+        self.vo_d = B.to_device_u32(batch.velo_offsets)
+        self.tracks = B.Tracks(batch.n_velo_total)
+        self.config = B.make_config(params)
+
+    def decode(self):
+        self.B.ut_decode(self.raw_d, self.bo_d, self.batch.n_events, self.geom, self.hits)
+
+    def compass(self):
+        self.B.compass_track(self.hits, self.hits.hit_offsets, self.velo, self.vo_d, self.batch.n_events, self.config,
+                             self.tracks)
+
+    def step(self):
+        self.decode()
+        self.compass()
+
+    def timed(self, torch, flush, steps, warmup):
+        """CUDA events on the launch stream around each call of each step, L2 flushed between steps.
+        Returns the per-step (decode ms, compass ms, step ms) lists."""
+        stream = torch.cuda.current_stream()
+        for _ in range(warmup):
+            flush.zero_()
+            self.step()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        torch.cuda.synchronize()
+        for k in range(steps):
+            flush.zero_()
+            ev[k][0].record(stream)
+            self.decode()
+            ev[k][1].record(stream)
+            self.compass()
+            ev[k][2].record(stream)
+        torch.cuda.synchronize()
+        return ([e[0].elapsed_time(e[1]) for e in ev], [e[1].elapsed_time(e[2]) for e in ev],
+                [e[0].elapsed_time(e[2]) for e in ev])
+
+    def facts(self):
+        ne, ng = self.batch.n_events, self.tables.n_groups
+        n_hits = int(self.hits.hit_offsets[ne * ng].item()) & 0xFFFFFFFF
+        status = (int(self.hits.status.item()) | int(self.tracks.status.item())) & 0xFFFFFFFF
+        return n_hits, status
+
+
+def kernel_table(batch, abytes, md, mc, hbm_peak):
+    return {
+        "ut_decode_kernel": {"ms": md, "bytes": abytes["decode"], "gbs": abytes["decode"] / md / 1e6,
+                             "frac_hbm": abytes["decode"] / md / 1e6 / hbm_peak,
+                             "events_per_s": batch.n_events / md * 1e3},
+        "compass_kernel": {"ms": mc, "bytes": abytes["compass"], "gbs": abytes["compass"] / mc / 1e6,
+                           "frac_hbm": abytes["compass"] / mc / 1e6 / hbm_peak,
+                           "events_per_s": batch.n_events / mc * 1e3},
+    }
+
+
+def per_config_report(B, torch, flush, prepared, hbm_peak, steps):
+    """north_star: "events/s and achieved fraction of the HBM roofline reported for each [config]".  Device-resident
+    inputs, a few steps each; config 5 in its default setting (min_hits 3, scale 1, C 16) on all 10 000 events."""
+    rows = {}
+    for cid, (cfg, geom_t, batch, params) in prepared.items():
+        w = DeviceWorkload(B, geom_t, batch, params)
+        t_dec, t_cmp, t_step = w.timed(torch, flush, steps, 3)
+        n_hits, status = w.facts()
+        ab = algorithmic_bytes(batch, geom_t, n_hits)
+        md, mc, ms = statistics.mean(t_dec), statistics.mean(t_cmp), statistics.mean(t_step)
+        k = kernel_table(batch, ab, md, mc, hbm_peak)
+        rows[cfg.name] = {
+            "events": batch.n_events, "hits": n_hits, "velo_tracks": batch.n_velo_total, "steps": steps,
+            "events_per_s": batch.n_events / ms * 1e3, "ms_per_step": ms,
+            "decode_only_events_per_s": k["ut_decode_kernel"]["events_per_s"],
+            "tracking_only_events_per_s": k["compass_kernel"]["events_per_s"],
+            "ms_decode": md, "ms_compass": mc,
+            "frac_hbm_decode": k["ut_decode_kernel"]["frac_hbm"], "frac_hbm_compass": k["compass_kernel"]["frac_hbm"],
+            "frac_hbm_step": ab["e2e"] / ms / 1e6 / hbm_peak, "gbs_step": ab["e2e"] / ms / 1e6,
+            "min_hits": params.min_hits, "max_candidates_per_layer": params.max_candidates_per_layer,
+            "status_word": status, "launch": B.last_launch_info()}
+        del w
+        torch.cuda.empty_cache()
+    return rows
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -281,9 +423,16 @@ def main():
     import synth
     cfg = synth.CONFIGS[args.config]
     n_events = args.events or cfg.n_events
+    workers = min(8, os.cpu_count() or 1)
     # generate before CUDA is initialised (the generator may fork workers)
-    geom_t, batch, params = synth.make_workload(args.config, n_events=n_events, workers=min(8, os.cpu_count() or 1),
+    geom_t, batch, params = synth.make_workload(args.config, n_events=n_events, workers=workers,
                                                 first_event=rank * n_events)
+    prepared = {}
+    if world == 1 and not args.no_per_config and args.events is None:
+        for cid in (1, 2, 3, 4, 5):
+            if cid != args.config:
+                g_, b_, p_ = synth.make_workload(cid, workers=workers)
+                prepared[cid] = (synth.CONFIGS[cid], g_, b_, p_)
     import torch
     import torch.distributed as dist
     import __graft_entry__ as entry
@@ -296,26 +445,16 @@ def main():
     from paper_2002_11529_b200 import binding as B
     dev = torch.device("cuda", local_rank)
 
-    geom = B.ut_geometry_upload(geom_t)
-    hits = B.Hits(batch.hit_capacity, batch.n_events, geom)
-    raw_d, bo_d = B.to_device_raw(batch.raw), B.to_device_u32(batch.bank_offsets)
-    velo = B.VeloStates(batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty, batch.velo_z)
-    vo_d = B.to_device_u32(batch.velo_offsets)
-    tracks = B.Tracks(batch.n_velo_total)
-    config = B.make_config(params)
+    w = DeviceWorkload(B, geom_t, batch, params)
+    geom, hits, tracks, vo_d, config = w.geom, w.hits, w.tracks, w.vo_d, w.config
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     stream = torch.cuda.current_stream()
 
-    def step():
-        B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
-        B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
-
-    step()
+    w.step()
     torch.cuda.synchronize()
     launches_per_step = 2
     info = B.last_launch_info()
-    n_hits = int(hits.hit_offsets[batch.n_events * geom.n_groups].item()) & 0xFFFFFFFF
-    status = (int(hits.status.item()) | int(tracks.status.item())) & 0xFFFFFFFF
+    n_hits, status = w.facts()
     abytes = algorithmic_bytes(batch, geom_t, n_hits)
 
     if world > 1:
@@ -346,6 +485,7 @@ def main():
         for _ in range(3):
             run()
         torch.cuda.synchronize()
+        e2e_launches = B.last_launch_info()["kernels_launched"]
         k_e2e = max(10, min(args.steps, 100))
         if world > 1:
             dist.barrier()
@@ -367,7 +507,7 @@ def main():
         e2e = {"value": events_all * k_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": 28 * T + 12, "steps": k_e2e,
                "ms_per_step_mean": 1e3 * t_e2e / k_e2e, "ms_per_step_median": 1e3 * statistics.median(t_steps),
-               "ms_per_step_min": 1e3 * min(t_steps),
+               "ms_per_step_min": 1e3 * min(t_steps), "kernels_per_step": e2e_launches,
                "api": "ut_pipeline_run_host (pinned host buffers in, host track SoA out, sync per step)"}
         ok = np.array_equal(out_h["n_hits"][:T].numpy(), tracks.n_hits[:T].cpu().numpy())
         e2e["matches_device_path"] = bool(ok)
@@ -376,7 +516,7 @@ def main():
     sampler = ClockSampler(local_rank) if rank == 0 and not os.environ.get("BENCH_NO_SAMPLER") else None
     for _ in range(max(args.warmup, 3)):
         flush.zero_()
-        step()
+        w.step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -388,9 +528,9 @@ def main():
     for k in range(args.steps):
         flush.zero_()
         ev[k][0].record(stream)
-        B.ut_decode(raw_d, bo_d, batch.n_events, geom, hits)
+        w.decode()
         ev[k][1].record(stream)
-        B.compass_track(hits, hits.hit_offsets, velo, vo_d, batch.n_events, config, tracks)
+        w.compass()
         ev[k][2].record(stream)
     torch.cuda.synchronize()
     t_wall = time.perf_counter() - t_wall0
@@ -436,31 +576,26 @@ def main():
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "MEASURED_PEAKS.json hbm_gbs (measured copy)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     md, mc, ms = statistics.mean(t_dec), statistics.mean(t_cmp), statistics.mean(t_step)
-    kern = {
-        "ut_decode_kernel": {"ms": md, "bytes": abytes["decode"], "gbs": abytes["decode"] / md / 1e6,
-                             "frac_hbm": abytes["decode"] / md / 1e6 / hbm_peak,
-                             "events_per_s": batch.n_events / md * 1e3},
-        "compass_kernel": {"ms": mc, "bytes": abytes["compass"], "gbs": abytes["compass"] / mc / 1e6,
-                           "frac_hbm": abytes["compass"] / mc / 1e6 / hbm_peak,
-                           "events_per_s": batch.n_events / mc * 1e3},
-    }
+    kern = kernel_table(batch, abytes, md, mc, hbm_peak)
     dom = "ut_decode_kernel" if md >= mc else "compass_kernel"
+    counters, why_not = (ncu_counters(cfg.name) if batch.n_events == cfg.n_events
+                         else (None, "not the workload's full size"))
     roof = {"kernel": dom, "bound": "hbm", "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
             "frac": kern[dom]["frac_hbm"],
-            "traffic": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get(dom) if batch.n_events == cfg.n_events else None,
-            "traffic_source": NCU_DRAM_TRAFFIC.get(cfg.name, {}).get("source"), "peak_source": peak_src,
-            "algorithmic_bytes_per_launch": kern[dom]["bytes"],
-            "issue": None,
+            "traffic": counters.get(dom, {}).get("dram_bytes") if counters else None,
+            "traffic_source": (f"{counters['source']} (commit {counters['commit']})" if counters else why_not),
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": kern[dom]["bytes"], "issue": None,
             "end_to_end": {"bytes": abytes["e2e"], "gbs": abytes["e2e"] / ms / 1e6,
                            "frac": abytes["e2e"] / ms / 1e6 / hbm_peak, "frac_of_8TBs": abytes["e2e"] / ms / 1e6 / 8000.0}}
-    winst = NCU_WARP_INST.get(cfg.name, {}) if batch.n_events == cfg.n_events else {}
-    if winst:
+    if counters:
         issue_peak = 148 * 4 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6          # warp-inst / s
-        roof["issue"] = {k: {"warp_inst_per_launch": winst[k], "achieved_ginst_s": winst[k] / kern[k]["ms"] / 1e6,
-                             "peak_ginst_s": issue_peak / 1e9, "frac": winst[k] / (kern[k]["ms"] * 1e-3) / issue_peak}
-                         for k in kern if k in winst}
+        roof["issue"] = {k: {"warp_inst_per_launch": counters[k]["warp_inst"],
+                             "achieved_ginst_s": counters[k]["warp_inst"] / kern[k]["ms"] / 1e6,
+                             "peak_ginst_s": issue_peak / 1e9,
+                             "frac": counters[k]["warp_inst"] / (kern[k]["ms"] * 1e-3) / issue_peak}
+                         for k in kern if k in counters and "warp_inst" in counters[k]}
         roof["issue"]["note"] = ("context: both kernels are issue / latency bound, not HBM bound; instruction counts from "
-                                 "the committed ncu captures")
+                                 "the committed ncu capture")
     line = {
         "metric": METRIC, "value": events_all * args.steps / (total_ms * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
@@ -473,6 +608,8 @@ def main():
                    "status_word": status, "launch": info},
         "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "e2e": e2e,
         "roofline": roof, "kernels": kern,
+        "decode_only_events_per_s": kern["ut_decode_kernel"]["events_per_s"],
+        "tracking_only_events_per_s": kern["compass_kernel"]["events_per_s"],
         "median_ms": {"decode": statistics.median(t_dec), "compass": statistics.median(t_cmp),
                       "step": statistics.median(t_step), "step_min": min(t_step)},
         "wall_events_per_s_incl_flush": batch.n_events * args.steps / t_wall,
@@ -481,6 +618,10 @@ def main():
                                                "frac_hbm": cons_bytes / t_cons / 1e6 / hbm_peak,
                                                "note": "SURVEY.md 8(f) row 1, timed alone, not part of the step"}},
     }
+    if prepared:
+        del w
+        line["per_config"] = per_config_report(B, torch, flush, prepared, hbm_peak, max(3, min(args.steps, 10)))
+        line["per_config"][cfg.name] = "this line (value, kernels, roofline)"
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(batch, geom_t, params)
     print(json.dumps(line), flush=True)
