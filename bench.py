@@ -305,7 +305,7 @@ def run_sweep(args, local_rank):
                              "ghost_rate": m["ghost_rate"], "charge_ok": m["charge_ok"],
                              "four_hit_fraction": m["four_hit_fraction"], "n_tracklets": m["n_tracklets"],
                              "n_reconstructible": m["n_reconstructible"],
-                             "status_word": (int(hits.status.item()) | int(tracks.status.item())) & 0xFFFFFFFF})
+                             "status_word": (int(hits.status.item()) | int(tracks.status[0].item())) & 0xFFFFFFFF})
     base = next(r for r in rows if (r["min_hits"], r["window_scale"], r["max_candidates_per_layer"]) == (3, 1.0, 16))
     line = {"metric": METRIC, "value": base["events_per_s"], "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": 3,
             "ms_per_step": base["ms_decode"] + base["ms_compass"], "higher_is_better": True, "scaling": "weak",
@@ -366,7 +366,7 @@ class DeviceWorkload:
     def facts(self):
         ne, ng = self.batch.n_events, self.tables.n_groups
         n_hits = int(self.hits.hit_offsets[ne * ng].item()) & 0xFFFFFFFF
-        status = (int(self.hits.status.item()) | int(self.tracks.status.item())) & 0xFFFFFFFF
+        status = (int(self.hits.status.item()) | int(self.tracks.status[0].item())) & 0xFFFFFFFF
         return n_hits, status
 
 

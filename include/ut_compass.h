@@ -105,10 +105,22 @@ typedef struct {
   uint32_t* status;           /* device word, OR-ed with UT_STATUS_* (caller zeroes it) */
   void* workspace;            /* device, ut_decode_workspace_bytes() bytes, zeroed once by
                                  ut_decode_workspace_init(); reusable across calls on one stream.
-                                 compass_track keeps its event ticket here too: calls that share one
-                                 ut_hits must be ordered on one stream.  May be NULL for a container that
-                                 ut_decode did not fill (compass_track then assigns events statically). */
+                                 Only ut_decode uses it: may be NULL for a container filled otherwise. */
+  /* Optional per-sector view of the same hits (the "layer / sector / x-sorted" order of the problem statement;
+   * PAPER.md:288-290 searches sector by sector): every dense sector's hits contiguous, in container order inside
+   * the sector.  All three pointers or none (NULL).  ut_decode fills it in the same launch; compass_track stages
+   * an event's window-search data from it with three bulk copies instead of re-bucketing the group-sorted arrays
+   * (same results either way).  Entry k of sector s of event e sits at hit_offsets[n_groups*e] + sector_offsets
+   * [e][s] + k. */
+  float* x_by_sector;         /* [capacity rounded up to a multiple of 8] x_at_y0 */
+  uint16_t* idx_by_sector;    /* [same] container index of the entry, relative to the event's first hit */
+  uint16_t* sector_offsets;   /* [max_events][ut_sector_offsets_stride(geometry)]: n_sectors + 1 offsets relative to
+                                 the event's first hit, then a word that is UT_SECTOR_INDEX_VALID if the row may be
+                                 used (an event of > 65535 hits, a group larger than the decode's sort buffer or a
+                                 capacity overflow leaves it 0 and compass_track re-buckets that event itself) */
 } ut_hits;
+#define UT_SECTOR_INDEX_VALID 0xA5A5u
+uint32_t ut_sector_offsets_stride(const ut_geometry* geometry);   /* u16 elements per event, a multiple of 8 */
 
 /* Bytes of `workspace` for batches of up to `max_events` events decoded with `geometry` (control words and one
  * look-back word per event; `geometry` may be NULL: the size does not depend on the tables today, the argument
@@ -168,7 +180,9 @@ typedef struct {
   int32_t* n_hits;   /* [n_velo_total] 0 (no tracklet), 3 or 4 */
   float* qop;        /* [n_velo_total] q/p in 1/MeV, sign = charge; 0 if none */
   float* chi2;       /* [n_velo_total] 0 if none */
-  uint32_t* status;  /* device word */
+  uint32_t* status;  /* device u32[4]: [0] status word (OR-ed with UT_STATUS_*, caller zeroes it); [1..3] scratch of
+                        compass_track (its work ticket: zero once, the kernel re-arms it), so that calls with
+                        different outputs may run at the same time on any streams */
 } ut_tracks;
 
 /* compass_track -- PAPER.md section V, fused (window search + tracklet finding in one kernel; the
@@ -232,6 +246,8 @@ typedef struct {
   int32_t decode_raw_stage_bytes;   /* shared-memory staging of one event's raw banks (larger events read global memory) */
   int32_t decode_sort_buf;          /* per-warp sort buffer, in hits (larger groups rank by recomputation) */
   int32_t compass_grid, compass_block, compass_smem_bytes, compass_hit_stage;
+  int32_t compass_split;            /* CTAs sharing the tracks of one event (1, 2 or 4) */
+  int32_t compass_view;             /* 1: the container's per-sector view was offered to the kernel */
 } ut_launch_info;
 void ut_last_launch_info(ut_launch_info* out);
 

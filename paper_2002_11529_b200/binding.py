@@ -42,7 +42,8 @@ class ut_geometry(C.Structure):
 class ut_hits(C.Structure):
     _fields_ = [("x_at_y0", C.c_void_p), ("z_at_y0", C.c_void_p), ("y_begin", C.c_void_p), ("y_end", C.c_void_p),
                 ("dxdy", C.c_void_p), ("weight", C.c_void_p), ("id", C.c_void_p), ("capacity", C.c_uint64),
-                ("geom", C.POINTER(ut_geometry)), ("status", C.c_void_p), ("workspace", C.c_void_p)]
+                ("geom", C.POINTER(ut_geometry)), ("status", C.c_void_p), ("workspace", C.c_void_p),
+                ("x_by_sector", C.c_void_p), ("idx_by_sector", C.c_void_p), ("sector_offsets", C.c_void_p)]
 
 
 class velo_states(C.Structure):
@@ -77,10 +78,12 @@ class ut_tuning(C.Structure):
 class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_raw_stage_bytes",
-                 "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage")]
+                 "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage",
+                 "compass_split", "compass_view")]
 
 
-EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set", "ut_geometry_upload", "ut_geometry_free",
+EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set",
+           "ut_sector_offsets_stride", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
            "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
            "ut_pipeline_device_hits"]
@@ -110,11 +113,13 @@ _lib.ut_pipeline_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_vo
                                       C.POINTER(ut_tracks), C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ut_pipeline_device_hits.argtypes = [C.c_void_p, C.POINTER(ut_hits), C.POINTER(C.c_void_p)]
 _lib.ut_last_launch_info.argtypes = [C.POINTER(ut_launch_info)]
+_lib.ut_sector_offsets_stride.restype = C.c_uint32
+_lib.ut_sector_offsets_stride.argtypes = [C.POINTER(ut_geometry)]
 _lib.ut_tuning_get.argtypes = [C.POINTER(ut_tuning)]
 _lib.ut_tuning_set.argtypes = [C.POINTER(ut_tuning)]
 for _n in EXPORTS:
     if _n not in ("ut_version", "ut_last_error", "ut_decode_workspace_bytes", "ut_last_launch_info",
-                  "compass_consolidate_workspace_bytes"):
+                  "compass_consolidate_workspace_bytes", "ut_sector_offsets_stride"):
         getattr(_lib, _n).restype = C.c_int32
 
 
@@ -175,6 +180,10 @@ def ut_geometry_upload(tables) -> Geometry:
     return Geometry(tables)
 
 
+def ut_sector_offsets_stride(geometry: "Geometry") -> int:
+    return int(_lib.ut_sector_offsets_stride(C.byref(geometry.c)))
+
+
 def ut_decode_workspace_bytes(max_events: int, geometry: "Geometry | None" = None) -> int:
     return int(_lib.ut_decode_workspace_bytes(max_events, C.byref(geometry.c) if geometry is not None else None))
 
@@ -183,7 +192,9 @@ class Hits:
     """Caller-owned SoA hit container on the device (torch tensors) + its ut_hits descriptor."""
     FIELDS = ("x_at_y0", "z_at_y0", "y_begin", "y_end", "dxdy", "weight", "id")
 
-    def __init__(self, capacity: int, max_events: int, geometry: Geometry, device="cuda"):
+    def __init__(self, capacity: int, max_events: int, geometry: Geometry, device="cuda", sector_view: bool = True):
+        """sector_view: also allocate the optional per-sector view (x_by_sector, idx_by_sector, sector_offsets)
+        that ut_decode fills for compass_track."""
         self.capacity = int(capacity)
         n = max(self.capacity, 1)
         self.x_at_y0, self.z_at_y0, self.y_begin, self.y_end, self.dxdy, self.weight = (
@@ -194,9 +205,21 @@ class Hits:
         self.workspace = torch.zeros((nbytes + 15) // 16 * 2, dtype=torch.int64, device=device)   # zeroed once
         self.hit_offsets = torch.zeros(max_events * geometry.n_groups + 1, dtype=torch.int32, device=device)
         self.geometry = geometry
-        self.c = ut_hits(self.x_at_y0.data_ptr(), self.z_at_y0.data_ptr(), self.y_begin.data_ptr(),
-                         self.y_end.data_ptr(), self.dxdy.data_ptr(), self.weight.data_ptr(), self.id.data_ptr(),
-                         self.capacity, C.pointer(geometry.c), self.status.data_ptr(), self.workspace.data_ptr())
+        self.x_by_sector = self.idx_by_sector = self.sector_offsets = None
+        if sector_view:
+            n8 = (n + 7) // 8 * 8
+            self.x_by_sector = torch.empty(n8, dtype=torch.float32, device=device)
+            self.idx_by_sector = torch.empty(n8, dtype=torch.int16, device=device)
+            self.sector_offsets = torch.zeros(max(max_events, 1) * ut_sector_offsets_stride(geometry), dtype=torch.int16,
+                                              device=device)
+        self.c = self.descriptor()
+
+    def descriptor(self) -> "ut_hits":
+        ptr = lambda t: t.data_ptr() if t is not None else None
+        return ut_hits(self.x_at_y0.data_ptr(), self.z_at_y0.data_ptr(), self.y_begin.data_ptr(),
+                       self.y_end.data_ptr(), self.dxdy.data_ptr(), self.weight.data_ptr(), self.id.data_ptr(),
+                       self.capacity, C.pointer(self.geometry.c), self.status.data_ptr(), self.workspace.data_ptr(),
+                       ptr(self.x_by_sector), ptr(self.idx_by_sector), ptr(self.sector_offsets))
 
 
 class Tracks:
@@ -207,7 +230,7 @@ class Tracks:
         self.n_hits = torch.empty(n, dtype=torch.int32, device=device)
         self.qop = torch.empty(n, dtype=torch.float32, device=device)
         self.chi2 = torch.empty(n, dtype=torch.float32, device=device)
-        self.status = torch.zeros(1, dtype=torch.int32, device=device)
+        self.status = torch.zeros(4, dtype=torch.int32, device=device)     # [0] status word, [1..3] kernel scratch
         self.c = ut_tracks(self.hit_idx.data_ptr(), self.n_hits.data_ptr(), self.qop.data_ptr(),
                            self.chi2.data_ptr(), self.status.data_ptr())
 

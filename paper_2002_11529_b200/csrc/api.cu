@@ -242,6 +242,10 @@ int32_t ut_geometry_free(ut_geometry* g) {
   return UT_OK;
 }
 
+uint32_t ut_sector_offsets_stride(const ut_geometry* geometry) {
+  return geometry ? (geometry->n_sectors + 2u + 7u) & ~7u : 0u;
+}
+
 size_t ut_decode_workspace_bytes(int32_t max_events, const ut_geometry* /*geometry*/) {
   return 32 + 8 * (size_t)(max_events > 0 ? max_events : 0) + 8;   // 8 control words, then one look-back word per event
 }
@@ -268,6 +272,10 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
   if ((reinterpret_cast<uintptr_t>(raw_banks) & 15u) || (reinterpret_cast<uintptr_t>(bank_offsets) & 15u) ||
       (reinterpret_cast<uintptr_t>(hits_out->workspace) & 15u))
     return UT_ERR_ARG;
+  {                                   // the per-sector view: all three arrays or none
+    const int have = (hits_out->x_by_sector != nullptr) + (hits_out->idx_by_sector != nullptr) + (hits_out->sector_offsets != nullptr);
+    if (have != 0 && have != 3) return UT_ERR_ARG;
+  }
   hits_out->geom = geometry;
   if (n_events == 0)      // the offsets array still has its single entry
     return cudaMemsetAsync(hit_offsets_out, 0, 4, (cudaStream_t)stream) == cudaSuccess ? UT_OK : UT_ERR_CUDA;
@@ -361,9 +369,10 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
   const size_t s_raw = up(max_raw_bytes + 16), s_bo = up(((size_t)max_events * g->n_sectors + 1) * 4),
                s_ho = up(((size_t)max_events * g->n_groups + 1) * 4), s_vo = up(((size_t)max_events + 1) * 4),
-               s_st = 256, s_v = up((size_t)max_velo * 4), s_h = up((size_t)max_hits * 4),
-               s_ws = up(ut_decode_workspace_bytes(max_events, g)), s_ti = up((size_t)max_velo * 16);
-  const size_t total = s_raw + s_bo + s_ho + s_vo + s_st + 4 * s_v + 7 * s_h + s_ws + s_ti + 3 * s_v;
+               s_st = 256, s_v = up((size_t)max_velo * 4), s_h = up((size_t)max_hits * 4 + 32),
+               s_ws = up(ut_decode_workspace_bytes(max_events, g)), s_ti = up((size_t)max_velo * 16),
+               s_so = up((size_t)max_events * ut_sector_offsets_stride(g) * 2);
+  const size_t total = s_raw + s_bo + s_ho + s_vo + s_st + 4 * s_v + 9 * s_h + s_ws + s_ti + 3 * s_v + s_so;
   if (cudaMalloc(&p->block, total) != cudaSuccess) { delete p; return UT_ERR_CUDA; }
   unsigned char* q = p->block;
   auto take = [&](size_t n) { unsigned char* r = q; q += n; return r; };
@@ -376,9 +385,11 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   p->hits.id = (uint32_t*)take(s_h);
   p->hits.capacity = max_hits; p->hits.geom = &p->geom; p->hits.status = p->status;
   p->hits.workspace = take(s_ws);
+  p->hits.x_by_sector = (float*)take(s_h); p->hits.idx_by_sector = (uint16_t*)take(s_h);   // (half of the slot used)
+  p->hits.sector_offsets = (uint16_t*)take(s_so);
   p->tracks.hit_idx = (int32_t*)take(s_ti);
   p->tracks.n_hits = (int32_t*)take(s_v); p->tracks.qop = (float*)take(s_v); p->tracks.chi2 = (float*)take(s_v);
-  p->tracks.status = p->status + 1;
+  p->tracks.status = p->status + 4;                    // 4 words: status + the kernel's work ticket
   if (cudaMemset(p->block, 0, total) != cudaSuccess) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
   bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess &&
@@ -421,13 +432,14 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 500);
   int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
-  bool ok = cudaMemsetAsync(p->status, 0, 8, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
+  bool ok = cudaMemsetAsync(p->status, 0, 32, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_out, p->ev_start, 0) == cudaSuccess;
   if (!ok) return UT_ERR_CUDA;
   if (n_events == 0) {
     ok = cudaMemsetAsync(p->hit_offsets, 0, 4, s) == cudaSuccess;
-    if (status_h) ok = ok && cudaMemcpyAsync(status_h, p->status, 8, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (status_h) ok = ok && cudaMemcpyAsync(status_h, p->status, 4, cudaMemcpyDeviceToHost, s) == cudaSuccess &&
+                     cudaMemcpyAsync(status_h + 1, p->status + 4, 4, cudaMemcpyDeviceToHost, s) == cudaSuccess;
     if (n_hits_h) ok = ok && cudaMemcpyAsync(n_hits_h, p->hit_offsets, 4, cudaMemcpyDeviceToHost, s) == cudaSuccess;
     return ok ? UT_OK : UT_ERR_CUDA;
   }
@@ -459,11 +471,13 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     // upper bound of this chunk's hits from its raw size alone (sizes the on-chip staging like a whole call)
     const size_t hdr = 6 * (size_t)ne * ns;
     const unsigned long long hint = r1 - r0 > hdr ? (r1 - r0 - hdr) / 2 : 1;
-    int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &p->hits, ho, s, k == 0 ? nullptr : ho, hint);
+    ut_hits hc = p->hits;                              // this chunk's rows of the per-sector view
+    hc.sector_offsets = p->hits.sector_offsets + (size_t)e0 * ut_sector_offsets_stride(g);
+    int32_t rc = launch_decode(p->raw, p->bank_offsets + (size_t)e0 * ns, ne, g, &hc, ho, s, k == 0 ? nullptr : ho, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
     if (cudaStreamWaitEvent(s, p->ev_velo[k], 0) != cudaSuccess) return UT_ERR_CUDA;
-    rc = launch_compass(&p->hits, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo, hint);
+    rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, s, n_velo, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
     ok = cudaEventRecord(p->ev_done[k], s) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess;
@@ -475,7 +489,7 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     if (!ok) return UT_ERR_CUDA;
   }
   launch_info().kernels_launched = launched;
-  if (status_h) ok = ok && d2h(status_h, p->status, 8);
+  if (status_h) ok = ok && d2h(status_h, p->status, 4) && d2h(status_h + 1, p->status + 4, 4);
   if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * ng, 4);
   ok = ok && cudaEventRecord(p->ev_out, p->s_out) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_out, 0) == cudaSuccess;
   return ok ? UT_OK : UT_ERR_CUDA;

@@ -3,33 +3,43 @@
 // The paper runs two kernels: "search UT windows" (2-D: 4 panels x tracks) writes
 // (first hit, size) ranges to global memory, then "tracklet finding" (thread per track)
 // reads them back through a shared-memory cache.  That shape leaves a B200 warp at
-// 7 of 32 lanes (profiles/r1a_first_path.md).  Here one CTA takes one event (atomic ticket) and keeps it on chip:
+// 7 of 32 lanes (profiles/r1a_first_path.md).  Here a CTA takes one work item = (event, part k of K) by an
+// atomic ticket and keeps the event on chip (K = 1, 2 or 4 CTAs share the tracks of an event: track i belongs
+// to part i mod K; K > 1 only for batches of fewer events than resident CTAs):
 //
-//   stage    the event's id and x ranges arrive by two TMA bulk copies into scratch that aliases the warp areas;
-//            a warp per sector group re-buckets them PER SECTOR into shared memory (x and the hit index only;
-//            one pass: match.any ranks, per-sector counts, warp scan).  A sector's y range, stereo slope, z and
-//            weight are rows of the geometry table, so the y test of the window search becomes a per-sector
-//            test: the scan touches the hits of the one sector row the track crosses instead of all 14 rows.
-//   order    the tracks of the event are ranked by their radius at the first layer (counting rank in shared memory):
-//            a batch costs what its heaviest track costs and the inner tracks cross the busy sectors, so like goes
-//            with like and the heavy batches start first.  Results do not depend on the order.
+//   stage    the event's window-search data is its per-sector view: x and the container index bucketed per
+//            dense sector plus the sector offsets.  When ut_decode wrote the view (ut_hits.x_by_sector ...) it
+//            arrives by three TMA bulk copies and no thread touches it; otherwise a warp per sector group
+//            re-buckets the group-sorted arrays in shared memory (match.any ranks, per-sector counts, warp
+//            scan).  A sector's y range, stereo slope, z and weight are rows of the geometry table, so the y
+//            test of the window search is a per-sector test: the scan touches the hits of the one sector row
+//            the track crosses instead of all rows of the column.
+//   order    the tracks of the item are binned by their radius at the first layer (counting sort over
+//            logarithmic bins, O(n)): a batch costs what its heaviest track costs and the inner tracks cross
+//            the busy sectors, so like goes with like and the heavy batches start first.  Results do not
+//            depend on the order.
 //   phase 1  lane = (track, layer), 8 tracks per warp (the paper's 2-D window kernel shape):
 //            straight-line extrapolation, column groups and sector row from a linear guess corrected against
 //            the tables (y ranges from L1), lower-bound search in busy sectors, |d| <= win test with early exit;
 //            accepted hits go to the (track, layer) candidate list in shared memory, kept sorted by hit index
-//            and capped to the `max_candidates_per_layer` closest in |d|.
+//            and capped to the `max_candidates_per_layer` closest in |d| (a run longer than the cap starts at
+//            the zero crossing minus the cap and ends at the first hit the full list rejects).
 //   phase 2  the nested loops of the tracklet search are spread over the 32 lanes of the warp:
-//            (a) seed rows (track, hit a) of the 8 tracks, one row per lane walking the partner hits b: slope +
-//                kink cuts; survivors are compacted (ballot) into a per-warp seed queue;
-//            (b) the queued seeds, 4 lanes per seed: compatible hits in the other two layers as 32-bit masks,
-//                giving the number of 3/4-hit combinations of the seed;
+//            (a) seed rows (track, hit a) of the 8 tracks, one row per lane walking the partner hits b with a
+//                cheap conservative filter of the slope + kink cuts (reciprocal instead of the division, a
+//                margin of 2e-6 relative: it never drops a pair the exact cuts keep); survivors are compacted
+//                (ballot) into a per-warp seed queue;
+//            (b) the queued seeds, 4 lanes per seed: the exact slope and kink cuts in the order of DESIGN.md
+//                section 3, then the compatible hits in the other two layers as 32-bit masks, giving the
+//                number of 3/4-hit combinations of the seed;
 //            (c) all combinations of those seeds, one fit per lane (linear chi2 fit with the VELO pseudo-point),
 //                packed (n, chi2, positions) key, atomicMin into the track's best key.
 //            Forward seeds first, backward only for tracks where forward found nothing valid (A11), or both
 //            directions for every track (compass_config.both_directions).
+//            When every candidate list of the batch has one z and one weight (always in a layer-uniform
+//            geometry) those come from two per-slot words instead of a table look-up per candidate.
 //   Candidate lists, queues and best keys never leave the SM; the phases of a warp are separated by
-//   __syncwarp only, and the 7 warps of a CTA pull 8-track batches from a shared-memory ticket (an event of up
-//   to 168 tracks is three rounds; the step at 1000 events is set by this latency, profiles/r1d_final_round1.md).
+//   __syncwarp only, and the warps of a CTA pull 8-track batches from a shared-memory ticket.
 //
 // Events that do not fit the staging buffer take the same phases with a group-level binary search on the
 // global x-sorted arrays (the plain definition of the window, per-hit y test).
@@ -45,12 +55,18 @@ constexpr float kGroupEps = 0.01f;     // slack of the group pre-selection [mm] 
 constexpr unsigned long long kNoKey = ~0ull;
 constexpr int kTPW = 8;                // tracks per warp batch (x 4 layers = 32 lanes)
 constexpr int kSeedQ = 64;             // per-warp seed ring (<= 31 left over + <= 32 new)
+constexpr int kBins = 128;             // radius bins of the batch order
+constexpr float kFilterEps = 2e-6f;    // relative margin of the seed pre-filter (>= 16 roundings of 6e-8)
 
 struct CompassArgs {
   const float* hx;
   const uint32_t* hid;
   const float *hyb, *hye;              // per-hit y range: only the global (unstaged) path reads them
   const uint32_t* hit_offsets;
+  const float* sx;                     // per-sector view written by ut_decode (or null)
+  const uint16_t* si;
+  const uint16_t* soff;
+  uint32_t soff_stride;
   const float *vx, *vy, *vtx, *vty;
   float vz;
   const uint32_t* velo_offsets;
@@ -62,13 +78,14 @@ struct CompassArgs {
   compass_config c;
   int32_t *out_idx, *out_n;
   float *out_qop, *out_chi2;
-  uint32_t* status;
+  uint32_t* status;                    // [0] status word, [1] next work item, [2] CTAs done
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
-  uint32_t trk_stage;                  // tracks of an event that can be ordered by radius (0: never)
+  uint32_t trk_stage;                  // tracks of an item that can be ordered by radius (0: never)
   unsigned long long capacity;         // elements of the hit arrays (bulk copies never read past it)
   uint32_t bulk_ok;                    // hit arrays are 16-byte aligned: the event's x and id ranges come by TMA
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
-  uint32_t* ticket;                    // [0] next event, [1] CTAs done (in the hit container's workspace) or null
+  uint32_t split;                      // K: CTAs sharing the tracks of one event
+  float slope_lim;                     // max_slope * (1 + kFilterEps): pre-filter limit
 };
 
 struct FitResult { float chi2, b; bool valid; };
@@ -122,94 +139,102 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, uint32
          (unsigned long long)((p0 << 18) | (p1 << 12) | (p2 << 6) | p3);
 }
 
+__device__ __forceinline__ float rcp_approx(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
 // Per-warp working set in shared memory.  Candidate i of lane-slot s (= track-in-batch * 4 + layer) lives at
-// [i * 32 + s]: the 32 lanes of phase 1 append without bank conflicts.
+// [s * CS + i] with CS odd: the rows (track, hit) and the 4 lanes of a seed in phase 2 read consecutive banks.
 struct WarpArea {
-  float* cd;                   // [C * 32] residual d of the candidate
-  uint32_t* chs;               // [C * 32] (hit index relative to the event) << 16 | dense sector
-  uint2* seedq;                // [kSeedQ] (track << 10 | ia << 5 | ib, seed slope bits)
+  float* cd;                   // [32 * CS] residual d of the candidate
+  uint32_t* chs;               // [32 * CS] (hit index relative to the event) << 16 | dense sector
+  uint32_t* seedq;             // [kSeedQ] track << 10 | ia << 5 | ib
   unsigned long long* best;    // [kTPW]
   int* n;                      // [32] candidates per slot
+  float* zs;                   // [32] z of the slot's candidates when they all share one
+  float* ws;                   // [32] weight, likewise
+  int CS;
 };
 
+__host__ __device__ inline int cand_stride(int C) { return C | 1; }
 __host__ __device__ inline size_t warp_area_bytes(int C) {
-  return (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8 + 32 * 4;
+  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 3;
 }
 
 // Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
-__device__ __forceinline__ void cand_insert(const WarpArea& wa, int slot, int& n, int C, float d, uint32_t hs) {
+// Returns false when the list is full and the new hit is not closer than its worst entry.
+__device__ __forceinline__ bool cand_insert(const WarpArea& wa, int slot, int& n, int C, float d, uint32_t hs) {
+  float* cd = wa.cd + slot * wa.CS;
+  uint32_t* chs = wa.chs + slot * wa.CS;
   if (n == C) {
     int worst = 0;
-    float wabs = fabsf(wa.cd[slot]);
-    uint32_t whs = wa.chs[slot];
+    float wabs = fabsf(cd[0]);
+    uint32_t whs = chs[0];
     for (int i = 1; i < C; ++i) {
-      const float v = fabsf(wa.cd[i * 32 + slot]);
-      const uint32_t k = wa.chs[i * 32 + slot];
+      const float v = fabsf(cd[i]);
+      const uint32_t k = chs[i];
       if (v > wabs || (v == wabs && k > whs)) { wabs = v; whs = k; worst = i; }
     }
     const float nabs = fabsf(d);
-    if (!(nabs < wabs || (nabs == wabs && hs < whs))) return;
-    for (int i = worst; i < C - 1; ++i) {
-      wa.cd[i * 32 + slot] = wa.cd[(i + 1) * 32 + slot];
-      wa.chs[i * 32 + slot] = wa.chs[(i + 1) * 32 + slot];
-    }
+    if (!(nabs < wabs || (nabs == wabs && hs < whs))) return false;
+    for (int i = worst; i < C - 1; ++i) { cd[i] = cd[i + 1]; chs[i] = chs[i + 1]; }
     n = C - 1;
   }
   int i = n;
   while (i > 0) {
-    const uint32_t k = wa.chs[(i - 1) * 32 + slot];
+    const uint32_t k = chs[i - 1];
     if (k < hs) break;
-    wa.chs[i * 32 + slot] = k;
-    wa.cd[i * 32 + slot] = wa.cd[(i - 1) * 32 + slot];
+    chs[i] = k;
+    cd[i] = cd[i - 1];
     --i;
   }
-  wa.cd[i * 32 + slot] = d;
-  wa.chs[i * 32 + slot] = hs;
+  cd[i] = d;
+  chs[i] = hs;
   ++n;
+  return true;
 }
 
 // Shared-memory view of one CTA: geometry tables (staged once per CTA) and the current event's hits.
 struct SmemView {
   const float4* gA;      // [ng]  group: xmin, xmax, dxdy, row-hint base (y_hi of the first sector)
   const uint2* gB;       // [ng]  group: row-hint scale (float bits), first sector | end sector << 16
-  const float2* yr;      // [ns]  sector: y_begin - y_tol, y_end + y_tol
   const float2* lay;     // [4]   layer: group-hint base (xmax of the first group), scale
   const uint32_t* goff;  // [ng + 1] group offsets relative to the event's first hit
   const uint16_t* off;   // [ns + 1] bucketed position of every sector's first hit
-  const float* hx;       // [hit_stage] x_at_y0, bucketed per sector, x-sorted inside the sector
-  const uint16_t* hh;    // [hit_stage] hit index relative to the event
+  const float* hx;       // x_at_y0, bucketed per sector, x-sorted inside the sector (indexed by `off` positions)
+  const uint16_t* hh;    // hit index relative to the event
 };
+
+// y range of a sector widened by y_tol (same two roundings wherever it is evaluated)
+__device__ __forceinline__ float yr_hi(const CompassArgs& a, int s) {
+  return __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol);
+}
+__device__ __forceinline__ float2 yr_of(const CompassArgs& a, int s) {
+  return make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
+}
+
+// z / weight of the slot's candidates: remembered while they all agree (zu = NaN once they do not)
+__device__ __forceinline__ void note_zw(const CompassArgs& a, int s, bool first, float& zu, float& wu) {
+  const float z = __ldg(a.sec_z + s), w = __ldg(a.sec_w + s);
+  if (first) { zu = z; wu = w; }
+  else if (!(z == zu && w == wu)) zu = __int_as_float(0x7FC00000);
+}
 
 // ---- phase 1: candidate list of one (track, layer) -------------------------------------
 // Group and sector row are found from a linear guess corrected against the tables (exact lower bound of
 // the same predicates the oracle's search uses; O(1) on a regular layout, any sorted layout works).
-#ifndef UT_COMPASS_YR_SMEM
-#define UT_COMPASS_YR_SMEM 0           // 1: the 7 KB table of toleranced y ranges lives in shared memory
-#endif
-// y range of a sector widened by y_tol (same two roundings wherever it is evaluated)
-__device__ __forceinline__ float yr_hi(const CompassArgs& a, const SmemView& S, int s) {
-#if UT_COMPASS_YR_SMEM
-  return S.yr[s].y;
-#else
-  return __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol);
-#endif
-}
-__device__ __forceinline__ float2 yr_of(const CompassArgs& a, const SmemView& S, int s) {
-#if UT_COMPASS_YR_SMEM
-  return S.yr[s];
-#else
-  return make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
-#endif
-}
-
 template <bool BUCKETED>
 __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
-                                              int l, float x_e, float y_e, uint32_t h0) {
+                                              int l, float x_e, float y_e, uint32_t h0, float& zu, float& wu) {
   const int C = a.c.max_candidates_per_layer;
   const float D = a.c.win_half[l], negD = -D;
   const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
   const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
   const int g0 = l * (int)a.gpl, g1 = g0 + (int)a.gpl;
+  float* cd = wa.cd + slot * wa.CS;
+  uint32_t* chs = wa.chs + slot * wa.CS;
   int g;
   {                                                 // first group with group_xmax >= lo
     const float2 hint = S.lay[l];
@@ -233,11 +258,11 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
       if (a.rows_sorted) {                          // first sector row with y_e <= y_end + y_tol
         const int guess = (int)ceilf((y_e - grp.w) * __uint_as_float(gi.x));
         s = sa + max(0, min(guess, sb - sa - 1));
-        while (s > sa && y_e <= yr_hi(a, S, s - 1)) --s;
-        while (s < sb && !(y_e <= yr_hi(a, S, s))) ++s;
+        while (s > sa && y_e <= yr_hi(a, s - 1)) --s;
+        while (s < sb && !(y_e <= yr_hi(a, s))) ++s;
       }
       for (; s < sb; ++s) {
-        const float2 yr = yr_of(a, S, s);
+        const float2 yr = yr_of(a, s);
         if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
         if (!(y_e <= yr.y)) continue;
         const uint32_t p1 = S.off[s + 1];
@@ -247,24 +272,44 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
             const uint32_t half = cnt >> 1, mid = p + half;
             if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= negD) cnt = half; else { p = mid + 1; cnt -= half + 1; }
           }
+          if (p1 - p > (uint32_t)C) {
+            // a run that can overflow the cap: of the hits on the negative side only the C next to the zero
+            // crossing can be among the C closest (each one further out has C closer hits of this very run in
+            // front of it), so the scan starts there instead of evicting its way through the run
+            uint32_t zc = p;
+            for (uint32_t cnt = p1 - p; cnt > 0;) {
+              const uint32_t half = cnt >> 1, mid = zc + half;
+              if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= 0.f) cnt = half; else { zc = mid + 1; cnt -= half + 1; }
+            }
+            if (zc - p > (uint32_t)C) {
+              uint32_t q = zc - (uint32_t)C;
+              while (q > p && S.hx[q - 1] == S.hx[q]) --q;     // equal x: equal |d|, the lower index wins the tie
+              p = q;
+            }
+          }
         }
+        const int n_before = n;
+        bool took_any = false;
         for (; p < p1; ++p) {
           const float d = __fsub_rn(__fadd_rn(S.hx[p], syg), x_e);
           if (d > D) break;                         // x-sorted inside the sector: d only grows
           const bool acc = d >= negD;
           const uint32_t hs = ((uint32_t)S.hh[p] << 16) | (uint32_t)s;
           if (acc && (n >= C || (n > 0 && hs <= last))) {   // rare: cap reached or out of hit order
-            cand_insert(wa, slot, n, C, d, hs);
-            last = wa.chs[(n - 1) * 32 + slot];
+            const bool took = cand_insert(wa, slot, n, C, d, hs);
+            took_any |= took;
+            last = chs[n - 1];
+            if (!took && d >= 0.f) break;           // full list, positive side: every later hit is further still
             continue;
           }
           if (acc) {                                // hits arrive in ascending index almost always: append
-            wa.cd[n * 32 + slot] = d;
-            wa.chs[n * 32 + slot] = hs;
+            cd[n] = d;
+            chs[n] = hs;
             last = hs;
             ++n;
           }
         }
+        if (n != n_before || took_any) note_zw(a, s, n_before == 0, zu, wu);
       }
     } else {
       const float* X = a.hx + h0;
@@ -282,53 +327,78 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t rid = __ldg(a.hid + h0 + h) >> 9;
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;             // reported by the staging pass of the bucketed path only
-        cand_insert(wa, slot, n, C, d, (h << 16) | s);
+        const bool first_cand = n == 0;
+        if (cand_insert(wa, slot, n, C, d, (h << 16) | s)) note_zw(a, (int)s, first_cand, zu, wu);
       }
     }
   }
   return n;
 }
 
+// z of candidate `i` of `slot`
+template <bool UNI>
+__device__ __forceinline__ float cand_z(const CompassArgs& a, const WarpArea& wa, int slot, int i) {
+  return UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * wa.CS + i] & 0xFFFFu));
+}
+
 // ---- phase 2 (b) + (c): `cnt` queued seeds, one per lane, then all their 3/4-hit combinations --------------
+template <bool UNI>
 __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpArea& wa, int lane, int cnt, int qhead,
                                               int dir) {
-  const int LA = dir ? 3 : 0, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
+  const int LA = dir ? 3 : 0, LB = dir ? 1 : 2, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
+  const int CS = wa.CS;
   const bool min3 = a.c.min_hits == 3;
-  // (b) compatible hits of every seed as bit masks: 4 lanes share one seed (8 seeds per round), each lane
-  //     tests every 4th hit of the two other layers; the masks end up in lane = seed index
+  // (b) 4 lanes share one seed (8 seeds per round): the exact cuts of step 5, then every 4th hit of the two
+  //     other layers per lane; the masks of compatible hits end up in lane = seed index
   uint32_t pk = 0, mC = 0, mD = 0, k = 0;
-  if (lane < cnt) pk = wa.seedq[(qhead + lane) & (kSeedQ - 1)].x;
+  bool alive = false;                                // the seed of this lane passed the exact cuts
+  if (lane < cnt) pk = wa.seedq[(qhead + lane) & (kSeedQ - 1)];
   const int sub = lane & 3;
   for (int r0 = 0; r0 < cnt; r0 += 8) {
     const int q = r0 + (lane >> 2);
     uint32_t pC = 0, pD = 0;
+    bool ok = false;
     if (q < cnt) {
-      const uint2 sd = wa.seedq[(qhead + q) & (kSeedQ - 1)];
-      const float bs = __uint_as_float(sd.y);
-      const int j4 = (int)(sd.x >> 10) * 4, ia = (sd.x >> 5) & 31;
-      const float da = wa.cd[ia * 32 + j4 + LA];
-      const float za = __ldg(a.sec_z + (wa.chs[ia * 32 + j4 + LA] & 0xFFFFu));
-      const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
-      for (int i = sub; i < nC; i += 4) {
-        const float dc = wa.cd[i * 32 + j4 + LC];
-        const float zc = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LC] & 0xFFFFu));
-        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
-        if (fabsf(__fsub_rn(dc, pred)) <= a.c.seed_tol) pC |= 1u << i;
-      }
-      for (int i = sub; i < nD; i += 4) {
-        const float dd = wa.cd[i * 32 + j4 + LD];
-        const float zd = __ldg(a.sec_z + (wa.chs[i * 32 + j4 + LD] & 0xFFFFu));
-        const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
-        if (fabsf(__fsub_rn(dd, pred)) <= a.c.seed_tol) pD |= 1u << i;
+      const uint32_t sd = wa.seedq[(qhead + q) & (kSeedQ - 1)];
+      const int j4 = (int)(sd >> 10) * 4, ia = (sd >> 5) & 31, ib = sd & 31;
+      const float da = wa.cd[(j4 + LA) * CS + ia], db = wa.cd[(j4 + LB) * CS + ib];
+      const float za = cand_z<UNI>(a, wa, j4 + LA, ia), zb = cand_z<UNI>(a, wa, j4 + LB, ib);
+      const float bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
+      const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, a.c.z_mag)));
+      ok = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
+      if (ok) {
+        const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
+        const float* cC = wa.cd + (j4 + LC) * CS;
+        const float* cDl = wa.cd + (j4 + LD) * CS;
+        if (UNI) {
+          const float predC = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(wa.zs[j4 + LC], za)));
+          const float predD = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(wa.zs[j4 + LD], za)));
+          for (int i = sub; i < nC; i += 4)
+            if (fabsf(__fsub_rn(cC[i], predC)) <= a.c.seed_tol) pC |= 1u << i;
+          for (int i = sub; i < nD; i += 4)
+            if (fabsf(__fsub_rn(cDl[i], predD)) <= a.c.seed_tol) pD |= 1u << i;
+        } else {
+          for (int i = sub; i < nC; i += 4) {
+            const float zc = cand_z<false>(a, wa, j4 + LC, i);
+            const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
+            if (fabsf(__fsub_rn(cC[i], pred)) <= a.c.seed_tol) pC |= 1u << i;
+          }
+          for (int i = sub; i < nD; i += 4) {
+            const float zd = cand_z<false>(a, wa, j4 + LD, i);
+            const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
+            if (fabsf(__fsub_rn(cDl[i], pred)) <= a.c.seed_tol) pD |= 1u << i;
+          }
+        }
       }
     }
     pC |= __shfl_xor_sync(0xFFFFFFFFu, pC, 1); pC |= __shfl_xor_sync(0xFFFFFFFFu, pC, 2);
     pD |= __shfl_xor_sync(0xFFFFFFFFu, pD, 1); pD |= __shfl_xor_sync(0xFFFFFFFFu, pD, 2);
     const int src = ((lane - r0) & 7) * 4;               // lanes r0 .. r0+7 pick up the masks of their seed
     const uint32_t gC = __shfl_sync(0xFFFFFFFFu, pC, src), gD = __shfl_sync(0xFFFFFFFFu, pD, src);
-    if (lane >= r0 && lane < r0 + 8) { mC = gC; mD = gD; }
+    const bool gok = __shfl_sync(0xFFFFFFFFu, ok ? 1 : 0, src) != 0;
+    if (lane >= r0 && lane < r0 + 8) { mC = gC; mD = gD; alive = gok; }
   }
-  if (lane < cnt) {
+  if (lane < cnt && alive) {
     const uint32_t pc = __popc(mC), pd = __popc(mD);
     k = min3 ? (pc + 1) * (pd + 1) - 1 : pc * pd;   // (c or none) x (d or none) with >= min_hits hits in total
   }
@@ -365,10 +435,14 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
         pr[l] = pos[l] >= 0;
         d[l] = z[l] = w[l] = 0.f;
         if (pr[l]) {
-          const uint32_t s = wa.chs[pos[l] * 32 + j * 4 + l] & 0xFFFFu;
-          d[l] = wa.cd[pos[l] * 32 + j * 4 + l];
-          z[l] = __ldg(a.sec_z + s);
-          w[l] = __ldg(a.sec_w + s);
+          const int slot = j * 4 + l;
+          d[l] = wa.cd[slot * CS + pos[l]];
+          if (UNI) { z[l] = wa.zs[slot]; w[l] = wa.ws[slot]; }
+          else {
+            const uint32_t s = wa.chs[slot * CS + pos[l]] & 0xFFFFu;
+            z[l] = __ldg(a.sec_z + s);
+            w[l] = __ldg(a.sec_w + s);
+          }
           ++nh;
         }
       }
@@ -378,97 +452,113 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
                                         (uint32_t)pos[2] & 63u, (uint32_t)pos[3] & 63u));
     }
   }
-  (void)LA;
 }
 
+// ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
+template <bool UNI>
+__device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
+  const int j = lane & 7;
+  const int CS = wa.CS;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  for (int dir = 0; dir < 2 && todo; ++dir) {     // forward seeds (L0, L2), then backward (L3, L1)
+    const int LA = dir ? 3 : 0, LB = dir ? 1 : 2;
+    const uint32_t nA = wa.n[4 * j + LA], nB = wa.n[4 * j + LB];
+    // rows (track, hit a) of the batch, one per lane; the lane walks the partner hits b of its row
+    const uint32_t P = (lane < kTPW && ((todo >> j) & 1u) && nB > 0u) ? nA : 0u;
+    const uint32_t incl = warp_incl_scan(P, lane), excl = incl - P;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    int qn = 0, qhead = 0;
+    for (uint32_t base = 0; base < total; base += 32) {
+      const uint32_t i = base + lane;
+      int jj = 0;                               // owner track: largest jj < 8 with excl[jj] <= i
+#pragma unroll
+      for (int step = 4; step > 0; step >>= 1) {
+        const uint32_t e = __shfl_sync(0xFFFFFFFFu, excl, jj + step);
+        if (e <= i) jj += step;
+      }
+      const uint32_t ia = i - __shfl_sync(0xFFFFFFFFu, excl, jj);
+      int nBj = (int)__shfl_sync(0xFFFFFFFFu, nB, jj);
+      const int sA = jj * 4 + LA, sB = jj * 4 + LB;
+      const float* cB = wa.cd + sB * CS;
+      float da = 0.f, za = 0.f, zam = 0.f, rinv = 0.f, lim0 = 0.f;
+      if (i < total) {
+        da = wa.cd[sA * CS + ia];
+        za = cand_z<UNI>(a, wa, sA, (int)ia);
+        zam = za - a.c.z_mag;
+        if (UNI) rinv = rcp_approx(wa.zs[sB] - za);
+        lim0 = a.c.kink_tol + kFilterEps * (a.c.kink_tol + fabsf(da));
+      } else {
+        nBj = 0;
+      }
+      const int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+      for (int ib = 0; ib < maxB; ++ib) {
+        // conservative filter: bs and a0 through a reciprocal, accepted with a relative margin that covers the
+        // roundings of both evaluations; the exact cuts follow in process_seeds
+        bool pass = false;
+        if (ib < nBj) {
+          if (!UNI) rinv = rcp_approx(cand_z<false>(a, wa, sB, ib) - za);
+          const float bsa = (cB[ib] - da) * rinv;
+          const float t = bsa * zam;
+          pass = fabsf(bsa) <= a.slope_lim && fabsf(da - t) <= __fmaf_rn(kFilterEps, fabsf(t), lim0);
+        }
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
+        if (m == 0u) continue;
+        if (pass)
+          wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] = ((uint32_t)jj << 10) | (ia << 5) | (uint32_t)ib;
+        qn += __popc(m);
+        __syncwarp();
+        if (qn >= 32) {
+          process_seeds<UNI>(a, wa, lane, 32, qhead, dir);
+          qhead += 32;
+          qn -= 32;
+          __syncwarp();
+        }
+      }
+    }
+    if (qn > 0) process_seeds<UNI>(a, wa, lane, qn, qhead, dir);
+    __syncwarp();
+    if (!a.c.both_directions)                   // backward only if nothing valid (A11); else best of both
+      todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);
+  }
+}
+
+// The warps of the CTA pull 8-track batches of the item: track m of the item is VELO track t0 + m * K + part.
 template <bool BUCKETED>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
-                                           uint32_t h0, uint32_t t0, uint32_t t1, uint32_t T, const uint16_t* perm) {
+                                           uint32_t h0, uint32_t t0, uint32_t nTk, uint32_t part, uint32_t T,
+                                           const uint16_t* perm) {
   const int lane = threadIdx.x & 31;
   const int l = lane & 3;                         // layer of this lane in phase 1 and in the output
   const int j = lane & 7;                         // track-in-batch this lane does the bookkeeping for (lanes 0..7)
-  const uint32_t lt_mask = (1u << lane) - 1u;
+  const int CS = wa.CS;
   for (;;) {
     int batch = 0;
     if (lane == 0) batch = atomicAdd(s_ticket, 1);
     batch = __shfl_sync(0xFFFFFFFFu, batch, 0);
-    const uint32_t ti = (uint32_t)batch * kTPW + (uint32_t)(lane >> 2);      // track of the event, in batch order
-    if ((uint32_t)batch * kTPW >= t1 - t0) break;
-    const bool active = ti < t1 - t0;
-    const uint32_t tg = t0 + (active && perm ? (uint32_t)perm[ti] : ti);
+    const uint32_t ti = (uint32_t)batch * kTPW + (uint32_t)(lane >> 2);      // track of the item, in batch order
+    if ((uint32_t)batch * kTPW >= nTk) break;
+    const bool active = ti < nTk;
+    const uint32_t tg = t0 + (active ? (perm ? (uint32_t)perm[ti] : ti) * a.split + part : 0u);
     // ---------------- phase 1: window search, lane = (track, layer) ---------------------------------------
     int n_st = 0;
+    float zu = 0.f, wu = 0.f;
     if (active) {
       const float vx = __ldg(a.vx + tg), vy = __ldg(a.vy + tg), vtx = __ldg(a.vtx + tg), vty = __ldg(a.vty + tg);
       const float dzv = __fsub_rn(a.layer_z[l], a.vz);
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
-      n_st = collect_window<BUCKETED>(a, wa, S, lane, l, x_e, y_e, h0);
+      n_st = collect_window<BUCKETED>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
     }
     wa.n[lane] = n_st;
+    wa.zs[lane] = zu;
+    wa.ws[lane] = wu;
     if (lane < kTPW) wa.best[lane] = kNoKey;
+    const bool uni = __all_sync(0xFFFFFFFFu, zu == zu);      // every list of the batch has one z and one weight
     __syncwarp();
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
-    uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    for (int dir = 0; dir < 2 && todo; ++dir) {   // forward seeds (L0, L2), then backward (L3, L1)
-      const int LA = dir ? 3 : 0, LB = dir ? 1 : 2;
-      const uint32_t nA = wa.n[4 * j + LA], nB = wa.n[4 * j + LB];
-      // rows (track, hit a) of the batch, one per lane; the lane walks the partner hits b of its row
-      const uint32_t P = (lane < kTPW && ((todo >> j) & 1u) && nB > 0u) ? nA : 0u;
-      const uint32_t incl = warp_incl_scan(P, lane), excl = incl - P;
-      const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-      int qn = 0, qhead = 0;
-      for (uint32_t base = 0; base < total; base += 32) {
-        const uint32_t i = base + lane;
-        int jj = 0;                               // owner track: largest jj < 8 with excl[jj] <= i
-#pragma unroll
-        for (int step = 4; step > 0; step >>= 1) {
-          const uint32_t e = __shfl_sync(0xFFFFFFFFu, excl, jj + step);
-          if (e <= i) jj += step;
-        }
-        const uint32_t ia = i - __shfl_sync(0xFFFFFFFFu, excl, jj);
-        int nBj = (int)__shfl_sync(0xFFFFFFFFu, nB, jj);
-        const int sA = jj * 4 + LA, sB = jj * 4 + LB;
-        float da = 0.f, za = 0.f, zam = 0.f;
-        if (i < total) {
-          da = wa.cd[ia * 32 + sA];
-          za = __ldg(a.sec_z + (wa.chs[ia * 32 + sA] & 0xFFFFu));
-          zam = __fsub_rn(za, a.c.z_mag);
-        } else {
-          nBj = 0;
-        }
-        const int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
-        for (int ib = 0; ib < maxB; ++ib) {
-          bool pass = false;
-          float bs = 0.f;
-          if (ib < nBj) {
-            const float db = wa.cd[ib * 32 + sB];
-            const float zb = __ldg(a.sec_z + (wa.chs[ib * 32 + sB] & 0xFFFFu));
-            bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
-            const float a0 = __fsub_rn(da, __fmul_rn(bs, zam));
-            pass = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
-          }
-          const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
-          if (m == 0u) continue;
-          if (pass)
-            wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] =
-                make_uint2(((uint32_t)jj << 10) | (ia << 5) | (uint32_t)ib, __float_as_uint(bs));
-          qn += __popc(m);
-          __syncwarp();
-          if (qn >= 32) {
-            process_seeds(a, wa, lane, 32, qhead, dir);
-            qhead += 32;
-            qn -= 32;
-            __syncwarp();
-          }
-        }
-      }
-      if (qn > 0) process_seeds(a, wa, lane, qn, qhead, dir);
-      __syncwarp();
-      if (!a.c.both_directions)                   // backward only if nothing valid (A11); else best of both
-        todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);
-    }
+    const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
+    if (uni) find_tracklets<true>(a, wa, lane, todo); else find_tracklets<false>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
       const int q4 = lane & ~3;
@@ -487,8 +577,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
           pr[k] = pp[k] != 63u;
           d[k] = z[k] = w[k] = 0.f;
           if (pr[k]) {
-            const uint32_t hs = wa.chs[pp[k] * 32 + q4 + k];
-            d[k] = wa.cd[pp[k] * 32 + q4 + k];
+            const uint32_t hs = wa.chs[(q4 + k) * CS + pp[k]];
+            d[k] = wa.cd[(q4 + k) * CS + pp[k]];
             z[k] = __ldg(a.sec_z + (hs & 0xFFFFu));
             w[k] = __ldg(a.sec_w + (hs & 0xFFFFu));
             if (k == l) hidx = (int)(h0 + (hs >> 16));
@@ -504,7 +594,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
   }
 }
 
-// One CTA works through events blockIdx.x, blockIdx.x + gridDim.x, ...  Geometry tables are staged once.
+// One CTA works through work items (event, part) handed out by the ticket.  Geometry tables are staged once.
 template <int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -514,15 +604,17 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   Carver cvr(smem_raw);
   float4* s_gA = cvr.take<float4>(ng);
   uint2* s_gB = cvr.take<uint2>(ng);
-  float2* s_yr = cvr.take<float2>(UT_COMPASS_YR_SMEM ? ns : 0);
   uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);
-  uint16_t* s_off = cvr.take<uint16_t>(ns + 1);
-  float* s_hx = cvr.take<float>(a.hit_stage);
-  uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage);
+  uint16_t* s_off = cvr.take<uint16_t>(a.soff_stride);
+  float* s_hx = cvr.take<float>(a.hit_stage + 8);
+  uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage + 16);
   uint16_t* s_perm = cvr.take<uint16_t>(a.trk_stage);
-  unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by s_cnt below
+  unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by the scratch below
+  // scratch while no warp is in the track loop: radius bins + per-track (bin, position); re-bucketing counters and
+  // the event's id and x ranges (two bulk copies) when the container carries no per-sector view
+  uint32_t* s_bins = reinterpret_cast<uint32_t*>(s_warp_areas);
+  uint32_t* s_binpos = s_bins + kBins;
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp_areas);
-  // while staging, the same region also receives the event's id and x ranges by two bulk copies (TMA)
   uint32_t* s_tmp_id = reinterpret_cast<uint32_t*>(s_warp_areas + align16((size_t)ns * 8));
   float* s_tmp_x = reinterpret_cast<float*>(s_warp_areas + align16((size_t)ns * 8) + align16((size_t)(a.hit_stage + 8) * 4));
   __shared__ float2 s_lay[4];
@@ -533,8 +625,6 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t lt_mask = (1u << lane) - 1u;
 
   // ---- geometry tables, once per CTA ---------------------------------------------------------------------
-  for (uint32_t s = tid; UT_COMPASS_YR_SMEM && s < ns; s += nt)
-    s_yr[s] = make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
   for (uint32_t g = tid; g < ng; g += nt) {
     const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
     const float y0 = __fadd_rn(__ldg(a.sec_ye + sa), a.c.y_tol), y1 = __fadd_rn(__ldg(a.sec_ye + sb - 1), a.c.y_tol);
@@ -548,26 +638,35 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     s_lay[tid] = make_float2(x0, (a.gpl > 1 && x1 > x0) ? (float)(a.gpl - 1) / (x1 - x0) : 0.f);
   }
   SmemView S;
-  S.gA = s_gA; S.gB = s_gB; S.yr = s_yr; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
+  S.gA = s_gA; S.gB = s_gB; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
   WarpArea wa;
   {
+    const int CS = cand_stride(C);
     unsigned char* p = s_warp_areas + (size_t)warp * warp_area_bytes(C);
+    wa.CS = CS;
     wa.cd = reinterpret_cast<float*>(p);
-    wa.chs = reinterpret_cast<uint32_t*>(p + (size_t)C * 32 * 4);
-    wa.seedq = reinterpret_cast<uint2*>(p + (size_t)C * 32 * 8);
-    wa.best = reinterpret_cast<unsigned long long*>(p + (size_t)C * 32 * 8 + kSeedQ * 8);
-    wa.n = reinterpret_cast<int*>(p + (size_t)C * 32 * 8 + kSeedQ * 8 + kTPW * 8);
+    wa.chs = reinterpret_cast<uint32_t*>(p + (size_t)CS * 32 * 4);
+    p += (size_t)CS * 32 * 8;
+    wa.best = reinterpret_cast<unsigned long long*>(p);
+    wa.seedq = reinterpret_cast<uint32_t*>(p + kTPW * 8);
+    wa.n = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4);
+    wa.zs = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 4);
+    wa.ws = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 8);
   }
   const uint32_t Tend = __ldg(a.velo_offsets + a.n_events);
   const uint32_t T = a.idx_stride ? a.idx_stride : Tend;
+  const uint32_t K = a.split;
+  const uint32_t n_items = (uint32_t)a.n_events * K;
 
-  __shared__ int s_event[2];                       // double-buffered: a slow thread still reads the previous ticket
+  __shared__ uint32_t s_item[2];                   // double-buffered: a slow thread still reads the previous ticket
   for (int k = 0;; ++k) {
-    // events are dealt out dynamically (CTAs that finish early take more), statically without a workspace
-    if (tid == 0) s_event[k & 1] = a.ticket ? (int)atomicAdd(a.ticket, 1u) : (int)(blockIdx.x + (unsigned)k * gridDim.x);
-    __syncthreads();                               // tables staged / previous event fully consumed
-    const int e = s_event[k & 1];
-    if (e >= a.n_events) break;
+    // work items are dealt out dynamically: CTAs that finish early take more
+    if (tid == 0) s_item[k & 1] = atomicAdd(a.status + 1, 1u);
+    __syncthreads();                               // tables staged / previous item fully consumed
+    const uint32_t item = s_item[k & 1];
+    if (item >= n_items) break;
+    const int e = (int)(item / K);
+    const uint32_t part = item - (uint32_t)e * K;
     const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
     const uint32_t* go = a.hit_offsets + (size_t)e * ng;
     const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
@@ -583,23 +682,44 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     if (tid == 0) s_ticket = 0;
     const uint32_t n = h1 - h0;
-    // (__syncthreads_or returns a truth value, not the OR of the arguments; n is the same in every thread)
+    const uint32_t nT = t1 - t0;
+    const uint32_t nTk = nT > part ? (nT - part + K - 1) / K : 0u;      // tracks t0 + part, t0 + part + K, ...
     // an event whose hits end past `capacity` was not written by the decode (UT_STATUS_CAPACITY there): its range of
     // the hit arrays must not be read
+    // (__syncthreads_or returns a truth value, not the OR of the arguments; n is the same in every thread)
     const int flag = __syncthreads_or(bad ? 1 : 0) ? 1 : ((unsigned long long)h1 > a.capacity ? 4 : (n > 65535u ? 2 : 0));
-    if (flag) {                                    // uniform: report and emit "no tracklet" for every track
+    if (flag) {                                    // uniform: report and emit "no tracklet" for every track of the part
       if (tid == 0) atomicOr(a.status, (flag & 1 ? (uint32_t)UT_STATUS_BAD_OFFSETS : 0u) |
                                            (flag & 2 ? (uint32_t)UT_STATUS_EVENT_TOO_LARGE : 0u) |
                                            (flag & 4 ? (uint32_t)UT_STATUS_CAPACITY : 0u));
-      for (uint32_t t = t0 + tid; t < t1; t += nt) {
-        for (int k = 0; k < 4; ++k) a.out_idx[(size_t)k * T + t] = -1;
+      for (uint32_t m = tid; m < nTk; m += nt) {
+        const uint32_t t = t0 + m * K + part;
+        for (int q = 0; q < 4; ++q) a.out_idx[(size_t)q * T + t] = -1;
         a.out_n[t] = 0; a.out_qop[t] = 0.f; a.out_chi2[t] = 0.f;
       }
       continue;
     }
-    if (t1 == t0) continue;
+    if (nTk == 0) continue;
     const bool staged = n <= a.hit_stage;
-    if (staged) {
+    // the per-sector view of the event as ut_decode left it: three bulk copies, nothing to compute
+    const bool view = staged && a.soff != nullptr &&
+                      __ldg(a.soff + (size_t)e * a.soff_stride + ns + 1) == (uint16_t)UT_SECTOR_INDEX_VALID;
+    if (view) {
+      const uint32_t cx0 = h0 & ~3u, cx1 = (h1 + 3u) & ~3u, ci0 = h0 & ~7u, ci1 = (h1 + 7u) & ~7u;
+      if (tid == 0) {
+        fence_proxy_async();                 // earlier generic-proxy accesses of the staging arrays are done (barrier above)
+        mbar_expect_tx(&s_bar, (n > 0 ? (cx1 - cx0) * 4u + (ci1 - ci0) * 2u : 0u) + a.soff_stride * 2u);
+        bulk_g2s(s_off, a.soff + (size_t)e * a.soff_stride, a.soff_stride * 2u, &s_bar);
+        if (n > 0) {
+          bulk_g2s(s_hx, a.sx + cx0, (cx1 - cx0) * 4u, &s_bar);
+          bulk_g2s(s_hh, a.si + ci0, (ci1 - ci0) * 2u, &s_bar);
+        }
+      }
+      S.hx = s_hx + (h0 - cx0);
+      S.hh = s_hh + (h0 - ci0);
+    } else if (staged) {
+      S.hx = s_hx;
+      S.hh = s_hh;
       // ---- stage: a warp re-buckets one sector group at a time, per sector, keeping the x order -----------
       // (count -> warp scan over the group's sectors -> ordered scatter with match.any; no block barrier)
       bool bad_id = false;
@@ -706,58 +826,66 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
         }
       }
       if (bad_id) atomicOr(a.status, (uint32_t)UT_STATUS_BAD_HIT_ID);
-      __syncthreads();                             // s_cnt is dead from here on: the warp areas take its place
+      __syncthreads();                             // s_cnt is dead from here on: the bins / warp areas take its place
     }
-    // ---- batch order: the tracks of the event by radius at the first layer, inner tracks first ---------------
+    // ---- batch order: the tracks of the item binned by radius at the first layer, inner tracks first -----------
     // Inner tracks cross the busy sectors and have the long candidate lists; a batch costs what its heaviest
-    // track costs, so like goes with like and the heavy batches start first.  Results do not depend on the order.
-    const uint32_t nT = t1 - t0;
+    // track costs, so like goes with like and the heavy batches start first.  Results do not depend on the order
+    // (the order inside a bin is whatever the atomics make it).  Bin = exponent and 3 mantissa bits of r^2.
     const uint16_t* perm = nullptr;
-    if (nT > (uint32_t)kTPW && nT <= a.trk_stage) {
-      float* keys = reinterpret_cast<float*>(s_warp_areas);    // scratch: the warp areas are idle here
+    if (nTk > (uint32_t)kTPW && nTk <= a.trk_stage) {
+      for (uint32_t i = tid; i < (uint32_t)kBins; i += nt) s_bins[i] = 0;
+      __syncthreads();
       const float dz0 = __fsub_rn(a.layer_z[0], a.vz);
-      for (uint32_t i = tid; i < ((nT + 3u) & ~3u); i += nt) {
-        float k = __int_as_float(0x7F800000);
-        if (i < nT) {
-          const float x = __ldg(a.vx + t0 + i) + __ldg(a.vtx + t0 + i) * dz0, y = __ldg(a.vy + t0 + i) + __ldg(a.vty + t0 + i) * dz0;
-          k = x * x + y * y;
-          if (!(k == k)) k = __int_as_float(0x7F800000);       // NaN state: last, so that the rank stays a permutation
-        }
-        keys[i] = k;
+      for (uint32_t m = tid; m < nTk; m += nt) {
+        const uint32_t t = t0 + m * K + part;
+        const float x = __ldg(a.vx + t) + __ldg(a.vtx + t) * dz0, y = __ldg(a.vy + t) + __ldg(a.vty + t) * dz0;
+        const float r2 = x * x + y * y;
+        int b = (int)(__float_as_uint(r2) >> 20) - 0x418;        // r = 4 mm -> bin 0, r = 1 m -> bin 127
+        b = r2 == r2 ? max(0, min(kBins - 1, b)) : kBins - 1;    // NaN state: last
+        s_binpos[m] = ((uint32_t)b << 16) | atomicAdd(&s_bins[b], 1u);
       }
       __syncthreads();
-      for (uint32_t i = tid; i < nT; i += nt) {
-        const float ki = keys[i];
-        uint32_t rank = 0;
-        for (uint32_t j = 0; j < nT; j += 4) {
-          const float4 v = *reinterpret_cast<const float4*>(keys + j);
-          rank += (v.x < ki || (v.x == ki && j < i)) + (v.y < ki || (v.y == ki && j + 1 < i)) +
-                  (v.z < ki || (v.z == ki && j + 2 < i)) + (v.w < ki || (v.w == ki && j + 3 < i));
-        }
-        s_perm[rank] = (uint16_t)i;
+      if (warp == 0) {
+        uint32_t c[kBins / 32], run = 0;
+#pragma unroll
+        for (int q = 0; q < kBins / 32; ++q) { c[q] = s_bins[lane * (kBins / 32) + q]; run += c[q]; }
+        uint32_t ex = warp_incl_scan(run, lane) - run;
+#pragma unroll
+        for (int q = 0; q < kBins / 32; ++q) { s_bins[lane * (kBins / 32) + q] = ex; ex += c[q]; }
+      }
+      __syncthreads();
+      for (uint32_t m = tid; m < nTk; m += nt) {
+        const uint32_t bp = s_binpos[m];
+        s_perm[s_bins[bp >> 16] + (bp & 0xFFFFu)] = (uint16_t)m;
       }
       perm = s_perm;
-      __syncthreads();
     }
+    if (view) {
+      mbar_wait(&s_bar, bar_phase);
+      bar_phase ^= 1u;
+    }
+    __syncthreads();                               // order and staged data visible; scratch is dead from here on
     if (staged) {
-      track_loop<true>(a, wa, S, &s_ticket, h0, t0, t1, T, perm);
+      track_loop<true>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false>(a, wa, S, &s_ticket, h0, t0, t1, T, perm);
+      track_loop<false>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     }
   }
-  if (tid == 0 && a.ticket) {                 // last CTA out re-arms the ticket for the next call
+  if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
     __threadfence();
-    if (atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1) { a.ticket[0] = 0; a.ticket[1] = 0; __threadfence(); }
+    if (atomicAdd(a.status + 2, 1u) == gridDim.x - 1) { a.status[1] = 0; a.status[2] = 0; __threadfence(); }
   }
 }
 
-static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t hit_stage, int C, int block, uint32_t trk_stage = 0) {
-  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8) + (UT_COMPASS_YR_SMEM ? align16((size_t)ns * 8) : 0);
-  b += align16((ng + 1) * 4) + align16((ns + 1) * 2);
-  b += align16((size_t)hit_stage * 4) + align16((size_t)hit_stage * 2) + align16((size_t)trk_stage * 2);
+static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t soff_stride, uint32_t hit_stage, int C, int block,
+                                 uint32_t trk_stage = 0) {
+  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8);
+  b += align16((ng + 1) * 4) + align16((size_t)soff_stride * 2);
+  b += align16((size_t)(hit_stage + 8) * 4) + align16((size_t)(hit_stage + 16) * 2) + align16((size_t)trk_stage * 2);
   b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C)),
-                 align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4),   // staging scratch aliases the warp areas
-                 align16((size_t)trk_stage * 4)});                                      // and so do the ordering keys
+                 align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4),   // re-bucketing scratch aliases the warp areas
+                 align16((size_t)(kBins + trk_stage) * 4)});                            // and so do the radius bins
   return b;
 }
 
@@ -782,6 +910,14 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   CompassArgs a;
   a.hx = hits->x_at_y0; a.hid = hits->id; a.hyb = hits->y_begin; a.hye = hits->y_end;
   a.hit_offsets = hit_offsets;
+  a.soff_stride = (geom->n_sectors + 2u + 7u) & ~7u;
+  // the per-sector view is used when all three arrays are there and 16-byte aligned (bulk copies)
+  const bool view_ok = hits->x_by_sector && hits->idx_by_sector && hits->sector_offsets &&
+                       ((reinterpret_cast<uintptr_t>(hits->x_by_sector) | reinterpret_cast<uintptr_t>(hits->idx_by_sector) |
+                         reinterpret_cast<uintptr_t>(hits->sector_offsets)) & 15u) == 0;
+  a.sx = view_ok ? hits->x_by_sector : nullptr;
+  a.si = view_ok ? hits->idx_by_sector : nullptr;
+  a.soff = view_ok ? hits->sector_offsets : nullptr;
   a.vx = velo->x; a.vy = velo->y; a.vtx = velo->tx; a.vty = velo->ty; a.vz = velo->z;
   a.velo_offsets = velo_offsets; a.n_events = n_events;
   a.n_sectors = geom->n_sectors; a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
@@ -791,10 +927,10 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
+  a.slope_lim = cfg->max_slope * (1.0f + kFilterEps);
   a.idx_stride = idx_stride;
   a.capacity = hits->capacity;
   a.bulk_ok = ((reinterpret_cast<uintptr_t>(hits->x_at_y0) | reinterpret_cast<uintptr_t>(hits->id)) & 15u) == 0 ? 1u : 0u;
-  a.ticket = hits->workspace ? reinterpret_cast<uint32_t*>(hits->workspace) + 4 : nullptr;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
 
   const int C = cfg->max_candidates_per_layer;
@@ -812,7 +948,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= 768; b += 32) {
-      const size_t sm = compass_smem_bytes(ns, ng, hit_stage, C, b) + 1024;
+      const size_t sm = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, b) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
@@ -822,21 +958,21 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     if (block <= 0) block = 192;
   }
   block = std::max(32, std::min(768, (block / 32) * 32));
-  size_t smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
+  size_t smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
   while (smem > budget && block > 64) {             // fewer warps before giving up staging
     block -= 32;
-    smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
   }
   while (smem > budget && hit_stage > 0) {
     hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
-    smem = compass_smem_bytes(ns, ng, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  // room for ordering up to 2048 (else 1024, 512) tracks per event, if it costs no resident CTA
+  // room for ordering up to 2048 (else 1024, 512) tracks per item, if it costs no resident CTA
   a.trk_stage = 0;
   for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
-    const size_t with = compass_smem_bytes(ns, ng, hit_stage, C, block, want);
+    const size_t with = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block, want);
     if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
       a.trk_stage = want;
       smem = with;
@@ -847,12 +983,23 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
   if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);
-  const int grid = std::max(1, std::min(n_events, n_sm * per_sm));
+  // K CTAs share the tracks of an event only while whole events would leave resident CTAs idle (a 100-event batch
+  // on 592 CTA slots).  Measured on a B200, config 3: K = 1 127 us, K = 2 145 us, K = 4 182 us -- a part pays the
+  // event's fixed cost again (ticket, offsets, staging wait, order) and its last round of batches is emptier.
+  const int resident = n_sm * per_sm;
+  int split = tuned(tune.compass_split, 0);
+  if (split <= 0) {
+    split = 1;
+    while (split < 4 && (long long)n_events * split * 2 <= resident && avg >= 256) split *= 2;
+  }
+  split = split >= 4 ? 4 : (split >= 2 ? 2 : 1);
+  a.split = (uint32_t)split;
+  const int grid = std::max(1, (int)std::min<long long>((long long)n_events * split, resident));
   void* params[] = {&a};
   UTC_CUDA(cudaLaunchKernel(kernel, dim3(grid), dim3(block), params, smem, stream));
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.compass_grid = grid; li.compass_block = block; li.compass_smem_bytes = (int)smem;
-  li.compass_hit_stage = (int)hit_stage;
+  li.compass_hit_stage = (int)hit_stage; li.compass_split = split; li.compass_view = view_ok ? 1 : 0;
   return UT_OK;
 }
 

@@ -17,6 +17,9 @@
 //      tie-break order, so the rank IS the stable sort by x   (paper: pre-decode + find permutation)
 //   -> SoA store at base + group start + rank; a group is one contiguous window of every array
 //                                                            (paper: decode raw banks in order)
+//   -> optional per-sector view for compass_track (ut_hits.x_by_sector ...): the same warp re-emits the group's x
+//      and container index bucketed per sector (the fill order IS sector-major, so a sector's entries are a
+//      contiguous run and the position inside the run is the rank among the sector's own hits)
 //
 // There is no block barrier after the count: warps run independently through the groups.
 // Events or groups that do not fit the staging sizes take slower generic code with the same results.
@@ -44,6 +47,10 @@ struct DecodeArgs {
   uint32_t raw_stage_bytes;     // multiple of 16
   uint32_t sort_buf;            // elements of the per-warp sort buffer (multiple of 32)
   const uint32_t* carry_in;     // hits in front of event 0 (chunked pipeline) or null
+  float* sx;                    // per-sector view (ut_hits.x_by_sector / idx_by_sector / sector_offsets) or null
+  uint16_t* si;
+  uint16_t* soff;
+  uint32_t soff_stride;
 };
 
 __device__ __forceinline__ float decode_x(uint32_t word, float x0, float pitch) {
@@ -194,7 +201,15 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         if (g < ng) a.hit_offsets[(size_t)e * ng + g] = base + gs[q];
       }
     }
-    if (tot == 0) continue;
+    // per-sector view: usable by compass_track iff the event fits u16 positions and no group takes the generic path
+    const bool view = a.soff != nullptr && tot <= 65535u &&
+                      !__any_sync(0xFFFFFFFFu, gc[0] > a.sort_buf || gc[1] > a.sort_buf || gc[2] > a.sort_buf || gc[3] > a.sort_buf);
+    uint16_t* soff = a.soff ? a.soff + (size_t)e * a.soff_stride : nullptr;
+    if (warp == 0 && lane == 0 && soff) {
+      soff[ns] = (uint16_t)tot;
+      soff[ns + 1] = (view && (unsigned long long)base + tot <= a.capacity) ? (uint16_t)UT_SECTOR_INDEX_VALID : (uint16_t)0;
+    }
+    if (tot == 0 && !view) continue;
 
     // ---- warp per sector group (ticket inside the CTA) --------------------------------------------------
     for (;;) {
@@ -206,13 +221,17 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
       const uint32_t n = __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gc[0] : q4 == 1 ? gc[1] : q4 == 2 ? gc[2] : gc[3], (int)(g >> 2));
       const uint32_t gstart =
           __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gs[0] : q4 == 1 ? gs[1] : q4 == 2 ? gs[2] : gs[3], (int)(g >> 2));
-      if (n == 0) continue;
       const uint32_t sa = g_gfirst[g], nsec = g_gfirst[g + 1] - sa;      // nsec <= 32 (ut_geometry_upload)
+      if (n == 0) {
+        if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)gstart;
+        continue;
+      }
       // the group's banks: word count and word position per sector, exclusive prefix = fill order
       const uint32_t cnt_r = (uint32_t)lane < nsec ? s_cnt[sa + lane] : 0u;
       const uint32_t wpos_r = (uint32_t)lane < nsec ? s_wpos[sa + lane] : 0u;
       const uint32_t e_incl = warp_incl_scan(cnt_r, lane);
       const uint32_t e_r = (uint32_t)lane < nsec ? e_incl - cnt_r : n;   // lanes past the group: never selected
+      if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)(gstart + e_r);
       const bool in_regs = n <= 32u, in_buf = n <= a.sort_buf;
 
       // gather: element i of the fill order -> (sector r, word k), decode x
@@ -258,6 +277,22 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
           a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
           a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
         }
+        if (view) {
+          // per-sector view: lane r takes the hit of rank r (container order); its position inside its sector's run
+          // is its rank among the lanes of the same sector
+          if ((uint32_t)lane < n) { xbuf[rank] = x; wbuf[rank] = rw >> 16; }
+          __syncwarp();
+          const float xs = (uint32_t)lane < n ? xbuf[lane] : 0.f;
+          const uint32_t ss = (uint32_t)lane < n ? wbuf[lane] : 0xFFFFu;
+          const uint32_t peers = __match_any_sync(0xFFFFFFFFu, ss);
+          const uint32_t es = __shfl_sync(0xFFFFFFFFu, e_r, (int)(ss & 31u));
+          if ((uint32_t)lane < n) {
+            const size_t Q = P0 + es + __popc(peers & lt_mask);
+            a.sx[Q] = xs;
+            a.si[Q] = (uint16_t)(gstart + lane);
+          }
+          __syncwarp();                                 // the buffers are reused by the warp's next group
+        }
       } else if (in_buf) {
         // ---- <= sort_buf hits: rank against the warp's shared-memory copy -----------------------------------
         const uint32_t npad = (n + 3u) & ~3u;          // pad the tail of the buffer with +inf (never "smaller")
@@ -284,6 +319,27 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
             const size_t P = P0 + rank;
             a.x[P] = xi; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
             a.id[P] = (__float_as_uint(B.y) << 9) | (rwi & 0x1FFu);
+            if (view) wbuf[i] = (rwi & 0xFFFF0000u) | rank;          // (sector in group, rank) for the view below
+          }
+        }
+        if (view) {
+          // per-sector view: the fill order is sector-major, so the entries of sector r are elements
+          // [e_r, e_r + cnt_r) of the buffer; the position inside the run is the rank among them
+          __syncwarp();
+          for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+            const uint32_t i = c0 + lane;
+            const bool valid = i < n;
+            const uint32_t rwi = valid ? wbuf[i] : 0u;
+            const uint32_t rank = rwi & 0xFFFFu;
+            const uint32_t es = __shfl_sync(0xFFFFFFFFu, e_r, (int)(rwi >> 16));
+            const uint32_t cs = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)(rwi >> 16));
+            if (valid) {
+              uint32_t pos = 0;
+              for (uint32_t j = es; j < es + cs; ++j) pos += (wbuf[j] & 0xFFFFu) < rank ? 1u : 0u;
+              const size_t Q = P0 + es + pos;
+              a.sx[Q] = xbuf[i];
+              a.si[Q] = (uint16_t)(gstart + rank);
+            }
           }
         }
         __syncwarp();                                   // the buffer is reused by the warp's next group
@@ -365,6 +421,8 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   a.w = hits->weight; a.id = hits->id; a.capacity = hits->capacity; a.status = hits->status;
   a.hit_offsets = hit_offsets;
   a.carry_in = carry_in;
+  a.sx = hits->x_by_sector; a.si = hits->idx_by_sector; a.soff = hits->sector_offsets;
+  a.soff_stride = (geom->n_sectors + 2u + 7u) & ~7u;
   a.ctrl = reinterpret_cast<uint32_t*>(hits->workspace);
   a.flags = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hits->workspace) + 32);
 

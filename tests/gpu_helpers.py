@@ -9,10 +9,11 @@ class GpuRunner:
         self.B, self.torch = B, torch
         self.geom = B.ut_geometry_upload(geom_tables)
         self.tables = geom_tables
+        self.sector_view = True          # containers carry the optional per-sector view (ut_hits.x_by_sector ...)
 
     def decode(self, raw, bank_offsets, n_events, capacity):
         B, torch = self.B, self.torch
-        hits = B.Hits(capacity, max(n_events, 1), self.geom)
+        hits = B.Hits(capacity, max(n_events, 1), self.geom, sector_view=self.sector_view)
         raw_d = B.to_device_raw(raw)
         bo_d = B.to_device_u32(bank_offsets)
         B.ut_decode(raw_d, bo_d, n_events, self.geom, hits)
@@ -36,7 +37,7 @@ class GpuRunner:
         B.compass_track(hits, hits.hit_offsets, velo, vo, n_events, B.make_config(params), tracks)
         torch.cuda.synchronize()
         idx, n, qop, chi2 = tracks.numpy()
-        return dict(hit_idx=idx, n_hits=n, qop=qop, chi2=chi2, status=int(tracks.status.item()) & 0xFFFFFFFF)
+        return dict(hit_idx=idx, n_hits=n, qop=qop, chi2=chi2, status=int(tracks.status[0].item()) & 0xFFFFFFFF)
 
     def run(self, batch, params):
         hits = self.decode(batch.raw, batch.bank_offsets, batch.n_events, batch.hit_capacity)
@@ -72,7 +73,7 @@ def compare_tracks(ref, got, rel=1e-5, status=0):
 
 # ---- guard bands: every output array sits between two 4 KB canaries (the pool has no compute-sanitizer) -------
 GUARD = 1024                        # elements in front of and behind the array
-_CANARY = {"float32": -12345.678, "int32": -0x5A5A5A5B, "int64": -0x5A5A5A5A5A5A5A5B}
+_CANARY = {"float32": -12345.678, "int32": -0x5A5A5A5B, "int64": -0x5A5A5A5A5A5A5A5B, "int16": -0x5A5B}
 
 
 def _guarded(n, dtype):
@@ -89,7 +90,7 @@ def check_guards(guards):
         assert bool((front == c).all()) and bool((back == c).all()), f"canary of {name} overwritten"
 
 
-def guarded_hits(B, capacity, max_events, geometry):
+def guarded_hits(B, capacity, max_events, geometry, sector_view=True):
     """B.Hits whose arrays have EXACTLY `capacity` elements between canaries (hit_offsets, status, workspace too)."""
     import torch
     h = B.Hits(capacity, max_events, geometry)
@@ -109,9 +110,19 @@ def guarded_hits(B, capacity, max_events, geometry):
     full, h.workspace = _guarded(nw, torch.int64)
     h.workspace.zero_()
     guards.append(("workspace", full, nw))
-    h.c = B.ut_hits(h.x_at_y0.data_ptr(), h.z_at_y0.data_ptr(), h.y_begin.data_ptr(), h.y_end.data_ptr(),
-                    h.dxdy.data_ptr(), h.weight.data_ptr(), h.id.data_ptr(), int(capacity), h.c.geom,
-                    h.status.data_ptr(), h.workspace.data_ptr())
+    if sector_view:
+        n8 = (n + 7) // 8 * 8
+        full, h.x_by_sector = _guarded(n8, torch.float32)
+        guards.append(("x_by_sector", full, n8))
+        full, h.idx_by_sector = _guarded(n8, torch.int16)
+        guards.append(("idx_by_sector", full, n8))
+        nso = max(max_events, 1) * B.ut_sector_offsets_stride(geometry)
+        full, h.sector_offsets = _guarded(nso, torch.int16)
+        h.sector_offsets.zero_()
+        guards.append(("sector_offsets", full, nso))
+    else:
+        h.x_by_sector = h.idx_by_sector = h.sector_offsets = None
+    h.c = h.descriptor()
     return h, guards
 
 
@@ -121,7 +132,7 @@ def guarded_tracks(B, n_velo_total):
     n = max(int(n_velo_total), 1)
     guards = []
     for f, m, dt in (("hit_idx", 4 * n, torch.int32), ("n_hits", n, torch.int32), ("qop", n, torch.float32),
-                     ("chi2", n, torch.float32), ("status", 1, torch.int32)):
+                     ("chi2", n, torch.float32), ("status", 4, torch.int32)):
         full, view = _guarded(m, dt)
         setattr(t, f, view)
         guards.append(("tracks." + f, full, m))

@@ -16,7 +16,7 @@ def declared_functions():
     text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)          # comments
     text = re.sub(r"^\s*#.*$", " ", text, flags=re.M)           # preprocessor lines
     text = re.sub(r"typedef\s+struct\s*\{.*?\}\s*\w+\s*;", " ", text, flags=re.S)
-    names = re.findall(r"\b(?:int32_t|size_t|void|const\s+char\s*\*)\s+(\w+)\s*\(", text)
+    names = re.findall(r"\b(?:int32_t|uint32_t|size_t|void|const\s+char\s*\*)\s+(\w+)\s*\(", text)
     return sorted(set(names))
 
 

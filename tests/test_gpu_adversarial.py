@@ -25,13 +25,16 @@ def gpu(geom):
     return GpuRunner(geom)
 
 
-@pytest.fixture(params=["staged", "global"])
+@pytest.fixture(params=["view", "restage", "global", "split4"])
 def run(request, gpu):
-    """run(geom, batch, params): GPU == oracle bit for bit, returns the oracle's (hits, tracks).  Both window-search
-    paths of compass_track: per-sector buckets in shared memory, and the search on global memory (the path of
-    events that do not fit the staging)."""
+    """run(geom, batch, params): GPU == oracle bit for bit, returns the oracle's (hits, tracks).  Every data path
+    of compass_track: per-sector buckets in shared memory taken from the decode's per-sector view (bulk copies) or
+    re-bucketed by the kernel (container without the view), the search on global memory (the path of events that
+    do not fit the staging), and four CTAs sharing one event's tracks."""
     from gpu_helpers import compare_decode
-    gpu.B.ut_tuning_set(compass_hit_stage=-1 if request.param == "staged" else 0)
+    gpu.B.ut_tuning_set(compass_hit_stage=0 if request.param == "global" else -1,
+                        compass_split=4 if request.param == "split4" else -1)
+    gpu.sector_view = request.param != "restage"
 
     def run_both(geom, b, p):
         h_ref, t_ref = oracle.run_batch(b, geom, p)
@@ -47,6 +50,7 @@ def run(request, gpu):
 
     yield run_both
     gpu.B.ut_tuning_set(None)
+    gpu.sector_view = True
 
 
 @pytest.mark.parametrize("layer", [0, 1, 2, 3])
@@ -315,7 +319,7 @@ def test_two_host_threads(gpu, wl):
                     B.ut_decode(raw_d, bo_d, b.n_events, gpu.geom, hits, stream=s)
                     B.compass_track(hits, hits.hit_offsets, velo, vo, b.n_events, cfg, tracks, stream=s)
                 s.synchronize()
-                results[k] = (gpu.hits_numpy(hits, b.n_events), tracks.numpy(), int(tracks.status.item()))
+                results[k] = (gpu.hits_numpy(hits, b.n_events), tracks.numpy(), int(tracks.status[0].item()))
         except Exception as exc:                     # surfaced in the main thread
             errors.append(exc)
 

@@ -49,6 +49,50 @@ def test_config2(gpu, wl):
     check_batch(gpu, geom, b, p)
 
 
+def check_sector_view(gpu, geom, b, hits, h_ref):
+    """The per-sector view ut_decode writes beside the container (include/ut_compass.h): for every event and dense
+    sector the hits of that sector, in container order, found by their ids in the oracle's container."""
+    ne, ng, ns = b.n_events, geom.n_groups, geom.n_sectors
+    stride = gpu.B.ut_sector_offsets_stride(gpu.geom)
+    so = hits.sector_offsets.cpu().numpy().view(np.uint16).reshape(-1, stride)[:ne]
+    sx = hits.x_by_sector.cpu().numpy()
+    si = hits.idx_by_sector.cpu().numpy().view(np.uint16)
+    ev0 = h_ref.hit_offsets[::ng].astype(np.int64)
+    sec = geom.id_to_sector[h_ref.id[:h_ref.n_hits] >> 9].astype(np.int64)
+    for e in range(ne):
+        lo, hi = int(ev0[e]), int(ev0[e + 1])
+        assert so[e, ns + 1] == 0xA5A5 and so[e, ns] == hi - lo and so[e, 0] == 0
+        cnt = np.bincount(sec[lo:hi], minlength=ns)
+        assert np.array_equal(np.diff(so[e, :ns + 1].astype(np.int64)), cnt)
+        order = np.argsort(sec[lo:hi], kind="stable")              # sector-major, container order inside a sector
+        assert np.array_equal(si[lo:hi], order.astype(np.uint16))
+        assert np.array_equal(sx[lo:hi].view(np.uint32), h_ref.x_at_y0[lo:hi][order].view(np.uint32))
+
+
+def test_sector_view_contents(gpu, wl):
+    for c, n in ((2, 40), (4, 10)):
+        geom, b, p = wl(c, n)
+        h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+        hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+        check_sector_view(gpu, geom, b, hits, h_ref)
+
+
+@pytest.mark.parametrize("split", [1, 2, 4])
+@pytest.mark.parametrize("view", [True, False])
+def test_compass_data_paths(gpu, wl, view, split):
+    """Same results with and without the decode's per-sector view, and with 1, 2 or 4 CTAs per event."""
+    geom, b, p = wl(3, 120)
+    gpu.sector_view = view
+    gpu.B.ut_tuning_set(compass_split=split)
+    try:
+        check_batch(gpu, geom, b, p)
+        li = gpu.B.last_launch_info()
+        assert li["compass_view"] == int(view) and li["compass_split"] == split
+    finally:
+        gpu.sector_view = True
+        gpu.B.ut_tuning_set(None)
+
+
 def test_config3_subset(gpu, wl):
     geom, b, p = wl(3, 300)          # several waves of CTAs, ragged tail
     check_batch(gpu, geom, b, p)
@@ -439,7 +483,7 @@ def test_compass_status_paths(gpu, geom):
     tr.n_hits.fill_(-9)
     B.compass_track(hits, hits.hit_offsets, velo, B.to_device_u32(vo), 3, B.make_config(p), tr)
     torch.cuda.synchronize()
-    assert int(tr.status.item()) & B.UT_STATUS_BAD_OFFSETS
+    assert int(tr.status[0].item()) & B.UT_STATUS_BAD_OFFSETS
 
 
 def test_compass_bad_hit_id(gpu, geom):
@@ -451,7 +495,11 @@ def test_compass_bad_hit_id(gpu, geom):
     b = assemble_batch(geom, [generate_event(geom, m, 8, k) for k in range(3)])
     p = synth.make_compass_params()
     _, t_ref = oracle_run(b, geom, p)
-    hits = gpu.decode(b.raw, b.bank_offsets, 3, b.hit_capacity)
+    gpu.sector_view = False          # a container without the decode's per-sector view: compass_track reads the ids
+    try:
+        hits = gpu.decode(b.raw, b.bank_offsets, 3, b.hit_capacity)
+    finally:
+        gpu.sector_view = True
     k = int(hits.hit_offsets[64 + 3].item())                   # a hit of event 1
     hits.id[k] = (1023 << 9) | 5                                # raw sector id 1023 is not in the table
     trk = gpu.compass(hits, b, p)
