@@ -86,6 +86,9 @@ typedef struct {
 /* y_begin and y_end are non-decreasing over the sectors of every group: the sector row a track crosses
  * can be found by binary search (else compass_track scans the group's sectors). */
 #define UT_GEOM_ROWS_SORTED 1u
+/* every group of a layer has the same number of sectors with the same y ranges, row by row: compass_track finds the
+ * sector row a track crosses once per layer instead of once per group */
+#define UT_GEOM_ROWS_UNIFORM 2u
 
 /* Copies HOST tables (`host_tables` holds HOST pointers in the array fields) to the device, checks
  * the contract above and fills `device_out` with device pointers.  Synchronous; call once at set-up. */

@@ -181,6 +181,14 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
         return UT_ERR_GEOMETRY;                                           // bounds monotone inside a layer
     }
   }
+  bool rows_uniform = rows_sorted;
+  for (uint32_t g = 0; g < ng && rows_uniform; ++g) {
+    const uint32_t gl = (g / gpl) * gpl;                                  // first group of the layer
+    if (first[g + 1] - first[g] != first[gl + 1] - first[gl]) { rows_uniform = false; break; }
+    for (uint32_t r = 0; r < first[g + 1] - first[g]; ++r)
+      if (h->y_begin[first[g] + r] != h->y_begin[first[gl] + r] || h->y_end[first[g] + r] != h->y_end[first[gl] + r])
+        rows_uniform = false;
+  }
   // ---- one device block, 256-byte aligned sub-tables ----
   auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
   const size_t sz_id = up(h->id_table_size * 4), sz_s = up(ns * 4), sz_g = up((ng + 1) * 4);
@@ -197,7 +205,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
     return d;
   };
   *out = *h;
-  out->flags = rows_sorted ? UT_GEOM_ROWS_SORTED : 0u;
+  out->flags = (rows_sorted ? UT_GEOM_ROWS_SORTED : 0u) | (rows_uniform ? UT_GEOM_ROWS_UNIFORM : 0u);
   out->id_to_sector = (const uint32_t*)put(h->id_to_sector, h->id_table_size * 4, sz_id);
   out->sector_raw_id = (const uint32_t*)put(h->sector_raw_id, ns * 4, sz_s);
   out->sector_group = (const uint32_t*)put(h->sector_group, ns * 4, sz_s);

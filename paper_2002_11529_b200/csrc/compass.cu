@@ -72,6 +72,7 @@ struct CompassArgs {
   const uint32_t* velo_offsets;
   int32_t n_events;
   uint32_t n_sectors, n_groups, gpl, id_table_size, rows_sorted;
+  uint32_t rows_uniform;               // rows per group when every group of a layer has the same y rows, else 0
   const uint32_t *id_to_sector, *group_first_sector;
   const float *group_xmin, *group_xmax, *sec_yb, *sec_ye, *sec_dxdy, *sec_z, *sec_w;
   float layer_z[4], layer_dxdy[4];
@@ -197,10 +198,12 @@ __device__ __forceinline__ bool cand_insert(const WarpArea& wa, int slot, int& n
 }
 
 // Shared-memory view of one CTA: geometry tables (staged once per CTA) and the current event's hits.
+// (group tables are indexed by g + 2 * layer: the 4 lanes of a track read 4 different bank groups)
 struct SmemView {
-  const float4* gA;      // [ng]  group: xmin, xmax, dxdy, row-hint base (y_hi of the first sector)
-  const uint2* gB;       // [ng]  group: row-hint scale (float bits), first sector | end sector << 16
+  const float4* gA;      // [ng + 8]  group: xmin, xmax, dxdy, row-hint base (y_hi of the first sector)
+  const uint2* gB;       // [ng + 8]  group: row-hint scale (float bits), first sector | end sector << 16
   const float2* lay;     // [4]   layer: group-hint base (xmax of the first group), scale
+  const float2* yr;      // [4][rows] toleranced y range of a row of the layer (rows_uniform geometries)
   const uint32_t* goff;  // [ng + 1] group offsets relative to the event's first hit
   const uint16_t* off;   // [ns + 1] bucketed position of every sector's first hit
   const float* hx;       // x_at_y0, bucketed per sector, x-sorted inside the sector (indexed by `off` positions)
@@ -235,36 +238,56 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
   const int g0 = l * (int)a.gpl, g1 = g0 + (int)a.gpl;
   float* cd = wa.cd + slot * wa.CS;
   uint32_t* chs = wa.chs + slot * wa.CS;
+  const int pad = 2 * l;                            // bank padding of the group tables
   int g;
   {                                                 // first group with group_xmax >= lo
     const float2 hint = S.lay[l];
     const int guess = (int)ceilf((lo - hint.x) * hint.y);
     g = g0 + max(0, min(guess, (int)a.gpl - 1));
-    while (g > g0 && lo <= S.gA[g - 1].y) --g;
-    while (g < g1 && !(lo <= S.gA[g].y)) ++g;
+    while (g > g0 && lo <= S.gA[g - 1 + pad].y) --g;
+    while (g < g1 && !(lo <= S.gA[g + pad].y)) ++g;
+  }
+  // rows_uniform: the sector rows the track crosses, once for all groups of the layer (rows r0 .. r0 + nr - 1)
+  int r0 = 0, nr = 0;
+  if (BUCKETED && a.rows_uniform) {
+    const int R = (int)a.rows_uniform;
+    const float2* yr = S.yr + l * R;
+    const float4 grp0 = S.gA[g0 + pad];
+    const int guess = (int)ceilf((y_e - grp0.w) * __uint_as_float(S.gB[g0 + pad].x));
+    r0 = max(0, min(guess, R - 1));
+    while (r0 > 0 && y_e <= yr[r0 - 1].y) --r0;     // first row with y_e <= y_end + y_tol
+    while (r0 < R && !(y_e <= yr[r0].y)) ++r0;
+    while (r0 + nr < R && yr[r0 + nr].x <= y_e) ++nr;
+    if (nr == 0) return 0;                          // outside every row of the layer
   }
   int n = 0;
   uint32_t last = 0;
   for (; g < g1; ++g) {
-    const float4 grp = S.gA[g];
+    const float4 grp = S.gA[g + pad];
     if (!(grp.x <= hi)) break;
     const uint32_t ga = S.goff[g], gb = S.goff[g + 1];
     if (ga == gb) continue;
     const float syg = __fmul_rn(grp.z, y_e);        // one stereo angle per group (container contract)
     if (BUCKETED) {
-      const uint2 gi = S.gB[g];
-      const int sa = (int)(gi.y & 0xFFFFu), sb = (int)(gi.y >> 16);
-      int s = sa;
-      if (a.rows_sorted) {                          // first sector row with y_e <= y_end + y_tol
+      const uint2 gi = S.gB[g + pad];
+      const int sa = (int)(gi.y & 0xFFFFu);
+      int s = sa, sb = (int)(gi.y >> 16);
+      const bool per_sector_y = a.rows_uniform == 0;
+      if (!per_sector_y) {
+        s = sa + r0;
+        sb = s + nr;
+      } else if (a.rows_sorted) {                   // first sector row with y_e <= y_end + y_tol
         const int guess = (int)ceilf((y_e - grp.w) * __uint_as_float(gi.x));
         s = sa + max(0, min(guess, sb - sa - 1));
         while (s > sa && y_e <= yr_hi(a, s - 1)) --s;
         while (s < sb && !(y_e <= yr_hi(a, s))) ++s;
       }
       for (; s < sb; ++s) {
-        const float2 yr = yr_of(a, s);
-        if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
-        if (!(y_e <= yr.y)) continue;
+        if (per_sector_y) {
+          const float2 yr = yr_of(a, s);
+          if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
+          if (!(y_e <= yr.y)) continue;
+        }
         const uint32_t p1 = S.off[s + 1];
         uint32_t p = S.off[s];
         if (p1 - p > 6u) {                          // busy sector: lower bound of d >= -D
@@ -335,7 +358,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
   return n;
 }
 
-// z of candidate `i` of `slot`
+// z of candidate `i` of `slot` (UNI: every list of the batch has one z, kept per slot)
 template <bool UNI>
 __device__ __forceinline__ float cand_z(const CompassArgs& a, const WarpArea& wa, int slot, int i) {
   return UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * wa.CS + i] & 0xFFFFu));
@@ -455,6 +478,8 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 }
 
 // ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
+// (process_seeds has ONE call site per variant: the kernel's code size decides how well it stays in the
+//  instruction cache)
 template <bool UNI>
 __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
   const int j = lane & 7;
@@ -491,6 +516,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         nBj = 0;
       }
       const int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+      const bool last_chunk = base + 32 >= total;
       for (int ib = 0; ib < maxB; ++ib) {
         // conservative filter: bs and a0 through a reciprocal, accepted with a relative margin that covers the
         // roundings of both evaluations; the exact cuts follow in process_seeds
@@ -502,21 +528,21 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
           pass = fabsf(bsa) <= a.slope_lim && fabsf(da - t) <= __fmaf_rn(kFilterEps, fabsf(t), lim0);
         }
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
-        if (m == 0u) continue;
+        const bool last = last_chunk && ib + 1 >= maxB;
+        if (m == 0u && !last) continue;
         if (pass)
           wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] = ((uint32_t)jj << 10) | (ia << 5) | (uint32_t)ib;
         qn += __popc(m);
-        __syncwarp();
-        if (qn >= 32) {
-          process_seeds<UNI>(a, wa, lane, 32, qhead, dir);
-          qhead += 32;
-          qn -= 32;
+        while (qn >= 32 || (last && qn > 0)) {  // a full queue, or the rest after the last pair
+          __syncwarp();
+          const int cnt = min(qn, 32);
+          process_seeds<UNI>(a, wa, lane, cnt, qhead, dir);
+          qhead += cnt;
+          qn -= cnt;
           __syncwarp();
         }
       }
     }
-    if (qn > 0) process_seeds<UNI>(a, wa, lane, qn, qhead, dir);
-    __syncwarp();
     if (!a.c.both_directions)                   // backward only if nothing valid (A11); else best of both
       todo &= ~__ballot_sync(0xFFFFFFFFu, lane < kTPW && wa.best[j] != kNoKey);
   }
@@ -602,8 +628,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t ng = a.n_groups, ns = a.n_sectors;
   const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
-  float4* s_gA = cvr.take<float4>(ng);
-  uint2* s_gB = cvr.take<uint2>(ng);
+  float4* s_gA = cvr.take<float4>(ng + 8);
+  uint2* s_gB = cvr.take<uint2>(ng + 8);
+  float2* s_yr = cvr.take<float2>(4 * a.rows_uniform);
   uint32_t* s_goff = cvr.take<uint32_t>(ng + 1);
   uint16_t* s_off = cvr.take<uint16_t>(a.soff_stride);
   float* s_hx = cvr.take<float>(a.hit_stage + 8);
@@ -629,8 +656,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
     const float y0 = __fadd_rn(__ldg(a.sec_ye + sa), a.c.y_tol), y1 = __fadd_rn(__ldg(a.sec_ye + sb - 1), a.c.y_tol);
     const float inv = (sb - sa > 1 && y1 > y0) ? (float)(sb - sa - 1) / (y1 - y0) : 0.f;
-    s_gA[g] = make_float4(__ldg(a.group_xmin + g), __ldg(a.group_xmax + g), __ldg(a.sec_dxdy + sa), y0);
-    s_gB[g] = make_uint2(__float_as_uint(inv), sa | (sb << 16));
+    const uint32_t gp = g + 2 * (g / a.gpl);
+    s_gA[gp] = make_float4(__ldg(a.group_xmin + g), __ldg(a.group_xmax + g), __ldg(a.sec_dxdy + sa), y0);
+    s_gB[gp] = make_uint2(__float_as_uint(inv), sa | (sb << 16));
+  }
+  for (uint32_t i = tid; i < 4 * a.rows_uniform; i += nt) {     // y rows of a layer = those of its first group
+    const uint32_t s = __ldg(a.group_first_sector + (i / a.rows_uniform) * a.gpl) + i % a.rows_uniform;
+    s_yr[i] = make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
   }
   if (tid < 4) {
     const uint32_t ga = tid * a.gpl, gb = ga + a.gpl;
@@ -638,7 +670,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     s_lay[tid] = make_float2(x0, (a.gpl > 1 && x1 > x0) ? (float)(a.gpl - 1) / (x1 - x0) : 0.f);
   }
   SmemView S;
-  S.gA = s_gA; S.gB = s_gB; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
+  S.gA = s_gA; S.gB = s_gB; S.yr = s_yr; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
   WarpArea wa;
   {
     const int CS = cand_stride(C);
@@ -742,7 +774,8 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
       }
       for (uint32_t g = warp; g < ng; g += nwarps) {
         const uint32_t ga = s_goff[g], gb = s_goff[g + 1];
-        const uint32_t sa = s_gB[g].y & 0xFFFFu, sb = s_gB[g].y >> 16;
+        const uint32_t gp = g + 2 * (g / a.gpl);
+        const uint32_t sa = s_gB[gp].y & 0xFFFFu, sb = s_gB[gp].y >> 16;
         if (g == ng - 1 && lane == 0) s_off[ns] = (uint16_t)n;
         if (gb - ga <= 64u && sb - sa <= 32u) {
           // one pass, <= 2 hits per lane: rank among the lanes of the same sector (match.any keeps the x
@@ -878,9 +911,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   }
 }
 
-static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t soff_stride, uint32_t hit_stage, int C, int block,
-                                 uint32_t trk_stage = 0) {
-  size_t b = align16((size_t)ng * 16) + align16((size_t)ng * 8);
+static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32_t soff_stride, uint32_t hit_stage, int C,
+                                 int block, uint32_t trk_stage = 0) {
+  size_t b = align16((size_t)(ng + 8) * 16) + align16((size_t)(ng + 8) * 8) + align16((size_t)rows * 32);
   b += align16((ng + 1) * 4) + align16((size_t)soff_stride * 2);
   b += align16((size_t)(hit_stage + 8) * 4) + align16((size_t)(hit_stage + 16) * 2) + align16((size_t)trk_stage * 2);
   b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C)),
@@ -922,6 +955,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.velo_offsets = velo_offsets; a.n_events = n_events;
   a.n_sectors = geom->n_sectors; a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
   a.id_table_size = geom->id_table_size; a.rows_sorted = (geom->flags & UT_GEOM_ROWS_SORTED) ? 1u : 0u;
+  a.rows_uniform = (geom->flags & UT_GEOM_ROWS_UNIFORM) ? geom->n_sectors / geom->n_groups : 0u;
   a.id_to_sector = geom->id_to_sector; a.group_first_sector = geom->group_first_sector;
   a.group_xmin = geom->group_xmin; a.group_xmax = geom->group_xmax;
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
@@ -948,7 +982,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= 768; b += 32) {
-      const size_t sm = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, b) + 1024;
+      const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
@@ -958,21 +992,21 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     if (block <= 0) block = 192;
   }
   block = std::max(32, std::min(768, (block / 32) * 32));
-  size_t smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
+  size_t smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
   while (smem > budget && block > 64) {             // fewer warps before giving up staging
     block -= 32;
-    smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
   }
   while (smem > budget && hit_stage > 0) {
     hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
-    smem = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
   // room for ordering up to 2048 (else 1024, 512) tracks per item, if it costs no resident CTA
   a.trk_stage = 0;
   for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
-    const size_t with = compass_smem_bytes(ns, ng, a.soff_stride, hit_stage, C, block, want);
+    const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, want);
     if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
       a.trk_stage = want;
       smem = with;
