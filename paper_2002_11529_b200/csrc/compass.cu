@@ -87,6 +87,7 @@ struct CompassArgs {
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
   uint32_t split;                      // K: CTAs sharing the tracks of one event
   float slope_lim;                     // max_slope * (1 + kFilterEps): pre-filter limit
+  int32_t interval_min;                // seed partner lists longer than this are searched, not walked
 };
 
 struct FitResult { float chi2, b; bool valid; };
@@ -156,12 +157,13 @@ struct WarpArea {
   int* n;                      // [32] candidates per slot
   float* zs;                   // [32] z of the slot's candidates when they all share one
   float* ws;                   // [32] weight, likewise
+  int* srt;                    // [32] 1: the slot's residuals ascend with the position (kernels with INTERVAL only)
   int CS;
 };
 
 __host__ __device__ inline int cand_stride(int C) { return C | 1; }
 __host__ __device__ inline size_t warp_area_bytes(int C) {
-  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 3;
+  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 4;
 }
 
 // Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
@@ -288,14 +290,46 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
           if (!(yr.x <= y_e)) { if (a.rows_sorted) break; continue; }
           if (!(y_e <= yr.y)) continue;
         }
-        const uint32_t p1 = S.off[s + 1];
+        uint32_t p1 = S.off[s + 1];
         uint32_t p = S.off[s];
         if (p1 - p > 6u) {                          // busy sector: lower bound of d >= -D
           for (uint32_t cnt = p1 - p; cnt > 0;) {
             const uint32_t half = cnt >> 1, mid = p + half;
             if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= negD) cnt = half; else { p = mid + 1; cnt -= half + 1; }
           }
-          if (p1 - p > (uint32_t)C) {
+          if (n == 0 && p1 - p > (uint32_t)C) {
+            // the slot's first run may overflow the cap by itself: of a run that is sorted in d the C closest in
+            // (|d|, index) are a contiguous stretch around the zero crossing.  Find the end of the window, then
+            // grow the stretch from the zero crossing one hit at a time (ties go to the left: lower index), and
+            // let the scan below append exactly that stretch -- no eviction.
+            uint32_t ub = p;
+            for (uint32_t cnt = p1 - p; cnt > 0;) {           // first hit with d > D
+              const uint32_t half = cnt >> 1, mid = ub + half;
+              if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) > D) cnt = half; else { ub = mid + 1; cnt -= half + 1; }
+            }
+            p1 = ub;
+            if (ub - p > (uint32_t)C) {
+              uint32_t zc = p;
+              for (uint32_t cnt = ub - p; cnt > 0;) {         // first hit with d >= 0
+                const uint32_t half = cnt >> 1, mid = zc + half;
+                if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= 0.f) cnt = half; else { zc = mid + 1; cnt -= half + 1; }
+              }
+              uint32_t L = zc, R = zc;                        // the stretch is [L, R)
+              float dl = L > p ? fabsf(__fsub_rn(__fadd_rn(S.hx[L - 1], syg), x_e)) : 0.f;
+              float dr = R < ub ? fabsf(__fsub_rn(__fadd_rn(S.hx[R], syg), x_e)) : 0.f;
+              for (int k = 0; k < C; ++k) {
+                const bool left = L > p && (R >= ub || dl <= dr);
+                if (left) { --L; dl = L > p ? fabsf(__fsub_rn(__fadd_rn(S.hx[L - 1], syg), x_e)) : 0.f; }
+                else { ++R; dr = R < ub ? fabsf(__fsub_rn(__fadd_rn(S.hx[R], syg), x_e)) : 0.f; }
+              }
+              // (equal x across the left cut: the lower index beats the kept one, the C closest are not one
+              //  stretch -- leave the run to the eviction path below)
+              if (!(L > p && S.hx[L - 1] == S.hx[L])) {
+                p = L;
+                p1 = R;
+              }
+            }
+          } else if (p1 - p > (uint32_t)C) {
             // a run that can overflow the cap: of the hits on the negative side only the C next to the zero
             // crossing can be among the C closest (each one further out has C closer hits of this very run in
             // front of it), so the scan starts there instead of evicting its way through the run
@@ -480,7 +514,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 // ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
 // (process_seeds has ONE call site per variant: the kernel's code size decides how well it stays in the
 //  instruction cache)
-template <bool UNI>
+template <bool UNI, bool INTERVAL>
 __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
   const int j = lane & 7;
   const int CS = wa.CS;
@@ -515,20 +549,46 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
       } else {
         nBj = 0;
       }
-      const int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+      int maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+      int ib0 = 0;
+      if (INTERVAL && maxB > a.interval_min && __all_sync(0xFFFFFFFFu, nBj == 0 || wa.srt[sB] != 0)) {
+        // long partner lists that ascend in d (one x-sorted run, or runs of x-disjoint sectors): the partners that
+        // can pass the slope and kink cuts are an interval of d, found by two searches instead of a walk over the
+        // whole list.  [lo, hi] contains every db the cuts accept (real arithmetic widened by 1e-5 relative; a NaN
+        // bound opens the interval), the filter below and the exact cuts still decide.
+        const float dz = wa.zs[sB] - za, sdz = a.slope_lim * fabsf(dz);
+        const float rho = zam * rinv, rr = rcp_approx(rho);
+        const float k1 = a.c.kink_tol * (1.f + 1e-5f);
+        const float qa = (da - k1) * rr, qb = (da + k1) * rr;
+        float lo = fmaxf(da - sdz, da + fminf(qa, qb)), hi = fminf(da + sdz, da + fmaxf(qa, qb));
+        const float mg = 1e-5f * (fabsf(da) + fabsf(lo) + fabsf(hi)) + 1e-6f;
+        lo -= mg; hi += mg;
+        if (!(fabsf(rho) > 1e-12f) || !(lo == lo) || !(hi == hi)) { lo = -__int_as_float(0x7F800000); hi = -lo; }
+        int plo = 0, phi = 0;
+#pragma unroll
+        for (int step = 32; step > 0; step >>= 1) {
+          const int q1 = plo + step, q2 = phi + step;
+          if (q1 <= nBj && cB[q1 - 1] < lo) plo = q1;           // first partner with d >= lo
+          if (q2 <= nBj && cB[q2 - 1] <= hi) phi = q2;          // first partner with d > hi
+        }
+        ib0 = plo;
+        nBj = max(phi - plo, 0);
+        maxB = __reduce_max_sync(0xFFFFFFFFu, nBj);
+      }
       const bool last_chunk = base + 32 >= total;
-      for (int ib = 0; ib < maxB; ++ib) {
+      for (int ik = 0; ik < (INTERVAL ? max(maxB, last_chunk ? 1 : 0) : maxB); ++ik) {
         // conservative filter: bs and a0 through a reciprocal, accepted with a relative margin that covers the
         // roundings of both evaluations; the exact cuts follow in process_seeds
         bool pass = false;
-        if (ib < nBj) {
+        const int ib = INTERVAL ? ib0 + ik : ik;
+        if (ik < nBj) {
           if (!UNI) rinv = rcp_approx(cand_z<false>(a, wa, sB, ib) - za);
           const float bsa = (cB[ib] - da) * rinv;
           const float t = bsa * zam;
           pass = fabsf(bsa) <= a.slope_lim && fabsf(da - t) <= __fmaf_rn(kFilterEps, fabsf(t), lim0);
         }
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, pass);
-        const bool last = last_chunk && ib + 1 >= maxB;
+        const bool last = last_chunk && ik + 1 >= maxB;
         if (m == 0u && !last) continue;
         if (pass)
           wa.seedq[(qhead + qn + __popc(m & lt_mask)) & (kSeedQ - 1)] = ((uint32_t)jj << 10) | (ia << 5) | (uint32_t)ib;
@@ -549,7 +609,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
 }
 
 // The warps of the CTA pull 8-track batches of the item: track m of the item is VELO track t0 + m * K + part.
-template <bool BUCKETED>
+template <bool BUCKETED, bool INTERVAL>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
                                            uint32_t h0, uint32_t t0, uint32_t nTk, uint32_t part, uint32_t T,
                                            const uint16_t* perm) {
@@ -578,13 +638,21 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     wa.n[lane] = n_st;
     wa.zs[lane] = zu;
     wa.ws[lane] = wu;
+    // long lists that ascend in d (one x-sorted run, or runs of x-disjoint sectors) are searched, not walked
+    if (INTERVAL && __any_sync(0xFFFFFFFFu, n_st > a.interval_min)) {
+      int srt = 1;
+      const float* cdl = wa.cd + lane * CS;
+      for (int i = 1; i < n_st; ++i) srt &= cdl[i] >= cdl[i - 1] ? 1 : 0;
+      wa.srt[lane] = srt;
+    }
     if (lane < kTPW) wa.best[lane] = kNoKey;
     const bool uni = __all_sync(0xFFFFFFFFu, zu == zu);      // every list of the batch has one z and one weight
     __syncwarp();
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
     const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    if (uni) find_tracklets<true>(a, wa, lane, todo); else find_tracklets<false>(a, wa, lane, todo);
+    if (uni) find_tracklets<true, INTERVAL>(a, wa, lane, todo);
+    else find_tracklets<false, false>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
       const int q4 = lane & ~3;
@@ -621,7 +689,9 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
 }
 
 // One CTA works through work items (event, part) handed out by the ticket.  Geometry tables are staged once.
-template <int MAXT, int MINB>
+// INTERVAL: the seed search of long, d-sorted partner lists by interval (worth its code only when
+// max_candidates_per_layer allows long lists; the kernel without it is the faster one for short lists).
+template <int MAXT, int MINB, bool INTERVAL>
 __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -684,6 +754,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     wa.n = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4);
     wa.zs = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 4);
     wa.ws = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 8);
+    wa.srt = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 12);
   }
   const uint32_t Tend = __ldg(a.velo_offsets + a.n_events);
   const uint32_t T = a.idx_stride ? a.idx_stride : Tend;
@@ -900,9 +971,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     __syncthreads();                               // order and staged data visible; scratch is dead from here on
     if (staged) {
-      track_loop<true>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<true, INTERVAL>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<false, INTERVAL>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     }
   }
   if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
@@ -925,8 +996,11 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32
 // Two register budgets: CTAs of <= 224 threads at 4 per SM (72 registers), and larger CTAs (big events / C = 32,
 // where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
 constexpr int kSmallBlock = 224;
-static const void* const kKernelSmall = reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4>);
-static const void* const kKernelLarge = reinterpret_cast<const void*>(&compass_kernel<768, 1>);
+static const void* const kKernels[2][2] = {
+    {reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4, false>),
+     reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4, true>)},
+    {reinterpret_cast<const void*>(&compass_kernel<768, 1, false>),
+     reinterpret_cast<const void*>(&compass_kernel<768, 1, true>)}};
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
@@ -934,11 +1008,13 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   DeviceInfo dev;
   int max_smem = 0, max_smem_large = 0;               // largest dynamic size a CTA may ask for on this device
   if (const int32_t rc = device_info(&dev)) return rc;
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernelSmall, kSlotCompassSmall, &max_smem)) return rc;
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernelLarge, kSlotCompassLarge, &max_smem_large)) return rc;
+  const ut_tuning tune = tuning_snapshot();
+  const int interval_min = tuned(tune.compass_interval_min, 16);
+  const int iv = cfg->max_candidates_per_layer > interval_min ? 1 : 0;    // long partner lists are possible
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[0][iv], kSlotCompassSmall + iv, &max_smem)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[1][iv], kSlotCompassLarge + iv, &max_smem_large)) return rc;
   max_smem = std::min(max_smem, max_smem_large);
   const int n_sm = dev.n_sm, sm_smem = dev.smem_per_sm;
-  const ut_tuning tune = tuning_snapshot();
   const ut_geometry* geom = hits->geom;
   CompassArgs a;
   a.hx = hits->x_at_y0; a.hid = hits->id; a.hyb = hits->y_begin; a.hye = hits->y_end;
@@ -962,6 +1038,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
   a.slope_lim = cfg->max_slope * (1.0f + kFilterEps);
+  a.interval_min = iv ? std::min(interval_min, 8) : interval_min;     // inside the interval kernel the search pays from ~8 partners
   a.idx_stride = idx_stride;
   a.capacity = hits->capacity;
   a.bulk_ok = ((reinterpret_cast<uintptr_t>(hits->x_at_y0) | reinterpret_cast<uintptr_t>(hits->id)) & 15u) == 0 ? 1u : 0u;
@@ -1013,7 +1090,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
       break;
     }
   }
-  const void* kernel = block <= kSmallBlock ? kKernelSmall : kKernelLarge;
+  const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv];
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
   if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);
