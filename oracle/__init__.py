@@ -67,6 +67,8 @@ def _load():
             lib.oracle_compass.restype = C.c_int32
             lib.oracle_fit.restype = C.c_int32
             lib.oracle_consolidate.restype = C.c_int32
+            lib.oracle_search_windows.restype = C.c_int32
+            lib.oracle_compass_from_windows.restype = C.c_int32
             _lib = lib
     return _lib
 
@@ -239,3 +241,49 @@ def consolidate(hit_idx, n_hits, qop, chi2, velo_offsets, n_events: int, capacit
         raise RuntimeError(f"oracle_consolidate rc={rc}")
     K = min(int(off[-1]), cap)
     return CompactTracks(o_v[:K], o_i[:, :K] if cap else o_i[:, :0], o_n[:K], o_q[:K], o_c[:K], off, int(st.value))
+
+
+def search_windows(hits: Hits, velo_x, velo_y, velo_tx, velo_ty, velo_z: float, velo_offsets, n_events: int, geom,
+                   params, n_sectors_search: int):
+    """PAPER.md:286-322 as the plain definition: window ranges as signed 16-bit (begin, size)
+    per track x panel x {1, 3, 5} sector groups in the layout of Fig. 7: i16 [T, 4, 2W] (W begins, then W sizes;
+    begin relative to the event's first hit; (-1, -1) = no hits).  Returns (windows, status)."""
+    lib = _load()
+    W = int(n_sectors_search)
+    velo_offsets = np.ascontiguousarray(velo_offsets, dtype=np.uint32)
+    T = int(velo_offsets[n_events])
+    win = np.full((max(T, 1), 4, 2 * W), -9, np.int16)
+    gs, keep = _geom_struct(geom)
+    cs = _config_struct(params)
+    hs = hits._struct()
+    st = C.c_uint32(0)
+    f = lambda a: _p(np.ascontiguousarray(a, np.float32))
+    rc = lib.oracle_search_windows(C.byref(hs), _p(hits.hit_offsets), f(velo_x), f(velo_y), f(velo_tx), f(velo_ty),
+                                   C.c_float(velo_z), _p(velo_offsets), C.c_int32(n_events), C.byref(gs), C.byref(cs),
+                                   C.c_int32(W), _p(win), C.byref(st))
+    if rc != 0:
+        raise RuntimeError(f"oracle_search_windows rc={rc}")
+    return win[:T], int(st.value)
+
+
+def compass_from_windows(hits: Hits, windows, velo_x, velo_y, velo_tx, velo_ty, velo_z: float, velo_offsets,
+                         n_events: int, geom, params, n_sectors_search: int) -> Tracks:
+    """PAPER.md:324-348 from stored window ranges.  cand_n = candidates per layer before the cap."""
+    lib = _load()
+    W = int(n_sectors_search)
+    velo_offsets = np.ascontiguousarray(velo_offsets, dtype=np.uint32)
+    T = int(velo_offsets[n_events])
+    out = Tracks(np.full((4, T), -1, np.int32), np.zeros(T, np.int32), np.zeros(T, np.float32), np.zeros(T, np.float32),
+                 None, np.zeros((T, 4), np.int32), None, None)
+    gs, keep = _geom_struct(geom)
+    cs = _config_struct(params)
+    hs = hits._struct()
+    win = np.ascontiguousarray(windows, np.int16)
+    f = lambda a: _p(np.ascontiguousarray(a, np.float32))
+    rc = lib.oracle_compass_from_windows(C.byref(hs), _p(hits.hit_offsets), f(velo_x), f(velo_y), f(velo_tx), f(velo_ty),
+                                         C.c_float(velo_z), _p(velo_offsets), C.c_int32(n_events), C.byref(gs),
+                                         C.byref(cs), C.c_int32(W), _p(win), _p(out.hit_idx), _p(out.n_hits), _p(out.qop),
+                                         _p(out.chi2), _p(out.cand_n))
+    if rc != 0:
+        raise RuntimeError(f"oracle_compass_from_windows rc={rc}")
+    return out

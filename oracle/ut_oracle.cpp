@@ -427,6 +427,138 @@ int32_t oracle_compass(int32_t mode, const oracle_hits* hits, const uint32_t* hi
   return 0;
 }
 
+// ---------------------------------------------------------------------------------------
+// the paper's two-kernel layout (Fig. 7) as plain definitions.
+//
+// "Search UT windows": per VELO track and panel (layer), the sector group the extrapolation
+// points to and its neighbours (W = 1, 3 or 5 groups in all: the central one, then -1, +1, -2, +2; PAPER.md:300,
+// :332); in each the window range = the hits of the group's x-sorted run with |d| <= win_half[l], found by two
+// searches on the monotone residual and nothing else ("only two pointers to the hits").  The y
+// test is left to the tracklet step ("has to still be performed again in the tracking kernel").
+// Stored as Fig. 7 draws it: per track, per panel, W begin indices then W sizes, signed 16-bit, the begin
+// relative to the first hit of the track's event; an empty or missing range is (-1, -1).
+// Central group (A23): the first group of the layer with group_xmax >= c, c = x_e - layer_dxdy*y_e
+// (the last group if there is none).  Events of more than 32767 hits cannot be indexed by a short: all their
+// ranges are (-1, -1) and status bit 32 is set.
+// ---------------------------------------------------------------------------------------
+static int central_group(const oracle_geometry* g, int l, float c) {
+  const int gpl = (int)(g->n_groups / g->n_layers);
+  for (int k = 0; k < gpl; ++k)
+    if (g->group_xmax[l * gpl + k] >= c) return l * gpl + k;
+  return l * gpl + gpl - 1;
+}
+static int slot_group(const oracle_geometry* g, int l, int central, int k) {      // k-th range: 0, -1, +1, -2, +2
+  const int gpl = (int)(g->n_groups / g->n_layers);
+  const int off = k == 0 ? 0 : (k % 2 == 1 ? -((k + 1) / 2) : k / 2);
+  const int gi = central + off;
+  return (gi < l * gpl || gi >= (l + 1) * gpl) ? -1 : gi;
+}
+
+int32_t oracle_search_windows(const oracle_hits* hits, const uint32_t* hit_offsets, const float* vx, const float* vy,
+                              const float* vtx, const float* vty, float vz, const uint32_t* velo_offsets,
+                              int32_t n_events, const oracle_geometry* g, const oracle_config* c, int32_t W,
+                              int16_t* windows /* [T][4][2W] */, uint32_t* status) {
+  if (!hits || !hit_offsets || !velo_offsets || !g || !c || !windows || n_events < 0) return -1;
+  if (W != 1 && W != 3 && W != 5) return -2;
+  const HitsView H{hits->x_at_y0, hits->z_at_y0, hits->y_begin, hits->y_end, hits->dxdy, hits->weight};
+  uint32_t st = 0;
+  for (int32_t e = 0; e < n_events; ++e) {
+    const uint32_t* goff = hit_offsets + (uint64_t)e * g->n_groups;
+    const int64_t ev0 = goff[0], ev1 = goff[g->n_groups];
+    const bool too_large = ev1 - ev0 > 32767;
+    if (too_large) st |= 32u;
+    for (int64_t t = velo_offsets[e]; t < (int64_t)velo_offsets[e + 1]; ++t) {
+      for (int l = 0; l < 4; ++l) {
+        int16_t* w = windows + (t * 4 + l) * 2 * W;
+        const float dzv = g->layer_z[l] - vz;
+        const float x_e = vx[t] + vtx[t] * dzv;
+        const float y_e = vy[t] + vty[t] * dzv;
+        const float D = c->win_half[l];
+        const float sy = g->layer_dxdy[l] * y_e;
+        const int central = central_group(g, l, x_e - sy);
+        for (int k = 0; k < W; ++k) {
+          w[k] = -1; w[W + k] = -1;
+          const int gi = slot_group(g, l, central, k);
+          if (gi < 0 || too_large) continue;
+          int64_t first = goff[gi], n = (int64_t)goff[gi + 1] - first;        // first hit with d >= -D
+          while (n > 0) {
+            const int64_t half = n / 2, mid = first + half;
+            if (resid(H, mid, x_e, y_e) >= -D) n = half; else { first = mid + 1; n -= half + 1; }
+          }
+          int64_t last = first;                                                // first hit with d > D
+          n = (int64_t)goff[gi + 1] - last;
+          while (n > 0) {
+            const int64_t half = n / 2, mid = last + half;
+            if (resid(H, mid, x_e, y_e) > D) n = half; else { last = mid + 1; n -= half + 1; }
+          }
+          if (last > first) { w[k] = (int16_t)(first - ev0); w[W + k] = (int16_t)(last - first); }
+        }
+      }
+    }
+  }
+  if (status) *status = st;
+  return 0;
+}
+
+// "Tracklet finding" from stored window ranges: the candidates of a layer are the hits of its
+// W ranges that pass the y test, capped and ordered as step 3; steps 4-7 as oracle_compass.
+int32_t oracle_compass_from_windows(const oracle_hits* hits, const uint32_t* hit_offsets, const float* vx,
+                                    const float* vy, const float* vtx, const float* vty, float vz,
+                                    const uint32_t* velo_offsets, int32_t n_events, const oracle_geometry* g,
+                                    const oracle_config* c, int32_t W, const int16_t* windows, int32_t* out_hit_idx,
+                                    int32_t* out_n_hits, float* out_qop, float* out_chi2, int32_t* cand_n /* [T][4] or null */) {
+  if (!hits || !hit_offsets || !velo_offsets || !g || !c || !windows || n_events < 0) return -1;
+  if ((W != 1 && W != 3 && W != 5) || (c->min_hits != 3 && c->min_hits != 4) || c->max_candidates_per_layer < 1) return -2;
+  const HitsView H{hits->x_at_y0, hits->z_at_y0, hits->y_begin, hits->y_end, hits->dxdy, hits->weight};
+  const int64_t T = velo_offsets[n_events];
+  std::vector<Cand> cand[4];
+  for (int32_t e = 0; e < n_events; ++e) {
+    const int64_t ev0 = hit_offsets[(uint64_t)e * g->n_groups];
+    for (int64_t t = velo_offsets[e]; t < (int64_t)velo_offsets[e + 1]; ++t) {
+      int nonempty = 0;
+      for (int l = 0; l < 4; ++l) {
+        const int16_t* w = windows + (t * 4 + l) * 2 * W;
+        const float dzv = g->layer_z[l] - vz;
+        const float x_e = vx[t] + vtx[t] * dzv;
+        const float y_e = vy[t] + vty[t] * dzv;
+        cand[l].clear();
+        for (int k = 0; k < W; ++k) {
+          if (w[W + k] <= 0) continue;                                       // (-1, -1): no hits
+          for (int64_t h = ev0 + w[k]; h < ev0 + w[k] + w[W + k]; ++h) {
+            const float d = resid(H, h, x_e, y_e);
+            if (std::fabs(d) <= c->win_half[l] && y_ok(H, h, y_e, c->y_tol)) cand[l].push_back(Cand{(int32_t)h, d, H.z[h], H.w[h]});
+          }
+        }
+        std::sort(cand[l].begin(), cand[l].end(), [](const Cand& a, const Cand& b) { return a.h < b.h; });
+        if (cand_n) cand_n[t * 4 + l] = (int32_t)cand[l].size();
+        const size_t C = (size_t)c->max_candidates_per_layer;
+        if (cand[l].size() > C) {                                           // step 3
+          std::sort(cand[l].begin(), cand[l].end(), [](const Cand& a, const Cand& b) {
+            const float fa = std::fabs(a.d), fb = std::fabs(b.d);
+            return fa < fb || (fa == fb && a.h < b.h);
+          });
+          cand[l].resize(C);
+          std::sort(cand[l].begin(), cand[l].end(), [](const Cand& a, const Cand& b) { return a.h < b.h; });
+        }
+        if (!cand[l].empty()) ++nonempty;
+      }
+      Best result;
+      if (nonempty >= c->min_hits) {
+        Best fwd, bwd;
+        search_direction(cand, 0, 2, 1, 3, c, fwd);
+        if (c->both_directions || !fwd.best.valid) search_direction(cand, 3, 1, 2, 0, c, bwd);
+        result = combine_directions(fwd, bwd, c->both_directions != 0);
+      }
+      const Tracklet& b = result.best;
+      for (int l = 0; l < 4; ++l) out_hit_idx[(int64_t)l * T + t] = b.valid ? b.h[l] : -1;
+      out_n_hits[t] = b.valid ? b.n : 0;
+      out_qop[t] = b.valid ? b.qop : 0.f;
+      out_chi2[t] = b.valid ? b.chi2 : 0.f;
+    }
+  }
+  return 0;
+}
+
 // The fit alone, for the lstsq / collinear pins: n points (layer order), returns a, b, chi2.
 int32_t oracle_fit(int32_t n, const float* d, const float* z, const float* w, const oracle_config* c,
                    float* a_out, float* b_out, float* chi2_out, float* qop_out) {
