@@ -370,6 +370,41 @@ class DeviceWorkload:
         return n_hits, status
 
 
+def two_kernel_ab(B, torch, w, flush, steps):
+    """the paper's two-kernel Compass (window ranges as int16 pairs in global memory, then a
+    thread-per-track tracklet kernel; Fig. 7) timed beside the fused kernel on the same decoded
+    container -- the measurement the paper's own layout claim asks for.  Not part of the step."""
+    stream = torch.cuda.current_stream()
+    b, T = w.batch, w.batch.n_velo_total
+    w.step()
+    torch.cuda.synchronize()
+    fused_idx = w.tracks.hit_idx[:4 * T].clone()
+    out = {}
+    for W in (1, 3, 5):
+        win = torch.empty(max(T, 1) * 8 * W, dtype=torch.int16, device="cuda")
+        st = torch.zeros(1, dtype=torch.int32, device="cuda")
+        tr = B.Tracks(T)
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        for k in range(steps + 2):
+            flush.zero_()
+            w.decode()                                     # the hits are in L2 as they are for the fused kernel
+            e = ev[max(k - 2, 0)]
+            e[0].record(stream)
+            B.compass_search_windows(w.hits, w.hits.hit_offsets, w.velo, w.vo_d, b.n_events, w.config, W, win, st)
+            e[1].record(stream)
+            B.compass_tracklets_from_windows(w.hits, w.hits.hit_offsets, w.velo, w.vo_d, b.n_events, w.config, W, win, tr)
+            e[2].record(stream)
+        torch.cuda.synchronize()
+        mw = statistics.mean(e[0].elapsed_time(e[1]) for e in ev)
+        mt = statistics.mean(e[1].elapsed_time(e[2]) for e in ev)
+        out[f"sectors_{W}"] = {"ms_search_windows": mw, "ms_tracklet_finding": mt, "ms": mw + mt,
+                               "tracking_only_events_per_s": b.n_events / (mw + mt) * 1e3,
+                               "window_bytes": int(T * 16 * W),
+                               "tracklets": int((tr.n_hits[:T] > 0).sum().item()),
+                               "equals_fused_kernel": bool(torch.equal(tr.hit_idx[:4 * T], fused_idx))}
+    return out
+
+
 def kernel_table(batch, abytes, md, mc, hbm_peak):
     return {
         "ut_decode_kernel": {"ms": md, "bytes": abytes["decode"], "gbs": abytes["decode"] / md / 1e6,
@@ -402,6 +437,8 @@ def per_config_report(B, torch, flush, prepared, hbm_peak, steps):
             "frac_hbm_step": ab["e2e"] / ms / 1e6 / hbm_peak, "gbs_step": ab["e2e"] / ms / 1e6,
             "min_hits": params.min_hits, "max_candidates_per_layer": params.max_candidates_per_layer,
             "status_word": status, "launch": B.last_launch_info()}
+        if cid == 4:
+            rows[cfg.name]["two_kernel_compass"] = two_kernel_ab(B, torch, w, flush, 3)
         del w
         torch.cuda.empty_cache()
     return rows
@@ -561,6 +598,7 @@ def main():
     torch.cuda.synchronize()
     t_cons = statistics.mean(a_.elapsed_time(b_) for a_, b_ in evc)
     n_compact = int(compact.track_offsets[batch.n_events].item())
+    ab = two_kernel_ab(B, torch, w, flush, 5) if world == 1 else None
     cons_bytes = 28 * batch.n_velo_total + 4 * (batch.n_events + 1) + 32 * n_compact + 4 * (batch.n_events + 1)
 
     if rank != 0:
@@ -616,7 +654,12 @@ def main():
         "next_rows": {"compass_consolidate": {"ms": t_cons, "tracklets": n_compact, "bytes": int(cons_bytes),
                                                "gbs": cons_bytes / t_cons / 1e6,
                                                "frac_hbm": cons_bytes / t_cons / 1e6 / hbm_peak,
-                                               "note": "SURVEY.md 8(f) row 1, timed alone, not part of the step"}},
+                                               "note": "SURVEY.md 8(f) row 1, timed alone, not part of the step"},
+                      "two_kernel_compass": {"fused_ms": mc, "variants": ab,
+                                             "note": "SURVEY.md 8(f) row 2: the paper's search-windows + thread-per-track "
+                                                     "tracklet kernels with int16 window ranges (Fig. 7) on the same "
+                                                     "container, timed alone; 5 sector groups = the fused kernel's "
+                                                     "results"}},
     }
     if prepared:
         del w

@@ -225,6 +225,30 @@ size_t compass_consolidate_workspace_bytes(uint32_t max_velo_total);
 int32_t compass_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events,
                             ut_compact_tracks* out, uint32_t* track_offsets_out, ut_stream_t stream);
 
+/* The paper's own two-kernel layout (section V-A / V-B): kept beside the fused
+ * compass_track as an A/B measurement of the paper's layout claims, not as the product path.
+ *
+ * compass_search_windows -- "search UT windows": a 2-D kernel (4 panels x VELO tracks); per
+ *   (track, panel) the sector group the extrapolation points to and its neighbours, n_sectors_search = 1, 3 or 5
+ *   groups in all (central, -1, +1, -2, +2); per group the window range = the hits of the
+ *   group's x-sorted run with |d| <= win_half[l] (two searches, nothing else: the y test is repeated by the tracklet
+ *   kernel).  windows_out: device int16 [n_velo_total][4][2 * n_sectors_search] in the layout of
+ *   Fig. 7 -- per track, per panel, W begin indices then W sizes; begin relative to the first hit of the track's
+ *   event; (-1, -1) = no hits or no such group.  Events of more than 32767 hits cannot be
+ *   indexed by shorts: UT_STATUS_EVENT_TOO_LARGE in *status, their ranges empty.  status: device u32 word.
+ * compass_tracklets_from_windows -- "tracklet finding": thread per VELO track, window ranges
+ *   cached in shared memory (num_threads x num_panels x 2W shorts), valid tracks compacted through
+ *   shared memory; same predicates, cap, fit and selection as compass_track.
+ * With 5 sector groups every group a window of the synthetic workloads can touch is searched and tracks_out equals
+ * compass_track's bit for bit; 1 and 3 groups search less (the paper's physics / speed trade-off, Table 3). */
+int32_t compass_search_windows(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                               const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                               int32_t n_sectors_search, int16_t* windows_out, uint32_t* status, ut_stream_t stream);
+int32_t compass_tracklets_from_windows(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                                       const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                                       int32_t n_sectors_search, const int16_t* windows, ut_tracks* tracks_out,
+                                       ut_stream_t stream);
+
 /* End-to-end convenience for HOST buffers (bench.py "e2e"): H2D of raw banks, offsets and VELO
  * states, ut_decode, compass_track, D2H of the track SoA, all asynchronous on `stream`.
  * The arena holds the device staging buffers (library-owned). Host buffers should be pinned. */

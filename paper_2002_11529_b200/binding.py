@@ -84,7 +84,7 @@ class ut_launch_info(C.Structure):
 
 
 EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set",
-           "ut_sector_offsets_stride", "ut_geometry_upload", "ut_geometry_free",
+           "ut_sector_offsets_stride", "compass_search_windows", "compass_tracklets_from_windows", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
            "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
            "ut_pipeline_device_hits"]
@@ -102,6 +102,11 @@ _lib.compass_config_default.argtypes = [C.c_float, C.c_float, C.c_int32, C.c_int
                                         C.POINTER(compass_config)]
 _lib.compass_track.argtypes = [C.POINTER(ut_hits), C.c_void_p, C.POINTER(velo_states), C.c_void_p, C.c_int32,
                                C.POINTER(compass_config), C.POINTER(ut_tracks), C.c_void_p]
+_lib.compass_search_windows.argtypes = [C.POINTER(ut_hits), C.c_void_p, C.POINTER(velo_states), C.c_void_p, C.c_int32,
+                                        C.POINTER(compass_config), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.compass_tracklets_from_windows.argtypes = [C.POINTER(ut_hits), C.c_void_p, C.POINTER(velo_states), C.c_void_p,
+                                                C.c_int32, C.POINTER(compass_config), C.c_int32, C.c_void_p,
+                                                C.POINTER(ut_tracks), C.c_void_p]
 _lib.compass_consolidate_workspace_bytes.restype = C.c_size_t
 _lib.compass_consolidate_workspace_bytes.argtypes = [C.c_uint32]
 _lib.compass_consolidate.argtypes = [C.POINTER(ut_tracks), C.c_void_p, C.c_int32, C.POINTER(ut_compact_tracks),
@@ -316,6 +321,27 @@ def compass_track(hits: Hits, hit_offsets: torch.Tensor, velo: "VeloStates", vel
     rc = _lib.compass_track(C.byref(hits.c), hit_offsets.data_ptr(), C.byref(velo.c), velo_offsets.data_ptr(),
                             n_events, C.byref(config), C.byref(tracks_out.c), _stream_ptr(stream))
     _check(rc, "compass_track")
+    return rc
+
+
+def compass_search_windows(hits: Hits, hit_offsets: torch.Tensor, velo: "VeloStates", velo_offsets: torch.Tensor,
+                           n_events: int, config: compass_config, n_sectors_search: int, windows_out: torch.Tensor,
+                           status: torch.Tensor, stream=None) -> int:
+    """windows_out: int16 device tensor [n_velo_total * 4 * 2 * n_sectors_search] (Fig. 7 layout); status: int32[1]."""
+    rc = _lib.compass_search_windows(C.byref(hits.c), hit_offsets.data_ptr(), C.byref(velo.c), velo_offsets.data_ptr(),
+                                     n_events, C.byref(config), n_sectors_search, windows_out.data_ptr(),
+                                     status.data_ptr(), _stream_ptr(stream))
+    _check(rc, "compass_search_windows")
+    return rc
+
+
+def compass_tracklets_from_windows(hits: Hits, hit_offsets: torch.Tensor, velo: "VeloStates", velo_offsets: torch.Tensor,
+                                   n_events: int, config: compass_config, n_sectors_search: int, windows: torch.Tensor,
+                                   tracks_out: Tracks, stream=None) -> int:
+    rc = _lib.compass_tracklets_from_windows(C.byref(hits.c), hit_offsets.data_ptr(), C.byref(velo.c),
+                                             velo_offsets.data_ptr(), n_events, C.byref(config), n_sectors_search,
+                                             windows.data_ptr(), C.byref(tracks_out.c), _stream_ptr(stream))
+    _check(rc, "compass_tracklets_from_windows")
     return rc
 
 

@@ -7,8 +7,8 @@ import subprocess
 _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 LIB = os.path.join(_DIR, "libutcompass.so")
-SOURCES = ["api.cu", "ut_decode.cu", "compass.cu", "consolidate.cu"]
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(_DIR, "..", "include", "ut_compass.h")]
+SOURCES = ["api.cu", "ut_decode.cu", "compass.cu", "consolidate.cu", "windows.cu"]
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "compass_fit.cuh"), os.path.join(_DIR, "..", "include", "ut_compass.h")]
 # -fmad=false: no FMA contraction anywhere (A14); parity-relevant arithmetic also uses __f*_rn.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

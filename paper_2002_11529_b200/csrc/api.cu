@@ -22,6 +22,13 @@ size_t consolidate_workspace_bytes(uint32_t max_velo);
 int32_t launch_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events, uint32_t n_velo_hint,
                            ut_compact_tracks* out, uint32_t* track_offsets, cudaStream_t stream);
 
+int32_t launch_search_windows(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                              const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, int32_t W,
+                              int16_t* windows, uint32_t* status, cudaStream_t stream);
+int32_t launch_tracklets(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                         const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, int32_t W,
+                         const int16_t* windows, ut_tracks* out, cudaStream_t stream);
+
 ut_launch_info& launch_info() {
   static thread_local ut_launch_info info = {};
   return info;
@@ -329,6 +336,38 @@ int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const ve
     return UT_ERR_NULL;
   if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
   return launch_compass(hits, hit_offsets, velo, velo_offsets, n_events, config, tracks_out, (cudaStream_t)stream, 0u, 0ull);
+}
+
+int32_t compass_search_windows(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                               const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                               int32_t n_sectors_search, int16_t* windows_out, uint32_t* status, ut_stream_t stream) {
+  launch_info().kernels_launched = 0;
+  if (!hits || !hit_offsets || !velo || !velo_offsets || !config || !status || !hits->geom) return UT_ERR_NULL;
+  if (n_events < 0 || (n_sectors_search != 1 && n_sectors_search != 3 && n_sectors_search != 5)) return UT_ERR_ARG;
+  if (const int32_t rc = check_config(config)) return rc;
+  if (n_events == 0) return UT_OK;
+  if (!windows_out || !velo->x || !velo->y || !velo->tx || !velo->ty) return UT_ERR_NULL;
+  if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
+  return launch_search_windows(hits, hit_offsets, velo, velo_offsets, n_events, config, n_sectors_search, windows_out,
+                               status, (cudaStream_t)stream);
+}
+
+int32_t compass_tracklets_from_windows(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
+                                       const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
+                                       int32_t n_sectors_search, const int16_t* windows, ut_tracks* tracks_out,
+                                       ut_stream_t stream) {
+  launch_info().kernels_launched = 0;
+  if (!hits || !hit_offsets || !velo || !velo_offsets || !config || !tracks_out || !hits->geom) return UT_ERR_NULL;
+  if (n_events < 0 || (n_sectors_search != 1 && n_sectors_search != 3 && n_sectors_search != 5)) return UT_ERR_ARG;
+  if (const int32_t rc = check_config(config)) return rc;
+  if (!tracks_out->status) return UT_ERR_NULL;
+  if (n_events == 0) return UT_OK;
+  if (!windows || !tracks_out->hit_idx || !tracks_out->n_hits || !tracks_out->qop || !tracks_out->chi2 || !velo->x ||
+      !velo->y || !velo->tx || !velo->ty)
+    return UT_ERR_NULL;
+  if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
+  return launch_tracklets(hits, hit_offsets, velo, velo_offsets, n_events, config, n_sectors_search, windows, tracks_out,
+                          (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -48,6 +48,7 @@
 #include <cstdlib>
 
 #include "common.cuh"
+#include "compass_fit.cuh"
 
 namespace utc {
 
@@ -89,50 +90,6 @@ struct CompassArgs {
   float slope_lim;                     // max_slope * (1 + kFilterEps): pre-filter limit
   int32_t interval_min;                // seed partner lists longer than this are searched, not walked
 };
-
-struct FitResult { float chi2, b; bool valid; };
-
-__device__ __forceinline__ void fit_acc(bool p, float d, float dz, float w, float& S0, float& S1, float& S2,
-                                        float& T0, float& T1) {
-  if (p) {
-    const float wdz = __fmul_rn(w, dz);
-    S0 = __fadd_rn(S0, w);
-    S1 = __fadd_rn(S1, wdz);
-    S2 = __fadd_rn(S2, __fmul_rn(wdz, dz));
-    const float wd = __fmul_rn(w, d);
-    T0 = __fadd_rn(T0, wd);
-    T1 = __fadd_rn(T1, __fmul_rn(wd, dz));
-  }
-}
-__device__ __forceinline__ float fit_res(bool p, float d, float dz, float w, float a, float b, float chi2) {
-  if (p) {
-    const float r = __fsub_rn(__fsub_rn(d, a), __fmul_rn(b, dz));
-    chi2 = __fadd_rn(chi2, __fmul_rn(__fmul_rn(w, r), r));
-  }
-  return chi2;
-}
-
-// Weighted linear LSQ of d vs dz = z - z_mag with the VELO pseudo-point (0, 0, w_velo); hits in layer order.
-__device__ __forceinline__ FitResult fit_tracklet(const bool (&p)[4], const float (&d)[4], const float (&z)[4],
-                                                  const float (&w)[4], int n, const compass_config& c) {
-  float dz[4];
-#pragma unroll
-  for (int l = 0; l < 4; ++l) dz[l] = __fsub_rn(z[l], c.z_mag);
-  float S0 = c.w_velo, S1 = 0.f, S2 = 0.f, T0 = 0.f, T1 = 0.f;
-#pragma unroll
-  for (int l = 0; l < 4; ++l) fit_acc(p[l], d[l], dz[l], w[l], S0, S1, S2, T0, T1);
-  const float det = __fsub_rn(__fmul_rn(S0, S2), __fmul_rn(S1, S1));
-  const float a = __fdiv_rn(__fsub_rn(__fmul_rn(T0, S2), __fmul_rn(T1, S1)), det);
-  const float b = __fdiv_rn(__fsub_rn(__fmul_rn(T1, S0), __fmul_rn(T0, S1)), det);
-  float chi2 = __fmul_rn(__fmul_rn(c.w_velo, a), a);
-#pragma unroll
-  for (int l = 0; l < 4; ++l) chi2 = fit_res(p[l], d[l], dz[l], w[l], a, b, chi2);
-  FitResult r;
-  r.chi2 = chi2;
-  r.b = b;
-  r.valid = chi2 <= __fmul_rn(c.max_chi2_ndf, (float)(n - 1));
-  return r;
-}
 
 // (n desc, chi2 asc, hit tuple asc): candidate positions are ascending in hit index, none = 63
 __device__ __forceinline__ unsigned long long make_key(int n, float chi2, uint32_t p0, uint32_t p1, uint32_t p2,
