@@ -41,7 +41,10 @@ class _Geometry(C.Structure):
                 ("x0", C.c_void_p), ("pitch", C.c_void_p), ("dxdy", C.c_void_p), ("z", C.c_void_p),
                 ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
                 ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
-                ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4)]
+                ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
+                ("kick_nx", C.c_uint32), ("kick_ny", C.c_uint32), ("kick_x_lo", C.c_float), ("kick_y_lo", C.c_float),
+                ("kick_inv_dx", C.c_float), ("kick_inv_dy", C.c_float), ("kick_z_ref", C.c_float),
+                ("kick_kappa", C.c_void_p), ("kick_z_mag", C.c_void_p)]
 
 
 class _Hits(C.Structure):
@@ -84,6 +87,13 @@ def _geom_struct(geom):
     s = _Geometry(geom.n_layers, geom.n_sectors, geom.n_groups, geom.id_table_size, *[_p(a) for a in keep])
     s.layer_z[:] = [float(v) for v in geom.layer_z]
     s.layer_dxdy[:] = [float(v) for v in geom.layer_dxdy]
+    lut = getattr(geom, "kick", None)
+    if lut is not None:                                   # position-dependent kick table (synth/field.py)
+        kk, kz = np.ascontiguousarray(lut.kappa, np.float32), np.ascontiguousarray(lut.z_mag, np.float32)
+        keep += [kk, kz]
+        s.kick_nx, s.kick_ny = lut.nx, lut.ny
+        s.kick_x_lo, s.kick_y_lo, s.kick_inv_dx, s.kick_inv_dy, s.kick_z_ref = lut.x_lo, lut.y_lo, lut.inv_dx, lut.inv_dy, lut.z_ref
+        s.kick_kappa, s.kick_z_mag = _p(kk), _p(kz)
     return s, keep
 
 

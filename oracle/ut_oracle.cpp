@@ -41,6 +41,10 @@ struct oracle_geometry {
   const float *x0, *pitch, *dxdy, *z, *y_begin, *y_end, *weight;   // [n_sectors]
   const float *group_xmin, *group_xmax;                            // [n_groups]
   float layer_z[4], layer_dxdy[4];
+  // optional position-dependent kick table; kick_nx == 0: constant kick
+  uint32_t kick_nx, kick_ny;
+  float kick_x_lo, kick_y_lo, kick_inv_dx, kick_inv_dy, kick_z_ref;
+  const float *kick_kappa, *kick_z_mag;                            // [kick_ny * kick_nx]
 };
 
 struct oracle_hits {                // SoA container of PAPER.md:243-254
@@ -164,6 +168,30 @@ static inline float resid(const HitsView& H, int64_t h, float x_e, float y_e) {
 }
 static inline bool y_ok(const HitsView& H, int64_t h, float y_e, float y_tol) {
   return (H.yb[h] - y_tol <= y_e) && (y_e <= H.ye[h] + y_tol);
+}
+
+// SURVEY.md 8(f) row 4 / DESIGN.md A24 ("look-up tables ... the influence of the magnetic field"):
+// the track's kick strength and kick plane from the table cell that holds its straight-line position at z_ref
+// (nearest cell, no interpolation; a NaN coordinate takes cell 0).  Without a table: the config's constants.
+static inline int lut_index(float v, float lo, float inv, uint32_t n) {
+  const float u = (v - lo) * inv;
+  if (!(u == u)) return 0;
+  const float f = std::floor(u);
+  if (f < 0.f) return 0;
+  if (f > (float)(n - 1)) return (int)n - 1;
+  return (int)f;
+}
+static oracle_config track_config(const oracle_geometry* g, const oracle_config* c, float vx, float vy, float vtx,
+                                  float vty, float vz) {
+  oracle_config ct = *c;
+  if (g->kick_nx == 0) return ct;
+  const float dzr = g->kick_z_ref - vz;
+  const float xk = vx + vtx * dzr, yk = vy + vty * dzr;
+  const int cell = lut_index(yk, g->kick_y_lo, g->kick_inv_dy, g->kick_ny) * (int)g->kick_nx +
+                   lut_index(xk, g->kick_x_lo, g->kick_inv_dx, g->kick_nx);
+  ct.kappa = g->kick_kappa[cell];
+  ct.z_mag = g->kick_z_mag[cell];
+  return ct;
 }
 
 // step 2 (+3): candidate list of one layer.  mode 0 = windowed (group pre-selection + binary
@@ -380,12 +408,13 @@ int32_t oracle_compass(int32_t mode, const oracle_hits* hits, const uint32_t* hi
       }
       Best result;
       int fits = 0;
+      const oracle_config ct = track_config(g, c, vx[t], vy[t], vtx[t], vty[t], vz);   // kick of THIS track (A24)
       if (nonempty >= c->min_hits) {                        // step 4
         if (mode != 2) {
           Best fwd, bwd;
-          search_direction(cand, 0, 2, 1, 3, c, fwd);       // forward seeds (L0, L2)
+          search_direction(cand, 0, 2, 1, 3, &ct, fwd);     // forward seeds (L0, L2)
           if (c->both_directions || !fwd.best.valid)        // A11: backward only if forward found nothing valid
-            search_direction(cand, 3, 1, 2, 0, c, bwd);
+            search_direction(cand, 3, 1, 2, 0, &ct, bwd);
           result = combine_directions(fwd, bwd, c->both_directions != 0);
           fits = result.n_fits;
         } else {
@@ -405,10 +434,10 @@ int32_t oracle_compass(int32_t mode, const oracle_hits* hits, const uint32_t* hi
                     const Cand *a = hit[LA[dct]], *b = hit[LB[dct]];
                     if (!a || !b) continue;
                     float bs;
-                    if (!seed_ok(*a, *b, c, &bs)) continue;
-                    if (hit[LC[dct]] && !compat(*a, bs, *hit[LC[dct]], c)) continue;
-                    if (hit[LD[dct]] && !compat(*a, bs, *hit[LD[dct]], c)) continue;
-                    dir[dct].offer(fit(hit, c));
+                    if (!seed_ok(*a, *b, &ct, &bs)) continue;
+                    if (hit[LC[dct]] && !compat(*a, bs, *hit[LC[dct]], &ct)) continue;
+                    if (hit[LD[dct]] && !compat(*a, bs, *hit[LD[dct]], &ct)) continue;
+                    dir[dct].offer(fit(hit, &ct));
                   }
                 }
           result = combine_directions(dir[0], dir[1], c->both_directions != 0);
@@ -543,10 +572,11 @@ int32_t oracle_compass_from_windows(const oracle_hits* hits, const uint32_t* hit
         if (!cand[l].empty()) ++nonempty;
       }
       Best result;
+      const oracle_config ct = track_config(g, c, vx[t], vy[t], vtx[t], vty[t], vz);
       if (nonempty >= c->min_hits) {
         Best fwd, bwd;
-        search_direction(cand, 0, 2, 1, 3, c, fwd);
-        if (c->both_directions || !fwd.best.valid) search_direction(cand, 3, 1, 2, 0, c, bwd);
+        search_direction(cand, 0, 2, 1, 3, &ct, fwd);
+        if (c->both_directions || !fwd.best.valid) search_direction(cand, 3, 1, 2, 0, &ct, bwd);
         result = combine_directions(fwd, bwd, c->both_directions != 0);
       }
       const Tracklet& b = result.best;

@@ -13,9 +13,10 @@ from .geometry import UTGeometry, make_geometry
 from .events import EventModel, Batch, generate_batch, generate_event, encode_event
 from .configs import CONFIGS, WorkloadConfig, CompassParams, make_compass_params, make_workload
 from .truth import physics_metrics
+from .field import KickLUT, make_kick_lut
 
 __all__ = [
     "UTGeometry", "make_geometry", "EventModel", "Batch", "generate_batch",
     "generate_event", "encode_event", "CONFIGS", "WorkloadConfig", "CompassParams",
-    "make_compass_params", "make_workload", "physics_metrics",
+    "make_compass_params", "make_workload", "physics_metrics", "KickLUT", "make_kick_lut",
 ]

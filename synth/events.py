@@ -124,7 +124,12 @@ def generate_event(geom: G.UTGeometry, model: EventModel, seed: int, event: int)
 
     zl = np.asarray(G.LAYER_Z)[None, :]
     dxdy = np.asarray(G.LAYER_DXDY)[None, :]
-    x = xv[:, None] + tx[:, None] * (zl - Z_VELO) + KAPPA * (q / p)[:, None] * (zl - Z_MAG)
+    kap, zm = np.full(T, KAPPA), np.full(T, Z_MAG)
+    if geom.kick is not None:                              # position-dependent kick (synth/field.py)
+        lut = geom.kick
+        cell = lut.cell64(xv + tx * (lut.z_ref - Z_VELO), yv + ty * (lut.z_ref - Z_VELO))
+        kap, zm = lut.kappa[cell].astype(np.float64), lut.z_mag[cell].astype(np.float64)
+    x = xv[:, None] + tx[:, None] * (zl - Z_VELO) + (kap * q / p)[:, None] * (zl - zm[:, None])
     y = yv[:, None] + ty[:, None] * (zl - Z_VELO)
     smear = rng.normal(0.0, model.sigma_hit, (T, 4))
     keep_draw = rng.uniform(0.0, 1.0, (T, 4))
@@ -205,8 +210,9 @@ def assemble_batch(geom: G.UTGeometry, events: list) -> Batch:
 
 
 def _gen_range(args):
-    model, seed, lo, hi = args
+    model, seed, lo, hi, kick = args
     geom = G.make_geometry()
+    geom.kick = kick
     return [generate_event(geom, model, seed, ev) for ev in range(lo, hi)]
 
 
@@ -217,7 +223,7 @@ def generate_batch(geom: G.UTGeometry, model: EventModel, seed: int, n_events: i
         import multiprocessing as mp
         cuts = np.linspace(first_event, first_event + n_events, workers + 1).astype(int)
         with mp.get_context("fork").Pool(workers) as pool:
-            parts = pool.map(_gen_range, [(model, seed, int(a), int(b)) for a, b in zip(cuts[:-1], cuts[1:])])
+            parts = pool.map(_gen_range, [(model, seed, int(a), int(b), geom.kick) for a, b in zip(cuts[:-1], cuts[1:])])
         events = [e for part in parts for e in part]
     else:
         events = [generate_event(geom, model, seed, ev) for ev in range(first_event, first_event + n_events)]

@@ -60,6 +60,8 @@ class UTGeometry:
     # float64 helpers for the generator only
     x_left64: np.ndarray = field(repr=False, default=None)
     y_c64: np.ndarray = field(repr=False, default=None)
+    # optional position-dependent kick table (synth/field.py), None = constant kick
+    kick: object = field(repr=False, default=None)
 
     @property
     def id_table_size(self) -> int:
