@@ -81,6 +81,16 @@ typedef struct {
                                          pitch}: the table row a decoded hit copies, packed for 128-bit loads */
   uint32_t flags;                     /* UT_GEOM_* properties found by ut_geometry_upload */
   void* owner;                        /* opaque allocation handle, NULL for caller-owned tables */
+  /* Optional position-dependent kick table ("look-up tables are used, which give quick access to the
+   * influence of the magnetic field", A24).  kick_nx == 0: the constants
+   * compass_config.kappa / z_mag apply to every track.  Otherwise every VELO track takes its kappa and z_mag from the
+   * cell that holds its straight-line position at kick_z_ref (nearest cell, no interpolation):
+   *   x_k = x + tx*(kick_z_ref - z0), y_k likewise (fp32);  ix = clamp(floor((x_k - kick_x_lo)*kick_inv_dx), 0, nx-1),
+   *   iy likewise (a NaN coordinate takes index 0);  cell = iy*kick_nx + ix.
+   * HOST arrays on input to ut_geometry_upload, device arrays in its output; at most 4096 cells. */
+  uint32_t kick_nx, kick_ny;
+  float kick_x_lo, kick_y_lo, kick_inv_dx, kick_inv_dy, kick_z_ref;
+  const float *kick_kappa, *kick_z_mag;   /* [kick_ny * kick_nx] */
 } ut_geometry;
 
 /* y_begin and y_end are non-decreasing over the sectors of every group: the sector row a track crosses

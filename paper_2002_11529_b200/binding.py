@@ -36,7 +36,10 @@ class ut_geometry(C.Structure):
                 ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
                 ("group_first_sector", C.c_void_p), ("sector_rows", C.c_void_p),
                 ("flags", C.c_uint32),
-                ("owner", C.c_void_p)]
+                ("owner", C.c_void_p),
+                ("kick_nx", C.c_uint32), ("kick_ny", C.c_uint32), ("kick_x_lo", C.c_float), ("kick_y_lo", C.c_float),
+                ("kick_inv_dx", C.c_float), ("kick_inv_dy", C.c_float), ("kick_z_ref", C.c_float),
+                ("kick_kappa", C.c_void_p), ("kick_z_mag", C.c_void_p)]
 
 
 class ut_hits(C.Structure):
@@ -167,6 +170,14 @@ class Geometry:
             setattr(host, name, arr.ctypes.data)
         host.layer_z[:] = [float(v) for v in tables.layer_z]
         host.layer_dxdy[:] = [float(v) for v in tables.layer_dxdy]
+        lut = getattr(tables, "kick", None)
+        if lut is not None:                                # optional position-dependent kick table
+            kk, kz = np.ascontiguousarray(lut.kappa, np.float32), np.ascontiguousarray(lut.z_mag, np.float32)
+            keep += [kk, kz]
+            host.kick_nx, host.kick_ny = lut.nx, lut.ny
+            host.kick_x_lo, host.kick_y_lo, host.kick_inv_dx, host.kick_inv_dy = lut.x_lo, lut.y_lo, lut.inv_dx, lut.inv_dy
+            host.kick_z_ref = lut.z_ref
+            host.kick_kappa, host.kick_z_mag = kk.ctypes.data, kz.ctypes.data
         self.c = ut_geometry()
         _check(_lib.ut_geometry_upload(C.byref(host), C.byref(self.c)), "ut_geometry_upload")
         self.n_sectors, self.n_groups = tables.n_sectors, tables.n_groups

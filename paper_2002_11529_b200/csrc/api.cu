@@ -201,7 +201,10 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
   const size_t sz_id = up(h->id_table_size * 4), sz_s = up(ns * 4), sz_g = up((ng + 1) * 4);
   const size_t sz_rows = up((size_t)ns * 32);
-  const size_t total = sz_id + 9 * sz_s + 3 * sz_g + sz_rows;
+  const uint32_t n_cells = h->kick_nx * h->kick_ny;
+  if (h->kick_nx != 0 && (n_cells == 0 || n_cells > 4096 || !h->kick_kappa || !h->kick_z_mag)) return UT_ERR_GEOMETRY;
+  const size_t sz_k = up((size_t)n_cells * 4);
+  const size_t total = sz_id + 9 * sz_s + 3 * sz_g + sz_rows + 2 * sz_k;
   unsigned char* dev = nullptr;
   if (cudaMalloc(&dev, total) != cudaSuccess) return UT_ERR_CUDA;
   std::vector<unsigned char> host(total, 0);
@@ -235,6 +238,13 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
       r[4] = h->weight[s]; memcpy(&r[5], &h->sector_raw_id[s], 4); r[6] = h->x0[s]; r[7] = h->pitch[s];
     }
     out->sector_rows = put(rows.data(), (size_t)ns * 32, sz_rows);
+  }
+  if (n_cells) {
+    out->kick_kappa = (const float*)put(h->kick_kappa, (size_t)n_cells * 4, sz_k);
+    out->kick_z_mag = (const float*)put(h->kick_z_mag, (size_t)n_cells * 4, sz_k);
+  } else {
+    out->kick_nx = out->kick_ny = 0;
+    out->kick_kappa = out->kick_z_mag = nullptr;
   }
   if (cudaMemcpy(dev, host.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaFree(dev);

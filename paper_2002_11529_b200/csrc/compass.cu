@@ -87,6 +87,7 @@ struct CompassArgs {
   uint32_t bulk_ok;                    // hit arrays are 16-byte aligned: the event's x and id ranges come by TMA
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
   uint32_t split;                      // K: CTAs sharing the tracks of one event
+  KickTable kick;                      // optional per-track kappa / z_mag (kick.nx == 0: the config's constants)
   float slope_lim;                     // max_slope * (1 + kFilterEps): pre-filter limit
   int32_t interval_min;                // seed partner lists longer than this are searched, not walked
 };
@@ -114,13 +115,15 @@ struct WarpArea {
   int* n;                      // [32] candidates per slot
   float* zs;                   // [32] z of the slot's candidates when they all share one
   float* ws;                   // [32] weight, likewise
+  float* tzm;                  // [kTPW] kick plane z_mag of the track
+  float* tkap;                 // [kTPW] kick strength kappa of the track
   int* srt;                    // [32] 1: the slot's residuals ascend with the position (kernels with INTERVAL only)
   int CS;
 };
 
 __host__ __device__ inline int cand_stride(int C) { return C | 1; }
 __host__ __device__ inline size_t warp_area_bytes(int C) {
-  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 4;
+  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 4 + kTPW * 4 * 2;
 }
 
 // Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
@@ -356,7 +359,7 @@ __device__ __forceinline__ float cand_z(const CompassArgs& a, const WarpArea& wa
 }
 
 // ---- phase 2 (b) + (c): `cnt` queued seeds, one per lane, then all their 3/4-hit combinations --------------
-template <bool UNI>
+template <bool UNI, bool KICK>
 __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpArea& wa, int lane, int cnt, int qhead,
                                               int dir) {
   const int LA = dir ? 3 : 0, LB = dir ? 1 : 2, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
@@ -378,7 +381,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
       const float da = wa.cd[(j4 + LA) * CS + ia], db = wa.cd[(j4 + LB) * CS + ib];
       const float za = cand_z<UNI>(a, wa, j4 + LA, ia), zb = cand_z<UNI>(a, wa, j4 + LB, ib);
       const float bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
-      const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, a.c.z_mag)));
+      const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, KICK ? wa.tzm[sd >> 10] : a.c.z_mag)));
       ok = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
       if (ok) {
         const int nC = wa.n[j4 + LC], nD = wa.n[j4 + LD];
@@ -460,7 +463,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
           ++nh;
         }
       }
-      const FitResult fr = fit_tracklet(pr, d, z, w, nh, a.c);
+      const FitResult fr = fit_tracklet(pr, d, z, w, nh, a.c, KICK ? wa.tzm[j] : a.c.z_mag);
       if (fr.valid)
         atomicMin(&wa.best[j], make_key(nh, fr.chi2, (uint32_t)pos[0] & 63u, (uint32_t)pos[1] & 63u,
                                         (uint32_t)pos[2] & 63u, (uint32_t)pos[3] & 63u));
@@ -471,7 +474,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 // ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
 // (process_seeds has ONE call site per variant: the kernel's code size decides how well it stays in the
 //  instruction cache)
-template <bool UNI, bool INTERVAL>
+template <bool UNI, bool INTERVAL, bool KICK>
 __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
   const int j = lane & 7;
   const int CS = wa.CS;
@@ -500,7 +503,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
       if (i < total) {
         da = wa.cd[sA * CS + ia];
         za = cand_z<UNI>(a, wa, sA, (int)ia);
-        zam = za - a.c.z_mag;
+        zam = za - (KICK ? wa.tzm[jj] : a.c.z_mag);
         if (UNI) rinv = rcp_approx(wa.zs[sB] - za);
         lim0 = a.c.kink_tol + kFilterEps * (a.c.kink_tol + fabsf(da));
       } else {
@@ -553,7 +556,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         while (qn >= 32 || (last && qn > 0)) {  // a full queue, or the rest after the last pair
           __syncwarp();
           const int cnt = min(qn, 32);
-          process_seeds<UNI>(a, wa, lane, cnt, qhead, dir);
+          process_seeds<UNI, KICK>(a, wa, lane, cnt, qhead, dir);
           qhead += cnt;
           qn -= cnt;
           __syncwarp();
@@ -566,7 +569,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
 }
 
 // The warps of the CTA pull 8-track batches of the item: track m of the item is VELO track t0 + m * K + part.
-template <bool BUCKETED, bool INTERVAL>
+template <bool BUCKETED, bool INTERVAL, bool KICK>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
                                            uint32_t h0, uint32_t t0, uint32_t nTk, uint32_t part, uint32_t T,
                                            const uint16_t* perm) {
@@ -591,6 +594,10 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
       n_st = collect_window<BUCKETED>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
+      if (KICK && l == 0) track_kick(a.kick, a.c, vx, vy, vtx, vty, a.vz, wa.tkap[lane >> 2], wa.tzm[lane >> 2]);
+    } else if (KICK && l == 0) {
+      wa.tkap[lane >> 2] = a.c.kappa;
+      wa.tzm[lane >> 2] = a.c.z_mag;
     }
     wa.n[lane] = n_st;
     wa.zs[lane] = zu;
@@ -608,8 +615,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
     const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    if (uni) find_tracklets<true, INTERVAL>(a, wa, lane, todo);
-    else find_tracklets<false, false>(a, wa, lane, todo);
+    if (uni) find_tracklets<true, INTERVAL, KICK>(a, wa, lane, todo);
+    else find_tracklets<false, false, KICK>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
       const int q4 = lane & ~3;
@@ -635,8 +642,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
             if (k == l) hidx = (int)(h0 + (hs >> 16));
           }
         }
-        const FitResult r = fit_tracklet(pr, d, z, w, nh, a.c);
-        qop = __fdiv_rn(r.b, a.c.kappa);
+        const FitResult r = fit_tracklet(pr, d, z, w, nh, a.c, KICK ? wa.tzm[lane >> 2] : a.c.z_mag);
+        qop = __fdiv_rn(r.b, KICK ? wa.tkap[lane >> 2] : a.c.kappa);
       }
       a.out_idx[(size_t)l * T + tg] = hidx;
       if (l == 0) { a.out_n[tg] = nh; a.out_qop[tg] = qop; a.out_chi2[tg] = chi2; }
@@ -648,7 +655,9 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
 // One CTA works through work items (event, part) handed out by the ticket.  Geometry tables are staged once.
 // INTERVAL: the seed search of long, d-sorted partner lists by interval (worth its code only when
 // max_candidates_per_layer allows long lists; the kernel without it is the faster one for short lists).
-template <int MAXT, int MINB, bool INTERVAL>
+// KICK: per-track kappa / z_mag from the kick table (ut_geometry.kick_*); without it the config's constants come
+// straight from the kernel parameters.
+template <int MAXT, int MINB, bool INTERVAL, bool KICK>
 __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -712,6 +721,8 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     wa.zs = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 4);
     wa.ws = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 8);
     wa.srt = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 12);
+    wa.tzm = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 16);
+    wa.tkap = wa.tzm + kTPW;
   }
   const uint32_t Tend = __ldg(a.velo_offsets + a.n_events);
   const uint32_t T = a.idx_stride ? a.idx_stride : Tend;
@@ -928,9 +939,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     __syncthreads();                               // order and staged data visible; scratch is dead from here on
     if (staged) {
-      track_loop<true, INTERVAL>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<true, INTERVAL, KICK>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false, INTERVAL>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<false, INTERVAL, KICK>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     }
   }
   if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
@@ -953,11 +964,12 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32
 // Two register budgets: CTAs of <= 224 threads at 4 per SM (72 registers), and larger CTAs (big events / C = 32,
 // where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
 constexpr int kSmallBlock = 224;
-static const void* const kKernels[2][2] = {
-    {reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4, false>),
-     reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4, true>)},
-    {reinterpret_cast<const void*>(&compass_kernel<768, 1, false>),
-     reinterpret_cast<const void*>(&compass_kernel<768, 1, true>)}};
+#define UTC_K(T, B, I, K) reinterpret_cast<const void*>(&compass_kernel<T, B, I, K>)
+static const void* const kKernels[2][2][2] = {     // [large CTAs][interval search][kick table]
+    {{UTC_K(kSmallBlock, 4, false, false), UTC_K(kSmallBlock, 4, false, true)},
+     {UTC_K(kSmallBlock, 4, true, false), UTC_K(kSmallBlock, 4, true, true)}},
+    {{UTC_K(768, 1, false, false), UTC_K(768, 1, false, true)}, {UTC_K(768, 1, true, false), UTC_K(768, 1, true, true)}}};
+#undef UTC_K
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
@@ -968,8 +980,9 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   const ut_tuning tune = tuning_snapshot();
   const int interval_min = tuned(tune.compass_interval_min, 16);
   const int iv = cfg->max_candidates_per_layer > interval_min ? 1 : 0;    // long partner lists are possible
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[0][iv], kSlotCompassSmall + iv, &max_smem)) return rc;
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[1][iv], kSlotCompassLarge + iv, &max_smem_large)) return rc;
+  const int kk = hits->geom->kick_nx != 0 ? 1 : 0;                        // per-track kick from the table
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[0][iv][kk], kSlotCompassSmall + 2 * iv + kk, &max_smem)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[1][iv][kk], kSlotCompassLarge + 2 * iv + kk, &max_smem_large)) return rc;
   max_smem = std::min(max_smem, max_smem_large);
   const int n_sm = dev.n_sm, sm_smem = dev.smem_per_sm;
   const ut_geometry* geom = hits->geom;
@@ -994,6 +1007,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
   a.c = *cfg;
+  a.kick = make_kick_table(geom);
   a.slope_lim = cfg->max_slope * (1.0f + kFilterEps);
   a.interval_min = iv ? std::min(interval_min, 8) : interval_min;     // inside the interval kernel the search pays from ~8 partners
   a.idx_stride = idx_stride;
@@ -1047,7 +1061,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
       break;
     }
   }
-  const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv];
+  const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv][kk];
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
   if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);

@@ -40,6 +40,7 @@ struct WindowArgs {
   const float *group_xmin, *group_xmax;
   float layer_z[4], layer_dxdy[4];
   compass_config c;
+  KickTable kick;
   int32_t W;
   int16_t* windows;            // [T][4][2W]
   unsigned long long capacity;
@@ -163,13 +164,14 @@ __device__ __forceinline__ bool better_t(int n, float chi2, const int (&h)[4], c
   return false;
 }
 
-__device__ void search_direction_t(const WindowArgs& a, const LocalCand& L, int LA, int LB, int LC, int LD, BestT& best) {
+__device__ void search_direction_t(const WindowArgs& a, const LocalCand& L, float z_mag, int LA, int LB, int LC, int LD,
+                                   BestT& best) {
   const compass_config& c = a.c;
   for (int ia = 0; ia < L.n[LA]; ++ia) {
     for (int ib = 0; ib < L.n[LB]; ++ib) {
       const float da = L.d[LA][ia], za = L.z[LA][ia];
       const float bs = __fdiv_rn(__fsub_rn(L.d[LB][ib], da), __fsub_rn(L.z[LB][ib], za));
-      const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, c.z_mag)));
+      const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, z_mag)));
       if (!(fabsf(bs) <= c.max_slope && fabsf(a0) <= c.kink_tol)) continue;
       uint32_t mC = 0, mD = 0;
       for (int i = 0; i < L.n[LC]; ++i)
@@ -195,7 +197,7 @@ __device__ void search_direction_t(const WindowArgs& a, const LocalCand& L, int 
             d[l] = pr[l] ? L.d[l][q] : 0.f; z[l] = pr[l] ? L.z[l][q] : 0.f; w[l] = pr[l] ? L.w[l][q] : 0.f;
             h[l] = pr[l] ? L.h[l][q] : -1;
           }
-          const FitResult fr = fit_tracklet(pr, d, z, w, nh, c);
+          const FitResult fr = fit_tracklet(pr, d, z, w, nh, c, z_mag);
           if (fr.valid && (!best.valid || better_t(nh, fr.chi2, h, best))) {
             best.valid = true; best.n = nh; best.chi2 = fr.chi2;
 #pragma unroll
@@ -292,9 +294,11 @@ __global__ void __launch_bounds__(kWinTracks) tracklets_kernel(const WindowArgs 
       BestT best;
       best.valid = false; best.n = 0; best.chi2 = 0.f;
       for (int l = 0; l < 4; ++l) best.h[l] = -1;
+      float kappa, z_mag;                                     // the track's kick (table cell or the config's constants)
+      track_kick(a.kick, c, vx, vy, vtx, vty, a.vz, kappa, z_mag);
       if (nonempty >= c.min_hits) {
-        search_direction_t(a, L, 0, 2, 1, 3, best);                           // forward seeds (L0, L2)
-        if (c.both_directions || !best.valid) search_direction_t(a, L, 3, 1, 2, 0, best);   // backward (L3, L1)
+        search_direction_t(a, L, z_mag, 0, 2, 1, 3, best);                    // forward seeds (L0, L2)
+        if (c.both_directions || !best.valid) search_direction_t(a, L, z_mag, 3, 1, 2, 0, best);   // backward (L3, L1)
       }
       float qop = 0.f;
       if (best.valid) {                                       // q/p of the winner: its fit again (step 6)
@@ -307,7 +311,7 @@ __global__ void __launch_bounds__(kWinTracks) tracklets_kernel(const WindowArgs 
             for (int i = 0; i < L.n[l]; ++i)
               if (L.h[l][i] == best.h[l]) { d[l] = L.d[l][i]; z[l] = L.z[l][i]; wv[l] = L.w[l][i]; }
         }
-        qop = __fdiv_rn(fit_tracklet(pr, d, z, wv, best.n, c).b, c.kappa);
+        qop = __fdiv_rn(fit_tracklet(pr, d, z, wv, best.n, c, z_mag).b, kappa);
       }
       for (int l = 0; l < 4; ++l) a.out_idx[(size_t)l * T + t] = best.valid ? best.h[l] : -1;
       a.out_n[t] = best.valid ? best.n : 0;
@@ -328,7 +332,7 @@ static void fill_args(WindowArgs& a, const ut_hits* hits, const uint32_t* hit_of
   a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
   a.group_xmin = geom->group_xmin; a.group_xmax = geom->group_xmax;
   for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
-  a.c = *cfg; a.W = W; a.capacity = hits->capacity;
+  a.c = *cfg; a.kick = make_kick_table(geom); a.W = W; a.capacity = hits->capacity;
   a.windows = nullptr; a.status = nullptr; a.out_idx = nullptr; a.out_n = nullptr; a.out_qop = nullptr; a.out_chi2 = nullptr;
 }
 

@@ -544,3 +544,38 @@ def test_host_pipeline_empty_and_invalid(gpu, wl):
         pipe.run_host(z(torch.uint8, 64), 0, z(torch.int32, 5 * 896 + 1), velo_h, 770.0, z(torch.int32, 6), 0, 5,
                       B.make_config(p), out_h)
     pipe.destroy()
+
+
+def test_kick_lut(gpu):
+    """SURVEY.md 8(f) row 4 (field table): per-track kappa and z_mag from the position-dependent kick table
+    (ut_geometry.kick_*, DESIGN.md A24), fused kernel and the two-kernel variant against the oracle bit for bit;
+    a table smaller than the acceptance exercises the clamped look-ups."""
+    import torch
+    from gpu_helpers import GpuRunner
+    from synth.events import generate_batch
+    p = synth.make_compass_params()
+    for kw in (dict(falloff=0.3, bow=120.0), dict(half_x=250.0, half_y=200.0, nx=7, ny=5)):
+        g = synth.make_geometry()
+        g.kick = synth.make_kick_lut(**kw)
+        b = generate_batch(g, EventModel(mean_tracks=150.0, efficiency=0.97, noise_mean=1500.0), seed=41, n_events=40)
+        runner = GpuRunner(g)
+        h_ref, t_ref = check_batch(runner, g, b, p)
+        # the table matters: the same events tracked with the constant kick give other q/p values
+        t_const = oracle.compass(h_ref, b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z, b.velo_offsets, b.n_events,
+                                 synth.make_geometry(), p)
+        assert (t_const.qop != t_ref.qop).sum() > 1000
+        # two-kernel variant with 5 sector groups
+        B = runner.B
+        hits = runner.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+        velo = B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z)
+        vo = B.to_device_u32(b.velo_offsets)
+        T = b.n_velo_total
+        win = torch.empty(T * 40, dtype=torch.int16, device="cuda")
+        st = torch.zeros(1, dtype=torch.int32, device="cuda")
+        tr = B.Tracks(T)
+        B.compass_search_windows(hits, hits.hit_offsets, velo, vo, b.n_events, B.make_config(p), 5, win, st)
+        B.compass_tracklets_from_windows(hits, hits.hit_offsets, velo, vo, b.n_events, B.make_config(p), 5, win, tr)
+        torch.cuda.synchronize()
+        idx, n, qop, chi2 = tr.numpy()
+        assert np.array_equal(idx, t_ref.hit_idx) and np.array_equal(qop.view(np.uint32), t_ref.qop.view(np.uint32))
+        assert np.array_equal(chi2.view(np.uint32), t_ref.chi2.view(np.uint32))
