@@ -138,8 +138,10 @@ class Tracks:
     n_fits: np.ndarray           # i32 [T]
 
 
-def decode(raw: np.ndarray, bank_offsets: np.ndarray, n_events: int, geom, capacity: int | None = None) -> Hits:
-    """PAPER.md section IV as the plain definition."""
+def decode(raw: np.ndarray, bank_offsets: np.ndarray, n_events: int, geom, capacity: int | None = None,
+           order: str = "x") -> Hits:
+    """PAPER.md section IV as the plain definition (SURVEY.md 8(c)).  order "x": groups sorted by x_at_y0 (A1);
+    "y": by (y_begin, x_at_y0) -- the paper's literal Y order."""
     lib = _load()
     raw = np.ascontiguousarray(raw, dtype=np.uint8)
     bank_offsets = np.ascontiguousarray(bank_offsets, dtype=np.uint32)
@@ -152,7 +154,7 @@ def decode(raw: np.ndarray, bank_offsets: np.ndarray, n_events: int, geom, capac
     hs = h._struct()
     st = C.c_uint32(0)
     rc = lib.oracle_decode(_p(raw), _p(bank_offsets), C.c_int32(n_events), C.byref(gs), C.byref(hs),
-                           _p(h.hit_offsets), C.byref(st))
+                           _p(h.hit_offsets), C.byref(st), C.c_int32({"x": 0, "y": 1}[order]))
     if rc != 0:
         raise RuntimeError(f"oracle_decode rc={rc}")
     h.status = int(st.value)

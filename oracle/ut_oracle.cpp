@@ -81,9 +81,11 @@ static inline uint32_t rd32(const uint8_t* p) {
 // (dense sector, k) (stable sort of the fill order).  hit_offsets = exclusive prefix of
 // group sizes, n_events*n_groups + 1 entries.
 // ---------------------------------------------------------------------------------------
+// order = 1 ("sort the hits by Y coordinate ... within the sector group";
+// DESIGN.md A1/A25): inside a group ascending y_begin, then ascending x, ties still in fill order.
 int32_t oracle_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t n_events,
                       const oracle_geometry* g, oracle_hits* out, uint32_t* hit_offsets,
-                      uint32_t* status) {
+                      uint32_t* status, int32_t order) {
   if (!bank_offsets || !g || !out || !hit_offsets || n_events < 0) return -1;
   const uint32_t ns = g->n_sectors, ng = g->n_groups;
   uint32_t st = 0;
@@ -128,7 +130,13 @@ int32_t oracle_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
           grp.push_back(Hit{x, s, strip});
         }
       }
-      std::stable_sort(grp.begin(), grp.end(), [](const Hit& a, const Hit& b) { return a.x < b.x; });
+      if (order == 1)
+        std::stable_sort(grp.begin(), grp.end(), [g](const Hit& a, const Hit& b) {
+          const float ya = g->y_begin[a.s], yb = g->y_begin[b.s];
+          return ya < yb || (ya == yb && a.x < b.x);
+        });
+      else
+        std::stable_sort(grp.begin(), grp.end(), [](const Hit& a, const Hit& b) { return a.x < b.x; });
       if (fits) {
         for (size_t i = 0; i < grp.size(); ++i) {
           const uint64_t p = total + i;
@@ -218,6 +226,32 @@ static void layer_candidates(int mode, const HitsView& H, const uint32_t* goff /
         const float d = resid(H, h, x_e, y_e);
         if (!(d <= D)) break;
         if (y_ok(H, h, y_e, c->y_tol)) out.push_back(Cand{(int32_t)h, d, H.z[h], H.w[h]});
+      }
+    }
+  } else if (mode == 3) {
+    // Y-sorted groups: the groups the x window can touch, in each "two binary searches over the Y
+    // axis, one to delimit the beginning of the region and another to delimit the end of it", then "the window
+    // range is refined by checking the hits".  The searches need y_begin and y_end non-decreasing along the group,
+    // which the (y_begin, x) order gives when the sector rows do not nest.
+    const float sy = g->layer_dxdy[l] * y_e;
+    const float ctr = x_e - sy;
+    const float lo = (ctr - D) - GROUP_EPS, hi = (ctr + D) + GROUP_EPS;
+    for (uint32_t gi = l * gpl; gi < (l + 1) * gpl; ++gi) {
+      if (!(g->group_xmax[gi] >= lo && g->group_xmin[gi] <= hi)) continue;
+      int64_t first = goff[gi], n = (int64_t)goff[gi + 1] - first;      // first hit with y_e <= y_end + y_tol
+      while (n > 0) {
+        const int64_t half = n / 2, mid = first + half;
+        if (y_e <= H.ye[mid] + c->y_tol) n = half; else { first = mid + 1; n -= half + 1; }
+      }
+      int64_t last = first;                                              // first hit with y_begin - y_tol > y_e
+      n = (int64_t)goff[gi + 1] - last;
+      while (n > 0) {
+        const int64_t half = n / 2, mid = last + half;
+        if (H.yb[mid] - c->y_tol > y_e) n = half; else { last = mid + 1; n -= half + 1; }
+      }
+      for (int64_t h = first; h < last; ++h) {
+        const float d = resid(H, h, x_e, y_e);
+        if (std::fabs(d) <= D && y_ok(H, h, y_e, c->y_tol)) out.push_back(Cand{(int32_t)h, d, H.z[h], H.w[h]});
       }
     }
   } else {
@@ -366,8 +400,9 @@ static void search_direction(const std::vector<Cand> cand[4], int LA, int LB, in
   }
 }
 
-// mode 0: windowed candidates + seeded search (the algorithm);
-// mode 1: linear-scan candidates + seeded search (BF-1);
+// mode 0: windowed candidates + seeded search (the algorithm, x-sorted groups);
+// mode 3: the same on Y-sorted groups (binary searches over Y);
+// mode 1: linear-scan candidates + seeded search (BF-1; any order inside the groups);
 // mode 2: linear-scan candidates, NO cap, exhaustive loop over every (h0|none, h1|none, h2|none,
 //         h3|none) combination under the same predicates (BF-2; tiny events only).
 // Optional outputs (may be null): runner_chi2 [T], cand_n [T*4] pre-cap counts,
