@@ -79,6 +79,8 @@ typedef struct {
   const uint32_t* group_first_sector; /* [n_groups + 1] */
   const void* sector_rows;            /* [n_sectors] 32-byte rows {z, y_begin, y_end, dxdy | weight, raw id, x0,
                                          pitch}: the table row a decoded hit copies, packed for 128-bit loads */
+  const uint32_t* sector_yorder;      /* [n_sectors] rank of the sector inside its group by (y_begin, dense index)
+                                         | (sector-in-group index of the sector with that rank) << 8 */
   uint32_t flags;                     /* UT_GEOM_* properties found by ut_geometry_upload */
   void* owner;                        /* opaque allocation handle, NULL for caller-owned tables */
   /* Optional position-dependent kick table ("look-up tables are used, which give quick access to the
@@ -131,7 +133,14 @@ typedef struct {
                                  the event's first hit, then a word that is UT_SECTOR_INDEX_VALID if the row may be
                                  used (an event of > 65535 hits, a group larger than the decode's sort buffer or a
                                  capacity overflow leaves it 0 and compass_track re-buckets that event itself) */
+  uint32_t order;             /* order inside a sector group, set by the caller before ut_decode: UT_ORDER_X (default)
+                                 ascending x_at_y0; UT_ORDER_Y the paper's literal order (SURVEY.md
+                                 8(f) row 3): ascending y_begin, then ascending x_at_y0.  Ties in fill order either way.
+                                 compass_track reads it (window look-up by binary searches over Y, when
+                                 it has to search global memory); the two-kernel variant takes UT_ORDER_X only. */
 } ut_hits;
+#define UT_ORDER_X 0u
+#define UT_ORDER_Y 1u
 #define UT_SECTOR_INDEX_VALID 0xA5A5u
 uint32_t ut_sector_offsets_stride(const ut_geometry* geometry);   /* u16 elements per event, a multiple of 8 */
 

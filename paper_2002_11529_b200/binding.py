@@ -24,6 +24,7 @@ UT_OK = 0
 UT_STATUS_UNKNOWN_SECTOR, UT_STATUS_DUPLICATE_SECTOR, UT_STATUS_BAD_BANK_SIZE, UT_STATUS_CAPACITY = 1, 2, 4, 8
 UT_STATUS_BAD_OFFSETS, UT_STATUS_EVENT_TOO_LARGE, UT_STATUS_BAD_HIT_ID = 16, 32, 64
 UT_MAX_CANDIDATES = 32
+UT_ORDER_X, UT_ORDER_Y = 0, 1
 
 
 class ut_geometry(C.Structure):
@@ -34,7 +35,7 @@ class ut_geometry(C.Structure):
                 ("y_begin", C.c_void_p), ("y_end", C.c_void_p), ("weight", C.c_void_p),
                 ("group_xmin", C.c_void_p), ("group_xmax", C.c_void_p),
                 ("layer_z", C.c_float * 4), ("layer_dxdy", C.c_float * 4),
-                ("group_first_sector", C.c_void_p), ("sector_rows", C.c_void_p),
+                ("group_first_sector", C.c_void_p), ("sector_rows", C.c_void_p), ("sector_yorder", C.c_void_p),
                 ("flags", C.c_uint32),
                 ("owner", C.c_void_p),
                 ("kick_nx", C.c_uint32), ("kick_ny", C.c_uint32), ("kick_x_lo", C.c_float), ("kick_y_lo", C.c_float),
@@ -46,7 +47,8 @@ class ut_hits(C.Structure):
     _fields_ = [("x_at_y0", C.c_void_p), ("z_at_y0", C.c_void_p), ("y_begin", C.c_void_p), ("y_end", C.c_void_p),
                 ("dxdy", C.c_void_p), ("weight", C.c_void_p), ("id", C.c_void_p), ("capacity", C.c_uint64),
                 ("geom", C.POINTER(ut_geometry)), ("status", C.c_void_p), ("workspace", C.c_void_p),
-                ("x_by_sector", C.c_void_p), ("idx_by_sector", C.c_void_p), ("sector_offsets", C.c_void_p)]
+                ("x_by_sector", C.c_void_p), ("idx_by_sector", C.c_void_p), ("sector_offsets", C.c_void_p),
+                ("order", C.c_uint32)]
 
 
 class velo_states(C.Structure):
@@ -209,10 +211,12 @@ class Hits:
     """Caller-owned SoA hit container on the device (torch tensors) + its ut_hits descriptor."""
     FIELDS = ("x_at_y0", "z_at_y0", "y_begin", "y_end", "dxdy", "weight", "id")
 
-    def __init__(self, capacity: int, max_events: int, geometry: Geometry, device="cuda", sector_view: bool = True):
+    def __init__(self, capacity: int, max_events: int, geometry: Geometry, device="cuda", sector_view: bool = True,
+                 order: str = "x"):
         """sector_view: also allocate the optional per-sector view (x_by_sector, idx_by_sector, sector_offsets)
         that ut_decode fills for compass_track."""
         self.capacity = int(capacity)
+        self.order = {"x": UT_ORDER_X, "y": UT_ORDER_Y}[order]
         n = max(self.capacity, 1)
         self.x_at_y0, self.z_at_y0, self.y_begin, self.y_end, self.dxdy, self.weight = (
             torch.empty(n, dtype=torch.float32, device=device) for _ in range(6))
@@ -236,7 +240,7 @@ class Hits:
         return ut_hits(self.x_at_y0.data_ptr(), self.z_at_y0.data_ptr(), self.y_begin.data_ptr(),
                        self.y_end.data_ptr(), self.dxdy.data_ptr(), self.weight.data_ptr(), self.id.data_ptr(),
                        self.capacity, C.pointer(self.geometry.c), self.status.data_ptr(), self.workspace.data_ptr(),
-                       ptr(self.x_by_sector), ptr(self.idx_by_sector), ptr(self.sector_offsets))
+                       ptr(self.x_by_sector), ptr(self.idx_by_sector), ptr(self.sector_offsets), self.order)
 
 
 class Tracks:

@@ -204,7 +204,7 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
   const uint32_t n_cells = h->kick_nx * h->kick_ny;
   if (h->kick_nx != 0 && (n_cells == 0 || n_cells > 4096 || !h->kick_kappa || !h->kick_z_mag)) return UT_ERR_GEOMETRY;
   const size_t sz_k = up((size_t)n_cells * 4);
-  const size_t total = sz_id + 9 * sz_s + 3 * sz_g + sz_rows + 2 * sz_k;
+  const size_t total = sz_id + 10 * sz_s + 3 * sz_g + sz_rows + 2 * sz_k;
   unsigned char* dev = nullptr;
   if (cudaMalloc(&dev, total) != cudaSuccess) return UT_ERR_CUDA;
   std::vector<unsigned char> host(total, 0);
@@ -238,6 +238,21 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
       r[4] = h->weight[s]; memcpy(&r[5], &h->sector_raw_id[s], 4); r[6] = h->x0[s]; r[7] = h->pitch[s];
     }
     out->sector_rows = put(rows.data(), (size_t)ns * 32, sz_rows);
+  }
+  {
+    // order of a group's sectors by (y_begin, dense index): what the Y order of the container follows
+    std::vector<uint32_t> yo(ns, 0);
+    for (uint32_t g = 0; g < ng; ++g) {
+      const uint32_t sa = first[g], n = first[g + 1] - first[g];
+      for (uint32_t r = 0; r < n; ++r) {
+        uint32_t rank = 0;
+        for (uint32_t q = 0; q < n; ++q)
+          rank += h->y_begin[sa + q] < h->y_begin[sa + r] || (h->y_begin[sa + q] == h->y_begin[sa + r] && q < r);
+        yo[sa + r] |= rank;
+        yo[sa + rank] |= r << 8;
+      }
+    }
+    out->sector_yorder = (const uint32_t*)put(yo.data(), ns * 4, sz_s);
   }
   if (n_cells) {
     out->kick_kappa = (const float*)put(h->kick_kappa, (size_t)n_cells * 4, sz_k);
@@ -288,8 +303,9 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
   launch_info().kernels_launched = 0;
   if (!bank_offsets || !geometry || !hits_out || !hit_offsets_out) return UT_ERR_NULL;
   if (n_events < 0) return UT_ERR_ARG;
-  if (!geometry->group_first_sector || !geometry->sector_rows)
+  if (!geometry->group_first_sector || !geometry->sector_rows || !geometry->sector_yorder)
     return UT_ERR_GEOMETRY;                                                                  // not uploaded
+  if (hits_out->order != UT_ORDER_X && hits_out->order != UT_ORDER_Y) return UT_ERR_ARG;
   if (geometry->n_sectors > UT_MAX_SECTORS || geometry->n_groups > UT_MAX_GROUPS) return UT_ERR_LIMIT;
   if (!hits_out->x_at_y0 || !hits_out->z_at_y0 || !hits_out->y_begin || !hits_out->y_end || !hits_out->dxdy ||
       !hits_out->weight || !hits_out->id)
@@ -358,6 +374,7 @@ int32_t compass_search_windows(const ut_hits* hits, const uint32_t* hit_offsets,
   if (n_events == 0) return UT_OK;
   if (!windows_out || !velo->x || !velo->y || !velo->tx || !velo->ty) return UT_ERR_NULL;
   if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
+  if (hits->order != UT_ORDER_X) return UT_ERR_ARG;                    // the group-wide binary search needs x order
   return launch_search_windows(hits, hit_offsets, velo, velo_offsets, n_events, config, n_sectors_search, windows_out,
                                status, (cudaStream_t)stream);
 }
@@ -376,6 +393,7 @@ int32_t compass_tracklets_from_windows(const ut_hits* hits, const uint32_t* hit_
       !velo->y || !velo->tx || !velo->ty)
     return UT_ERR_NULL;
   if (hits->geom->n_layers != UT_N_LAYERS || hits->geom->n_groups > UT_MAX_GROUPS) return UT_ERR_GEOMETRY;
+  if (hits->order != UT_ORDER_X) return UT_ERR_ARG;
   return launch_tracklets(hits, hit_offsets, velo, velo_offsets, n_events, config, n_sectors_search, windows, tracks_out,
                           (cudaStream_t)stream);
 }

@@ -13,7 +13,7 @@ constexpr int kWarp = 32;
 // Device-side view of the geometry tables (passed by value in kernel parameters).
 struct GeomDev {
   uint32_t n_sectors, n_groups, id_table_size, groups_per_layer;
-  const uint32_t *id_to_sector, *sector_raw_id, *sector_group, *group_first_sector;
+  const uint32_t *id_to_sector, *sector_raw_id, *sector_group, *group_first_sector, *sector_yorder;
   const float *x0, *pitch, *dxdy, *z, *y_begin, *y_end, *weight;
   const float *group_xmin, *group_xmax;
   const float4* sector_rows;
@@ -25,7 +25,7 @@ inline GeomDev make_geom_dev(const ut_geometry* g) {
   d.n_sectors = g->n_sectors; d.n_groups = g->n_groups; d.id_table_size = g->id_table_size;
   d.groups_per_layer = g->n_groups / UT_N_LAYERS;
   d.id_to_sector = g->id_to_sector; d.sector_raw_id = g->sector_raw_id; d.sector_group = g->sector_group;
-  d.group_first_sector = g->group_first_sector;
+  d.group_first_sector = g->group_first_sector; d.sector_yorder = g->sector_yorder;
   d.x0 = g->x0; d.pitch = g->pitch; d.dxdy = g->dxdy; d.z = g->z; d.y_begin = g->y_begin; d.y_end = g->y_end;
   d.weight = g->weight; d.group_xmin = g->group_xmin; d.group_xmax = g->group_xmax;
   d.sector_rows = reinterpret_cast<const float4*>(g->sector_rows);

@@ -74,6 +74,7 @@ struct CompassArgs {
   int32_t n_events;
   uint32_t n_sectors, n_groups, gpl, id_table_size, rows_sorted;
   uint32_t rows_uniform;               // rows per group when every group of a layer has the same y rows, else 0
+  uint32_t order_y;                    // the container's groups are in (y_begin, x) order (UT_ORDER_Y), not x order
   const uint32_t *id_to_sector, *group_first_sector;
   const float *group_xmin, *group_xmax, *sec_yb, *sec_ye, *sec_dxdy, *sec_z, *sec_w;
   float layer_z[4], layer_dxdy[4];
@@ -327,6 +328,31 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
           }
         }
         if (n != n_before || took_any) note_zw(a, s, n_before == 0, zu, wu);
+      }
+    } else if (a.order_y) {
+      // Y-sorted group: "two binary searches over the Y axis, one to delimit the beginning of the
+      // region and another to delimit the end of it", then "the window range is refined by checking the hits"
+      const float* X = a.hx + h0;
+      uint32_t first = ga, lastp = ga;
+      for (uint32_t cnt = gb - ga; cnt > 0;) {      // first hit with y_e <= y_end + y_tol
+        const uint32_t half = cnt >> 1, mid = first + half;
+        if (y_e <= __fadd_rn(__ldg(a.hye + h0 + mid), a.c.y_tol)) cnt = half; else { first = mid + 1; cnt -= half + 1; }
+      }
+      lastp = first;
+      for (uint32_t cnt = gb - first; cnt > 0;) {   // first hit with y_begin - y_tol > y_e
+        const uint32_t half = cnt >> 1, mid = lastp + half;
+        if (__fsub_rn(__ldg(a.hyb + h0 + mid), a.c.y_tol) > y_e) cnt = half; else { lastp = mid + 1; cnt -= half + 1; }
+      }
+      for (uint32_t h = first; h < lastp; ++h) {
+        const float d = __fsub_rn(__fadd_rn(__ldg(X + h), syg), x_e);
+        if (!(fabsf(d) <= D)) continue;
+        if (!(__fsub_rn(__ldg(a.hyb + h0 + h), a.c.y_tol) <= y_e && y_e <= __fadd_rn(__ldg(a.hye + h0 + h), a.c.y_tol)))
+          continue;
+        const uint32_t rid = __ldg(a.hid + h0 + h) >> 9;
+        const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
+        if (s >= a.n_sectors) continue;
+        const bool first_cand = n == 0;
+        if (cand_insert(wa, slot, n, C, d, (h << 16) | s)) note_zw(a, (int)s, first_cand, zu, wu);
       }
     } else {
       const float* X = a.hx + h0;
@@ -1002,6 +1028,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.n_sectors = geom->n_sectors; a.n_groups = geom->n_groups; a.gpl = geom->n_groups / UT_N_LAYERS;
   a.id_table_size = geom->id_table_size; a.rows_sorted = (geom->flags & UT_GEOM_ROWS_SORTED) ? 1u : 0u;
   a.rows_uniform = (geom->flags & UT_GEOM_ROWS_UNIFORM) ? geom->n_sectors / geom->n_groups : 0u;
+  a.order_y = hits->order == UT_ORDER_Y ? 1u : 0u;
   a.id_to_sector = geom->id_to_sector; a.group_first_sector = geom->group_first_sector;
   a.group_xmin = geom->group_xmin; a.group_xmax = geom->group_xmax;
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;

@@ -51,6 +51,9 @@ struct DecodeArgs {
   uint16_t* si;
   uint16_t* soff;
   uint32_t soff_stride;
+  uint32_t order_y;             // 1: inside a group ascending (y_begin, x) -- the paper's literal order (UT_ORDER_Y)
+  uint32_t view_ok;             // the per-sector view can describe this container (UT_ORDER_Y: only if a group's
+                                // sectors ascend in y_begin in dense order, else its sector runs are not in dense order)
 };
 
 __device__ __forceinline__ float decode_x(uint32_t word, float x0, float pitch) {
@@ -202,7 +205,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
       }
     }
     // per-sector view: usable by compass_track iff the event fits u16 positions and no group takes the generic path
-    const bool view = a.soff != nullptr && tot <= 65535u &&
+    const bool view = a.soff != nullptr && a.view_ok && tot <= 65535u &&
                       !__any_sync(0xFFFFFFFFu, gc[0] > a.sort_buf || gc[1] > a.sort_buf || gc[2] > a.sort_buf || gc[3] > a.sort_buf);
     uint16_t* soff = a.soff ? a.soff + (size_t)e * a.soff_stride : nullptr;
     if (warp == 0 && lane == 0 && soff) {
@@ -231,6 +234,51 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
       const uint32_t wpos_r = (uint32_t)lane < nsec ? s_wpos[sa + lane] : 0u;
       const uint32_t e_incl = warp_incl_scan(cnt_r, lane);
       const uint32_t e_r = (uint32_t)lane < nsec ? e_incl - cnt_r : n;   // lanes past the group: never selected
+      if (a.order_y) {
+        // ---- UT_ORDER_Y: sectors in (y_begin, dense index) order, x-sorted inside a sector.  A hit's
+        // place = its sector's start in that order + its rank among the words of its own bank: no group-wide rank.
+        const uint32_t yo = (uint32_t)lane < nsec ? __ldg(a.g.sector_yorder + sa + lane) : 0u;
+        const uint32_t cnt_y = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)((yo >> 8) & 31u));     // count of the lane-th sector in y order
+        const uint32_t cy = (uint32_t)lane < nsec ? cnt_y : 0u;
+        const uint32_t ey_k = warp_incl_scan(cy, lane) - cy;
+        const uint32_t ey_r = __shfl_sync(0xFFFFFFFFu, ey_k, (int)(yo & 31u));               // start of THIS lane's sector
+        if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)(gstart + ey_r);
+        if (!have_base) {
+          while (ld_volatile_shared_u32(&s_ready) == 0u) {}
+          __threadfence_block();
+          base = *reinterpret_cast<volatile uint32_t*>(&s_base);
+          have_base = true;
+        }
+        if ((unsigned long long)base + tot > a.capacity) continue;
+        const size_t P0 = (size_t)base + gstart;
+        for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+          const uint32_t i = c0 + lane;
+          int r = 0;                                    // largest r with e_r <= i (fill order -> sector, word)
+#pragma unroll
+          for (int step = 16; step > 0; step >>= 1) {
+            const uint32_t ev = __shfl_sync(0xFFFFFFFFu, e_r, r + step);
+            if (ev <= i) r += step;
+          }
+          const uint32_t k = i - __shfl_sync(0xFFFFFFFFu, e_r, r);
+          const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
+          const uint32_t cs = __shfl_sync(0xFFFFFFFFu, cnt_r, r);
+          const uint32_t ey = __shfl_sync(0xFFFFFFFFu, ey_r, r);
+          if (i < n) {
+            const uint32_t s = sa + (uint32_t)r;
+            const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
+            const uint32_t word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
+            const float x = decode_x(word, B.z, B.w);
+            uint32_t pos = 0;
+            for (uint32_t k2 = 0; k2 < cs; ++k2)
+              pos += before(decode_x(*reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k2), B.z, B.w), k2, x, k);
+            const size_t Q = P0 + ey + pos;
+            a.x[Q] = x; a.z[Q] = A.x; a.yb[Q] = A.y; a.ye[Q] = A.z; a.dxdy[Q] = A.w; a.w[Q] = B.x;
+            a.id[Q] = (__float_as_uint(B.y) << 9) | (word & 0x1FFu);
+            if (view) { a.sx[Q] = x; a.si[Q] = (uint16_t)(gstart + ey + pos); }
+          }
+        }
+        continue;
+      }
       if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)(gstart + e_r);
       const bool in_regs = n <= 32u, in_buf = n <= a.sort_buf;
 
@@ -423,6 +471,8 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   a.carry_in = carry_in;
   a.sx = hits->x_by_sector; a.si = hits->idx_by_sector; a.soff = hits->sector_offsets;
   a.soff_stride = (geom->n_sectors + 2u + 7u) & ~7u;
+  a.order_y = hits->order == UT_ORDER_Y ? 1u : 0u;
+  a.view_ok = (!a.order_y || (geom->flags & UT_GEOM_ROWS_SORTED)) ? 1u : 0u;
   a.ctrl = reinterpret_cast<uint32_t*>(hits->workspace);
   a.flags = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hits->workspace) + 32);
 

@@ -10,10 +10,11 @@ class GpuRunner:
         self.geom = B.ut_geometry_upload(geom_tables)
         self.tables = geom_tables
         self.sector_view = True          # containers carry the optional per-sector view (ut_hits.x_by_sector ...)
+        self.order = "x"                 # order inside a sector group: "x" (default) or "y" (the paper's literal order)
 
     def decode(self, raw, bank_offsets, n_events, capacity):
         B, torch = self.B, self.torch
-        hits = B.Hits(capacity, max(n_events, 1), self.geom, sector_view=self.sector_view)
+        hits = B.Hits(capacity, max(n_events, 1), self.geom, sector_view=self.sector_view, order=self.order)
         raw_d = B.to_device_raw(raw)
         bo_d = B.to_device_u32(bank_offsets)
         B.ut_decode(raw_d, bo_d, n_events, self.geom, hits)

@@ -579,3 +579,65 @@ def test_kick_lut(gpu):
         idx, n, qop, chi2 = tr.numpy()
         assert np.array_equal(idx, t_ref.hit_idx) and np.array_equal(qop.view(np.uint32), t_ref.qop.view(np.uint32))
         assert np.array_equal(chi2.view(np.uint32), t_ref.chi2.view(np.uint32))
+
+
+@pytest.mark.parametrize("name", ["regular", "staggered", "staggered_shuffled_rows"])
+def test_y_order(name):
+    """SURVEY.md 8(f) row 3 (Y-sorted groups): ut_decode with UT_ORDER_Y against the
+    oracle's order "y" bit for bit (container and per-sector view), and compass_track on that container -- per-sector
+    view, re-bucketing, and the search on global memory by two binary searches over Y -- against the oracle's linear
+    scan (mode 1) and its Y-window search (mode 3)."""
+    from gpu_helpers import GpuRunner, compare_decode, compare_tracks
+    from synth import variant as V
+    if name == "regular":
+        geom = synth.make_geometry()
+        b = generate_batch(geom, EventModel(mean_tracks=150.0, efficiency=0.97, noise_mean=1500.0), 19, 40)
+    else:
+        geom = V.make_staggered_geometry(shuffle_rows=name.endswith("shuffled_rows"))
+        b = V.generate_batch_tables(geom, EventModel(mean_tracks=150.0, efficiency=0.97, noise_mean=1500.0), seed=19, n_events=40)
+    runner = GpuRunner(geom)
+    runner.order = "y"
+    h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity, order="y")
+    args = (b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z, b.velo_offsets, b.n_events, geom)
+    B = runner.B
+    for p in (synth.make_compass_params(), synth.make_compass_params(min_hits=4, window_scale=2.0, max_candidates_per_layer=3)):
+        t_ref = oracle.compass(h_ref, *args, p, mode=1)
+        t3 = oracle.compass(h_ref, *args, p, mode=3)
+        assert np.array_equal(t_ref.hit_idx, t3.hit_idx)
+        for path in ("view", "restage", "global"):
+            runner.sector_view = path != "restage"
+            B.ut_tuning_set(compass_hit_stage=0 if path == "global" else -1)
+            try:
+                hits = runner.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+                got, off, st = runner.hits_numpy(hits, b.n_events)
+                compare_decode(h_ref, got, off, st)
+                trk = runner.compass(hits, b, p)
+            finally:
+                B.ut_tuning_set(None)
+            n_diff, _ = compare_tracks(t_ref, trk)
+            assert n_diff == 0, path
+            assert np.array_equal(trk["chi2"].view(np.uint32), t_ref.chi2.view(np.uint32)), path
+            assert np.array_equal(trk["qop"].view(np.uint32), t_ref.qop.view(np.uint32)), path
+        assert (t_ref.n_hits > 0).sum() > 1000
+    # the per-sector view of a Y-ordered container is the container itself, sector by sector in y order (where the
+    # dense sector order is the y order; with shuffled rows ut_decode marks the view unusable and compass_track
+    # re-buckets)
+    runner.sector_view = True
+    hits = runner.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+    n = h_ref.n_hits
+    stride = B.ut_sector_offsets_stride(runner.geom)
+    flags = hits.sector_offsets.cpu().numpy().view(np.uint16).reshape(-1, stride)[:b.n_events, geom.n_sectors + 1]
+    if name.endswith("shuffled_rows"):
+        assert np.all(flags == 0)
+        return
+    assert np.all(flags == 0xA5A5)
+    assert np.array_equal(hits.x_by_sector[:n].cpu().numpy().view(np.uint32), h_ref.x_at_y0[:n].view(np.uint32))
+    ev0 = np.repeat(h_ref.hit_offsets[::geom.n_groups][:-1].astype(np.int64), np.diff(h_ref.hit_offsets[::geom.n_groups].astype(np.int64)))
+    assert np.array_equal(hits.idx_by_sector[:n].cpu().numpy().view(np.uint16).astype(np.int64), np.arange(n) - ev0)
+    # the two-kernel variant searches x-sorted groups only
+    with pytest.raises(B.UTError):
+        import torch
+        B.compass_search_windows(hits, hits.hit_offsets, B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z),
+                                 B.to_device_u32(b.velo_offsets), b.n_events, B.make_config(synth.make_compass_params()), 3,
+                                 torch.empty(b.n_velo_total * 24, dtype=torch.int16, device="cuda"),
+                                 torch.zeros(1, dtype=torch.int32, device="cuda"))
