@@ -300,7 +300,7 @@ void ut_last_launch_info(ut_launch_info* out);
 /* Launch tuning, process-wide (HOST).  -1 = automatic.  The values are read ONCE from the environment when the
  * library is first used (UT_DECODE_BLOCK, UT_DECODE_RAW_STAGE, UT_DECODE_SORT_BUF, UT_DECODE_MAX_CTAS_PER_SM,
  * UT_COMPASS_BLOCK, UT_COMPASS_HIT_STAGE, UT_COMPASS_TRK_STAGE, UT_COMPASS_SPLIT, UT_COMPASS_INTERVAL_MIN,
- * UT_PIPELINE_CHUNK_EVENTS); the
+ * UT_PIPELINE_CHUNK_EVENTS, UT_PIPELINE_ZERO_COPY); the
  * hot-path calls never touch the environment.  ut_tuning_set replaces them (NULL: back to the environment's).
  * Results never depend on these values, only launch shapes and which of the equivalent code paths run. */
 typedef struct {
@@ -314,7 +314,9 @@ typedef struct {
   int32_t compass_split;            /* CTAs sharing one event's track batches (1, 2 or 4) */
   int32_t pipeline_chunk_events;    /* ut_pipeline_run_host: events per overlapped chunk */
   int32_t compass_interval_min;     /* seed partner lists longer than this are searched (interval of d), not walked */
-  int32_t reserved[6];
+  int32_t pipeline_zero_copy;       /* ut_pipeline_run_host: 0 = always stage the raw banks with copies; else the decode
+                                       reads mapped pinned host buffers directly over PCIe */
+  int32_t reserved[5];
 } ut_tuning;
 int32_t ut_tuning_get(ut_tuning* out);
 int32_t ut_tuning_set(const ut_tuning* in);

@@ -307,13 +307,14 @@ def test_invalid_arguments(gpu, wl):
         B.ut_decode(B.to_device_raw(b.raw), B.to_device_u32(b.bank_offsets), -1, gpu.geom, hits)
 
 
+@pytest.mark.parametrize("zero_copy", [0, 1], ids=["staged", "zero_copy"])
 @pytest.mark.parametrize("n_events", [1000, 37])
-def test_host_pipeline_matches_oracle(gpu, wl, n_events):
+def test_host_pipeline_matches_oracle(gpu, wl, n_events, zero_copy):
     """ut_pipeline_run_host (HOST buffers in, HOST track SoA out; the call bench.py's e2e figure times).
     1000 events run as 4 overlapped chunks of 250 (the default is chunks of >= 500 events), 37 events as
     one call: both must equal the oracle element by element."""
     import torch
-    gpu.B.ut_tuning_set(pipeline_chunk_events=250)
+    gpu.B.ut_tuning_set(pipeline_chunk_events=250, pipeline_zero_copy=zero_copy)
     geom, b, p = wl(3, n_events)
     h_ref, t_ref = oracle_run(b, geom, p)
     B = gpu.B
