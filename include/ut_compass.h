@@ -294,19 +294,21 @@ typedef struct {
   int32_t compass_grid, compass_block, compass_smem_bytes, compass_hit_stage;
   int32_t compass_split;            /* CTAs sharing the tracks of one event (1, 2 or 4) */
   int32_t compass_view;             /* 1: the container's per-sector view was offered to the kernel */
+  int32_t decode_hit_stage;         /* hits (padded fill order) of an event the decode CTA orders as a whole; larger events
+                                       and UT_ORDER_Y containers are ordered warp per sector group */
 } ut_launch_info;
 void ut_last_launch_info(ut_launch_info* out);
 
 /* Launch tuning, process-wide (HOST).  -1 = automatic.  The values are read ONCE from the environment when the
  * library is first used (UT_DECODE_BLOCK, UT_DECODE_RAW_STAGE, UT_DECODE_SORT_BUF, UT_DECODE_MAX_CTAS_PER_SM,
  * UT_COMPASS_BLOCK, UT_COMPASS_HIT_STAGE, UT_COMPASS_TRK_STAGE, UT_COMPASS_SPLIT, UT_COMPASS_INTERVAL_MIN,
- * UT_PIPELINE_CHUNK_EVENTS, UT_PIPELINE_ZERO_COPY); the
+ * UT_PIPELINE_CHUNK_EVENTS, UT_PIPELINE_ZERO_COPY, UT_DECODE_HIT_STAGE); the
  * hot-path calls never touch the environment.  ut_tuning_set replaces them (NULL: back to the environment's).
  * Results never depend on these values, only launch shapes and which of the equivalent code paths run. */
 typedef struct {
   int32_t decode_block;             /* threads per decode CTA */
   int32_t decode_raw_stage_bytes;   /* shared-memory staging of an event's raw banks */
-  int32_t decode_sort_buf;          /* per-warp sort buffer, in hits */
+  int32_t decode_sort_buf;          /* per-warp sort buffer of the warp-per-group path, in hits */
   int32_t decode_max_ctas_per_sm;
   int32_t compass_block;            /* threads per Compass CTA */
   int32_t compass_hit_stage;        /* hits of an event staged in shared memory; 0: window search on global memory */
@@ -316,7 +318,8 @@ typedef struct {
   int32_t compass_interval_min;     /* seed partner lists longer than this are searched (interval of d), not walked */
   int32_t pipeline_zero_copy;       /* ut_pipeline_run_host: 0 = always stage the raw banks with copies; else the decode
                                        reads mapped pinned host buffers directly over PCIe */
-  int32_t reserved[5];
+  int32_t decode_hit_stage;         /* largest event (hits) a decode CTA orders as a whole; 0: always warp per sector group */
+  int32_t reserved[4];
 } ut_tuning;
 int32_t ut_tuning_get(ut_tuning* out);
 int32_t ut_tuning_set(const ut_tuning* in);

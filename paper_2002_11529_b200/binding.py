@@ -77,15 +77,15 @@ class ut_tuning(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("decode_block", "decode_raw_stage_bytes", "decode_sort_buf", "decode_max_ctas_per_sm", "compass_block",
                  "compass_hit_stage", "compass_trk_stage", "compass_split", "pipeline_chunk_events",
-                 "compass_interval_min", "pipeline_zero_copy")] + \
-               [("reserved", C.c_int32 * 5)]
+                 "compass_interval_min", "pipeline_zero_copy", "decode_hit_stage")] + \
+               [("reserved", C.c_int32 * 4)]
 
 
 class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_raw_stage_bytes",
                  "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage",
-                 "compass_split", "compass_view")]
+                 "compass_split", "compass_view", "decode_hit_stage")]
 
 
 EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set",

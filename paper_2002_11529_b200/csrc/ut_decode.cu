@@ -6,23 +6,31 @@
 // Here one CTA owns one event at a time (dynamic ticket), keeps the event on chip and touches HBM
 // once per byte:
 //
-//   ticket -> bank offsets (coalesced) -> raw banks of the event by ONE TMA bulk copy into smem
-//   -> thread per bank: header check, sector claim, count   (paper: "calculate number of hits")
-//   -> event total published at once for the chained exclusive prefix over events (decoupled
-//      look-back by warp 0; paper: prefix sum + host sync; here no sync, no second launch); the
-//      event's base is only awaited in front of the first store
-//   -> warp per sector group (dynamic ticket inside the CTA): the lanes gather the group's words
-//      from its banks in fill order (sector, word), decode x, and rank them -- for <= 32 hits in
-//      registers with shuffles, else through a per-warp shared-memory buffer.  Lane order is the
-//      tie-break order, so the rank IS the stable sort by x   (paper: pre-decode + find permutation)
-//   -> SoA store at base + group start + rank; a group is one contiguous window of every array
-//                                                            (paper: decode raw banks in order)
-//   -> optional per-sector view for compass_track (ut_hits.x_by_sector ...): the same warp re-emits the group's x
-//      and container index bucketed per sector (the fill order IS sector-major, so a sector's entries are a
-//      contiguous run and the position inside the run is the rank among the sector's own hits)
+//   ticket -> bank offsets (coalesced, requested before the copy below is awaited) -> raw banks of the
+//      event by ONE TMA bulk copy into shared memory
+//   -> thread per bank: header check, sector claim, count            (paper: "calculate number of hits")
+//   -> CTA-wide exclusive prefix of the counts in dense sector order, in place: the fill order of the
+//      event is (sector, word), so a group's start and size and every bank's offset fall out; the
+//      event total is published at once for the chained exclusive prefix over events (decoupled
+//      look-back by warp 0; paper: prefix sum + host sync; here no sync, no second launch)
+//   -> while warp 0 resolves the look-back, the other warps (named barrier 1):
+//        fill   thread per bank: x and (sector, word) of its words at their place in the PADDED fill
+//               order (every group starts at a multiple of 4, pad slots hold +inf)   (paper: "pre-decode")
+//        rank   thread per hit: one sweep over its group's x (128-bit shared loads, one FSET.BF + one
+//               FADD per comparison) counts the hits with smaller x; atomicMin of the fill index into
+//               slot [group start + count] of the sorted order.  Hits with equal x collide there: the
+//               first in fill order keeps the slot, each later one is moved once to slot + (equal hits
+//               in front of it) -- so the result is the stable sort by x         (paper: "find permutation")
+//   -> output, all warps: thread per slot of the sorted order, the 7 SoA arrays by fully coalesced
+//      stores (a warp writes 32 consecutive elements of each array)    (paper: "decode raw banks in order")
+//      and the hit's entry in the per-sector view for compass_track (ut_hits.x_by_sector ...): the fill
+//      order is sector-major, so a sector's entries are a contiguous run and the position inside the run
+//      is the rank among the bank's own words (a short loop over them)
 //
-// There is no block barrier after the count: warps run independently through the groups.
-// Events or groups that do not fit the staging sizes take slower generic code with the same results.
+// Events whose padded fill order does not fit the buffers, and UT_ORDER_Y containers, are ordered warp per
+// sector group instead (ticket inside the CTA): gather into the warp's slice of the same buffers, rank per
+// chunk of 32 hits (<= for earlier chunks, < for the rest, ties inside the chunk by match.any), groups larger
+// than the slice by recomputation.  Same results on every path (tests/test_gpu_parity.py::test_decode_data_paths).
 // Arithmetic of x follows include/ut_compass.h exactly (__fmul_rn/__fadd_rn, never fused).
 #include <algorithm>
 #include <cstdio>
@@ -45,7 +53,9 @@ struct DecodeArgs {
   uint32_t* ctrl;               // [0] ticket, [1] CTAs done, [2] epoch   ([4], [5]: compass_track's event ticket)
   unsigned long long* flags;    // [n_events] look-back words: epoch:30 | state:2 | value:32
   uint32_t raw_stage_bytes;     // multiple of 16
-  uint32_t sort_buf;            // elements of the per-warp sort buffer (multiple of 32)
+  uint32_t hit_stage;           // largest padded event the CTA orders as a whole (0: always warp per group)
+  uint32_t buf_elems;           // elements of the x / word buffers: max(hit_stage, warps * sort_buf)
+  uint32_t sort_buf;            // elements of a warp's slice of those buffers on the warp-per-group path (multiple of 32)
   const uint32_t* carry_in;     // hits in front of event 0 (chunked pipeline) or null
   float* sx;                    // per-sector view (ut_hits.x_by_sector / idx_by_sector / sector_offsets) or null
   uint16_t* si;
@@ -68,34 +78,46 @@ __device__ __forceinline__ uint32_t ld_volatile_shared_u32(const uint32_t* p) {
   return v;
 }
 
+// 1.0f when a < b (a <= b, a == b), else 0.0f: one FSET.BF, and one FADD to count it (exact below 2^24; the compiler's
+// `n += a < b ? 1 : 0` is three instructions)
+__device__ __forceinline__ float lt(float a, float b) {
+  float d;
+  asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+__device__ __forceinline__ float le(float a, float b) {
+  float d;
+  asm("set.le.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+__device__ __forceinline__ float eq(float a, float b) {
+  float d;
+  asm("set.eq.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+constexpr uint32_t kTieBit = 0x8000u;   // in the (sector << 16 | word) entry: an earlier hit of the group has the same x
+
 // stable order of the fill sequence: (x, position in the fill order)
 __device__ __forceinline__ uint32_t before(float xj, uint32_t j, float x, uint32_t i) {
   return (xj < x || (xj == x && j < i)) ? 1u : 0u;
 }
 
-// Rank of this lane's x among the 32 lanes of the warp in the stable order (x, lane): lanes that hold no
-// element pass +inf and are never counted.  32 unrolled shuffles for "smaller", one match.any for the ties.
-__device__ __forceinline__ uint32_t warp_rank(float x, uint32_t lt_mask) {
-  uint32_t rank = 0;
-#pragma unroll
-  for (int j = 0; j < 32; ++j) rank += __shfl_sync(0xFFFFFFFFu, x, j) < x ? 1u : 0u;
-  const uint32_t ties = __match_any_sync(0xFFFFFFFFu, __float_as_uint(x + 0.0f));      // -0 == +0
-  return rank + __popc(ties & lt_mask);
-}
-
-__global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
+__global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t ns = a.g.n_sectors, ng = a.g.n_groups;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
 
   Carver cv(smem_raw);
-  unsigned char* s_rawstage = cv.take<unsigned char>(a.raw_stage_bytes);
+  // raw banks of the event; once every word is decoded the same bytes hold the sorted order (s_perm)
+  unsigned char* s_rawstage = cv.take<unsigned char>(max(a.raw_stage_bytes, 4u * a.hit_stage));
+  uint32_t* s_perm = reinterpret_cast<uint32_t*>(s_rawstage);
   uint16_t* g_gfirst = cv.take<uint16_t>(ng + 1);
-  uint32_t* s_cnt = cv.take<uint32_t>(ns);
+  uint32_t* s_pstart = cv.take<uint32_t>(ng + 1); // start of every group in the padded fill order (multiples of 4)
+  uint8_t* g_sgrp = cv.take<uint8_t>(ns);         // dense sector -> group (n_groups <= 128)
+  uint32_t* s_cnt = cv.take<uint32_t>(ns + 1);    // bank word counts, then their exclusive prefix in dense sector order
   uint32_t* s_wpos = cv.take<uint32_t>(ns);
-  uint32_t* s_gcnt = cv.take<uint32_t>(ng);
-  float* s_xbuf = cv.take<float>((size_t)nwarps * a.sort_buf);
-  uint32_t* s_wbuf = cv.take<uint32_t>((size_t)nwarps * a.sort_buf);
+  float* s_xbuf = cv.take<float>(a.buf_elems);    // x of the event's hits in padded fill order (warp slices on the group path)
+  uint32_t* s_wbuf = cv.take<uint32_t>(a.buf_elems);   // (dense sector << 16) | raw word, likewise
 
   __shared__ uint64_t s_bar;
   __shared__ int s_event;
@@ -104,6 +126,7 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
 
   // geometry tables: staged once per CTA, reused for every event this CTA takes
   for (uint32_t i = tid; i <= ng; i += nt) g_gfirst[i] = (uint16_t)a.g.group_first_sector[i];
+  for (uint32_t i = tid; i < ns; i += nt) g_sgrp[i] = (uint8_t)a.g.sector_group[i];
   if (tid == 0) {
     mbar_init(&s_bar, 1);
     fence_mbar_init();
@@ -117,6 +140,8 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   uint32_t* wbuf = s_wbuf + (size_t)warp * a.sort_buf;
 
   for (;;) {
+    // (drawing the ticket one event ahead was measured: 59 -> 71 us on config 3.  A CTA that holds its next event
+    //  while it is still busy keeps faster CTAs from taking it.)
     if (tid == 0) s_event = (int)atomicAdd(a.ctrl, 1u);
     __syncthreads();                     // also: every warp is done with the previous event's tables
     const int e = s_event;
@@ -125,8 +150,16 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
     // ---- bank offsets of the event, table reset -------------------------------------------------------
     const uint32_t* bo = a.bank_offsets + (size_t)e * ns;
     const uint32_t b0 = __ldg(bo), b1 = __ldg(bo + ns);          // first byte and end of the event's banks
+    // this thread's bank offsets are requested now and used after the raw copy has landed
+    constexpr int kPre = 3;
+    uint32_t o0r[kPre], o1r[kPre];
+#pragma unroll
+    for (int k = 0; k < kPre; ++k) {
+      const uint32_t j = (uint32_t)tid + (uint32_t)k * (uint32_t)nt;
+      o0r[k] = j < ns ? __ldg(bo + j) : 0u;
+      o1r[k] = j < ns ? __ldg(bo + j + 1) : 0u;
+    }
     for (uint32_t i = tid; i < ns; i += nt) { s_cnt[i] = 0; s_wpos[i] = kInvalid; }
-    for (uint32_t i = tid; i < ng; i += nt) s_gcnt[i] = 0;
     if (tid == 0) { s_ready = 0; s_gticket = 0; }
     __syncthreads();
 
@@ -146,48 +179,84 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
     }
 
     // ---- per bank: header check, sector claim, count ---------------------------------
-    uint32_t local = 0, st = range_ok ? 0u : (uint32_t)UT_STATUS_BAD_BANK_SIZE;
+    uint32_t st = range_ok ? 0u : (uint32_t)UT_STATUS_BAD_BANK_SIZE;
     if (range_ok) {
-      for (uint32_t j = tid; j < ns; j += nt) {
-        const uint32_t o0 = __ldg(bo + j), o1 = __ldg(bo + j + 1);
-        if ((o0 & 3u) || o1 < o0 + 6u || o0 < b0 || o1 > b1) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
+      auto bank = [&](uint32_t o0, uint32_t o1) {
+        if ((o0 & 3u) || o1 < o0 + 6u || o0 < b0 || o1 > b1) { st |= UT_STATUS_BAD_BANK_SIZE; return; }
         const uint32_t rel = o0 - b0a;
         const uint32_t rid = *reinterpret_cast<const uint32_t*>(rawp + rel);
         const uint32_t cnt = *reinterpret_cast<const uint32_t*>(rawp + rel + 4) & 0xFFFFu;
         uint32_t s = kInvalid;
         if (rid < a.g.id_table_size) s = __ldg(a.g.id_to_sector + rid);   // 4 KB table, L1 / L2 resident
-        if (s >= ns) { st |= UT_STATUS_UNKNOWN_SECTOR; continue; }
-        if (o1 - o0 != ((6u + 2u * cnt + 3u) & ~3u)) { st |= UT_STATUS_BAD_BANK_SIZE; continue; }
-        if (atomicCAS(&s_wpos[s], kInvalid, rel + 6u) != kInvalid) { st |= UT_STATUS_DUPLICATE_SECTOR; continue; }
+        if (s >= ns) { st |= UT_STATUS_UNKNOWN_SECTOR; return; }
+        if (o1 - o0 != ((6u + 2u * cnt + 3u) & ~3u)) { st |= UT_STATUS_BAD_BANK_SIZE; return; }
+        if (atomicCAS(&s_wpos[s], kInvalid, rel + 6u) != kInvalid) { st |= UT_STATUS_DUPLICATE_SECTOR; return; }
         s_cnt[s] = cnt;
-        if (cnt) atomicAdd(&s_gcnt[__ldg(a.g.sector_group + s)], cnt);
-        local += cnt;
-      }
+      };
+#pragma unroll
+      for (int k = 0; k < kPre; ++k)
+        if ((uint32_t)tid + (uint32_t)k * (uint32_t)nt < ns) bank(o0r[k], o1r[k]);
+      for (uint32_t j = (uint32_t)tid + (uint32_t)kPre * (uint32_t)nt; j < ns; j += nt) bank(__ldg(bo + j), __ldg(bo + j + 1));
     }
     if (st) atomicOr(&s_status, st);
-    local = warp_sum(local);
-    if (lane == 0) s_warp[warp] = local;
-    __syncthreads();                     // last block barrier of the event: warps run on their own from here
+    __syncthreads();
 
-    uint32_t tot = warp_sum(lane < nwarps ? s_warp[lane] : 0u);
-    // exclusive scan of the group counts, 4 groups per lane (ng <= 128), kept in registers by every warp
-    uint32_t gc[4], gs[4];
+    // ---- exclusive prefix of the bank counts in dense sector order, in place -----------------
+    // The fill order of the event is (dense sector, word), so s_cnt[s] becomes the place of sector s's first word in
+    // it; a group's sectors are contiguous: its start and size, and every bank's offset inside it, fall out.
+    uint32_t tot;
     {
-      uint32_t run = 0;
+      const uint32_t per = ((ns + (uint32_t)nt - 1u) / (uint32_t)nt) | 1u;     // odd: conflict-free strided rows
+      const uint32_t s0 = min((uint32_t)tid * per, ns), s1 = min(s0 + per, ns);
+      uint32_t sum = 0;
+      for (uint32_t q = s0; q < s1; ++q) sum += s_cnt[q];
+      const uint32_t incl = warp_incl_scan(sum, lane);
+      if (lane == 31) s_warp[warp] = incl;
+      __syncthreads();
+      const uint32_t wv = lane < nwarps ? s_warp[lane] : 0u;
+      const uint32_t wi = warp_incl_scan(wv, lane);
+      tot = __shfl_sync(0xFFFFFFFFu, wi, 31);
+      uint32_t run = __shfl_sync(0xFFFFFFFFu, wi - wv, warp) + incl - sum;
+      for (uint32_t q = s0; q < s1; ++q) { const uint32_t c = s_cnt[q]; s_cnt[q] = run; run += c; }
+      if (tid == 0) s_cnt[ns] = tot;
+    }
+    __syncthreads();                     // last block barrier of the event: warps run on their own from here
+    const uint32_t* s_start = s_cnt;
+
+    // ---- padded fill order: every group starts at a multiple of 4 so that the rank sweep reads whole float4 rows ----
+    if (warp == nwarps - 1) {
+      uint32_t gp[4], run = 0;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const uint32_t g = lane * 4 + q;
-        gc[q] = g < ng ? s_gcnt[g] : 0u;
-        run += gc[q];
+        gp[q] = g < ng ? (s_start[g_gfirst[g + 1]] - s_start[g_gfirst[g]] + 3u) & ~3u : 0u;
+        run += gp[q];
       }
-      uint32_t ex = warp_incl_scan(run, lane) - run;
+      const uint32_t incl = warp_incl_scan(run, lane);
+      uint32_t ex = incl - run;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) { gs[q] = ex; ex += gc[q]; }
+      for (int q = 0; q < 4; ++q) {
+        const uint32_t g = lane * 4 + q;
+        if (g < ng) s_pstart[g] = ex;
+        ex += gp[q];
+      }
+      if (lane == 31) s_pstart[ng] = incl;
     }
+    __syncthreads();
+    const uint32_t ptot = s_pstart[ng];
+    // The whole event is ordered by the CTA when its padded fill order fits the buffers; otherwise (and for
+    // UT_ORDER_Y) a warp takes one sector group at a time further down.
+    const bool cta_path = !a.order_y && nwarps > 1 && ptot <= a.hit_stage;
 
     // ---- event base: warp 0 publishes the total and resolves the chained prefix over events -----------
     uint32_t base = 0;
     bool have_base = false;
+    // per-sector view: usable by compass_track iff the event fits u16 positions and no group takes the generic path
+    bool big = false;
+    if (!cta_path)
+      for (uint32_t g = lane; g < ng; g += 32u) big |= s_start[g_gfirst[g + 1]] - s_start[g_gfirst[g]] > a.sort_buf;
+    const bool view = a.soff != nullptr && a.view_ok && tot <= 65535u && !__any_sync(0xFFFFFFFFu, big);
+    uint16_t* soff = a.soff ? a.soff + (size_t)e * a.soff_stride : nullptr;
     if (warp == 0) {
       base = event_base_lookback(a.flags, e, tot, s_epoch, lane, a.carry_in);
       have_base = true;
@@ -197,22 +266,113 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         *reinterpret_cast<volatile uint32_t*>(&s_ready) = 1u;
         if ((unsigned long long)base + tot > a.capacity) atomicOr(&s_status, (uint32_t)UT_STATUS_CAPACITY);
         if (e == a.n_events - 1) a.hit_offsets[(size_t)a.n_events * ng] = base + tot;
+        if (soff) {
+          soff[ns] = (uint16_t)tot;
+          soff[ns + 1] = (view && (unsigned long long)base + tot <= a.capacity) ? (uint16_t)UT_SECTOR_INDEX_VALID : (uint16_t)0;
+        }
       }
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const uint32_t g = lane * 4 + q;
-        if (g < ng) a.hit_offsets[(size_t)e * ng + g] = base + gs[q];
-      }
-    }
-    // per-sector view: usable by compass_track iff the event fits u16 positions and no group takes the generic path
-    const bool view = a.soff != nullptr && a.view_ok && tot <= 65535u &&
-                      !__any_sync(0xFFFFFFFFu, gc[0] > a.sort_buf || gc[1] > a.sort_buf || gc[2] > a.sort_buf || gc[3] > a.sort_buf);
-    uint16_t* soff = a.soff ? a.soff + (size_t)e * a.soff_stride : nullptr;
-    if (warp == 0 && lane == 0 && soff) {
-      soff[ns] = (uint16_t)tot;
-      soff[ns + 1] = (view && (unsigned long long)base + tot <= a.capacity) ? (uint16_t)UT_SECTOR_INDEX_VALID : (uint16_t)0;
+      for (uint32_t g = lane; g < ng; g += 32u) a.hit_offsets[(size_t)e * ng + g] = base + s_start[g_gfirst[g]];
     }
     if (tot == 0 && !view) continue;
+
+    if (cta_path) {
+      // Warp 0 is busy with the look-back; the other warps ("workers", named barrier 1) fill, clear and rank.
+      const uint32_t nw = (uint32_t)nt - 32u;
+      if (warp != 0) {
+        const uint32_t wt = (uint32_t)tid - 32u;
+        // x order: a sector's run of the view starts where its words start in the fill order
+        if (view)
+          for (uint32_t q = wt; q < ns; q += nw) soff[q] = (uint16_t)s_start[q];
+        // ---- fill: thread per bank, x and (sector, word) of its words at their place in the padded fill order
+        //      (paper: "pre-decode")
+        for (uint32_t sct = wt; sct < ns; sct += nw) {
+          const uint32_t es = s_start[sct], c = s_start[sct + 1] - es;
+          if (c == 0) continue;
+          const uint32_t g = g_sgrp[sct];
+          const uint32_t p0 = s_pstart[g] + (es - s_start[g_gfirst[g]]);
+          const float2 xp = __ldg(reinterpret_cast<const float2*>(a.g.sector_rows + 2 * sct + 1) + 1);      // {x0, pitch}
+          const uint16_t* wd = reinterpret_cast<const uint16_t*>(rawp + s_wpos[sct]);
+          for (uint32_t k = 0; k < c; ++k) {
+            const uint32_t word = wd[k];
+            s_xbuf[p0 + k] = decode_x(word, xp.x, xp.y);
+            s_wbuf[p0 + k] = (sct << 16) | (word & 0x3FFu);   // (ADC bits dropped: bit 15 is kTieBit)
+          }
+        }
+        for (uint32_t g = wt; g < ng; g += nw) {          // pad slots: +inf is never "smaller", kInvalid marks them
+          const uint32_t n = s_start[g_gfirst[g + 1]] - s_start[g_gfirst[g]];
+          for (uint32_t q = s_pstart[g] + n; q < s_pstart[g + 1]; ++q) { s_xbuf[q] = __int_as_float(0x7F800000); s_wbuf[q] = kInvalid; }
+        }
+        asm volatile("bar.sync 1, %0;" ::"r"(nw) : "memory");      // every word is decoded: the raw bytes are dead
+        for (uint32_t q = wt; q < ptot; q += nw) s_perm[q] = kInvalid;
+        asm volatile("bar.sync 1, %0;" ::"r"(nw) : "memory");
+        // ---- rank: thread per hit, one sweep over its group counts the hits with smaller x ("find permutation",
+        //      PAPER.md:273).  Hits with equal x get the same count: the first of them in fill order keeps the slot
+        //      (atomicMin), each of the others is moved once to slot + (equal hits in front of it).
+        for (uint32_t pi = wt; pi < ptot; pi += nw) {
+          const uint32_t rw = s_wbuf[pi];
+          if (rw == kInvalid) continue;
+          const float x = s_xbuf[pi];
+          const uint32_t g = g_sgrp[rw >> 16];
+          const uint32_t pga = s_pstart[g], pge = s_pstart[g + 1];
+          float r0 = 0.f, r1 = 0.f;
+          for (uint32_t j = pga; j < pge; j += 4u) {
+            const float4 v = *reinterpret_cast<const float4*>(s_xbuf + j);
+            r0 += lt(v.x, x); r1 += lt(v.y, x);
+            r0 += lt(v.z, x); r1 += lt(v.w, x);
+          }
+          const uint32_t rank = (uint32_t)(r0 + r1);
+          const uint32_t old = atomicMin(&s_perm[pga + rank], pi);
+          if (old != kInvalid) {                            // equal x: re-home the later one of the two
+            const uint32_t later = max(old, pi);
+            float o0 = 0.f, o1 = 0.f;
+            uint32_t j = pga;
+            for (; j + 4u <= later; j += 4u) {
+              const float4 v = *reinterpret_cast<const float4*>(s_xbuf + j);
+              o0 += eq(v.x, x); o1 += eq(v.y, x);
+              o0 += eq(v.z, x); o1 += eq(v.w, x);
+            }
+            for (; j < later; ++j) o0 += eq(s_xbuf[j], x);
+            s_perm[pga + rank + (uint32_t)(o0 + o1)] = later;
+            atomicOr(&s_wbuf[later], kTieBit);              // its place in its bank's run needs the exact order
+          }
+        }
+      }
+      __syncthreads();                                       // order complete, base known
+      base = s_base;
+      if ((unsigned long long)base + tot > a.capacity) continue;        // flagged by warp 0; offsets stay exact
+      // ---- output: thread per slot of the sorted order, coalesced SoA stores ("decode raw banks in order",
+      //      PAPER.md:274); the per-sector view entry of the same hit goes to its rank among its own bank's words
+      for (uint32_t q = tid; q < ptot; q += nt) {
+        const uint32_t pi = s_perm[q];
+        if (pi == kInvalid) continue;
+        const uint32_t rw = s_wbuf[pi], sct = rw >> 16;
+        const float x = s_xbuf[pi];
+        const uint32_t g = g_sgrp[sct];
+        const uint32_t pga = s_pstart[g], gfs = s_start[g_gfirst[g]];
+        const uint32_t hpos = gfs + (q - pga);               // place in the event's part of the container
+        const float4 A = __ldg(a.g.sector_rows + 2 * sct), B = __ldg(a.g.sector_rows + 2 * sct + 1);
+        const size_t P = (size_t)base + hpos;
+        a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
+        a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
+        if (view) {
+          const uint32_t es = s_start[sct], cs = s_start[sct + 1] - es, pes = pga + (es - gfs);
+          uint32_t pos = 0;
+          if (rw & kTieBit) { for (uint32_t j = pes; j < pes + cs; ++j) pos += before(s_xbuf[j], j, x, pi); }
+          else {
+            float f = 0.f;
+            for (uint32_t j = pes; j < pes + cs; ++j) f += lt(s_xbuf[j], x);
+            pos = (uint32_t)f;
+          }
+          const size_t Q = (size_t)base + es + pos;
+          a.sx[Q] = x;
+          a.si[Q] = (uint16_t)hpos;
+        }
+      }
+      continue;
+    }
+    // x order: a sector's run of the view starts where its words start in the fill order
+    if (view && !a.order_y)
+      for (uint32_t q = tid; q < ns; q += nt) soff[q] = (uint16_t)s_start[q];
 
     // ---- warp per sector group (ticket inside the CTA) --------------------------------------------------
     for (;;) {
@@ -220,20 +380,16 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
       if (lane == 0) g = atomicAdd(&s_gticket, 1u);
       g = __shfl_sync(0xFFFFFFFFu, g, 0);
       if (g >= ng) break;
-      const uint32_t q4 = g & 3u;                       // warp-uniform: pick the register, then the lane
-      const uint32_t n = __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gc[0] : q4 == 1 ? gc[1] : q4 == 2 ? gc[2] : gc[3], (int)(g >> 2));
-      const uint32_t gstart =
-          __shfl_sync(0xFFFFFFFFu, q4 == 0 ? gs[0] : q4 == 1 ? gs[1] : q4 == 2 ? gs[2] : gs[3], (int)(g >> 2));
-      const uint32_t sa = g_gfirst[g], nsec = g_gfirst[g + 1] - sa;      // nsec <= 32 (ut_geometry_upload)
+      const uint32_t sa = g_gfirst[g], sb = g_gfirst[g + 1], nsec = sb - sa;   // nsec <= 32 (ut_geometry_upload)
+      const uint32_t gstart = s_start[sa], n = s_start[sb] - gstart;
       if (n == 0) {
-        if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)gstart;
+        if (view && a.order_y && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)gstart;
         continue;
       }
-      // the group's banks: word count and word position per sector, exclusive prefix = fill order
-      const uint32_t cnt_r = (uint32_t)lane < nsec ? s_cnt[sa + lane] : 0u;
+      // the group's banks: word position, word count and offset inside the group's fill order, one bank per lane
       const uint32_t wpos_r = (uint32_t)lane < nsec ? s_wpos[sa + lane] : 0u;
-      const uint32_t e_incl = warp_incl_scan(cnt_r, lane);
-      const uint32_t e_r = (uint32_t)lane < nsec ? e_incl - cnt_r : n;   // lanes past the group: never selected
+      const uint32_t e_r = (uint32_t)lane < nsec ? s_start[sa + lane] - gstart : n;   // lanes past the group: never selected
+      const uint32_t cnt_r = (uint32_t)lane < nsec ? s_start[sa + lane + 1] - gstart - e_r : 0u;
       if (a.order_y) {
         // ---- UT_ORDER_Y: sectors in (y_begin, dense index) order, x-sorted inside a sector.  A hit's
         // place = its sector's start in that order + its rank among the words of its own bank: no group-wide rank.
@@ -279,113 +435,71 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         }
         continue;
       }
-      if (view && (uint32_t)lane < nsec) soff[sa + lane] = (uint16_t)(gstart + e_r);
-      const bool in_regs = n <= 32u, in_buf = n <= a.sort_buf;
-
-      // gather: element i of the fill order -> (sector r, word k), decode x
-      float x = 0.f;
-      uint32_t rw = 0;                                  // (sector-in-group << 16) | raw word
-      float4 Brow = make_float4(0.f, 0.f, 0.f, 0.f);
-      for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
-        const uint32_t i = c0 + lane;
-        int r = 0;                                      // largest r with e_r <= i
+      if (n <= a.sort_buf) {
+        // ---- gather: element i of the fill order -> (sector r, word k); x and the word go to the warp's buffer ----
+        for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+          const uint32_t i = c0 + lane;
+          int r = 0;                                    // largest r with e_r <= i
 #pragma unroll
-        for (int step = 16; step > 0; step >>= 1) {
-          const uint32_t ev = __shfl_sync(0xFFFFFFFFu, e_r, r + step);
-          if (ev <= i) r += step;
-        }
-        const uint32_t k = i - __shfl_sync(0xFFFFFFFFu, e_r, r);
-        const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
-        if (i < n) {
-          const uint32_t word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
-          Brow = __ldg(a.g.sector_rows + 2 * (sa + r) + 1);            // {weight, raw id, x0, pitch}
-          x = decode_x(word, Brow.z, Brow.w);
-          rw = ((uint32_t)r << 16) | word;
-          if (!in_regs && in_buf) { xbuf[i] = x; wbuf[i] = rw; }
-        }
-        if (!in_buf) break;                             // generic path gathers again below
-      }
-
-      if (!have_base) {                                 // the event's base is needed from here on
-        while (ld_volatile_shared_u32(&s_ready) == 0u) {}
-        __threadfence_block();
-        base = *reinterpret_cast<volatile uint32_t*>(&s_base);
-        have_base = true;
-      }
-      if ((unsigned long long)base + tot > a.capacity) continue;        // flagged by warp 0; offsets stay exact
-      const size_t P0 = (size_t)base + gstart;
-
-      if (in_regs) {
-        // ---- <= 32 hits: rank in registers, lane order = fill order --------------------------------------
-        const uint32_t rank = warp_rank((uint32_t)lane < n ? x : __int_as_float(0x7F800000), lt_mask);
-        if ((uint32_t)lane < n) {
-          const uint32_t s = sa + (rw >> 16);
-          const float4 A = __ldg(a.g.sector_rows + 2 * s), B = Brow;
-          const size_t P = P0 + rank;
-          a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
-          a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
-        }
-        if (view) {
-          // per-sector view: lane r takes the hit of rank r (container order); its position inside its sector's run
-          // is its rank among the lanes of the same sector
-          if ((uint32_t)lane < n) { xbuf[rank] = x; wbuf[rank] = rw >> 16; }
-          __syncwarp();
-          const float xs = (uint32_t)lane < n ? xbuf[lane] : 0.f;
-          const uint32_t ss = (uint32_t)lane < n ? wbuf[lane] : 0xFFFFu;
-          const uint32_t peers = __match_any_sync(0xFFFFFFFFu, ss);
-          const uint32_t es = __shfl_sync(0xFFFFFFFFu, e_r, (int)(ss & 31u));
-          if ((uint32_t)lane < n) {
-            const size_t Q = P0 + es + __popc(peers & lt_mask);
-            a.sx[Q] = xs;
-            a.si[Q] = (uint16_t)(gstart + lane);
+          for (int step = 16; step > 0; step >>= 1) {
+            const uint32_t ev = __shfl_sync(0xFFFFFFFFu, e_r, r + step);
+            if (ev <= i) r += step;
           }
-          __syncwarp();                                 // the buffers are reused by the warp's next group
+          const uint32_t k = i - __shfl_sync(0xFFFFFFFFu, e_r, r);
+          const uint32_t wp = __shfl_sync(0xFFFFFFFFu, wpos_r, r);
+          if (i < n) {
+            const uint32_t word = *reinterpret_cast<const uint16_t*>(rawp + wp + 2u * k);
+            const float2 xp = __ldg(reinterpret_cast<const float2*>(a.g.sector_rows + 2 * (sa + r) + 1) + 1);   // {x0, pitch}
+            xbuf[i] = decode_x(word, xp.x, xp.y);
+            wbuf[i] = ((uint32_t)r << 16) | word;       // (sector in group, raw word)
+          }
         }
-      } else if (in_buf) {
-        // ---- <= sort_buf hits: rank against the warp's shared-memory copy -----------------------------------
-        const uint32_t npad = (n + 3u) & ~3u;          // pad the tail of the buffer with +inf (never "smaller")
+        const uint32_t npad = (n + 3u) & ~3u;           // pad the tail of the buffer with +inf (never "smaller")
         if (n + lane < npad) xbuf[n + lane] = __int_as_float(0x7F800000);
         __syncwarp();
+        if (!have_base) {                               // the event's base is needed from here on
+          while (ld_volatile_shared_u32(&s_ready) == 0u) {}
+          __threadfence_block();
+          base = *reinterpret_cast<volatile uint32_t*>(&s_base);
+          have_base = true;
+        }
+        if ((unsigned long long)base + tot > a.capacity) continue;      // flagged by warp 0; offsets stay exact
+        const size_t P0 = (size_t)base + gstart;
+        // ---- rank = place in the stable order (x, fill index): one sweep over the buffer per chunk of 32 hits.
+        // Earlier chunks win ties (<=), the own and later chunks never (<); ties inside the chunk by one match.any.
         for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
           const uint32_t i = c0 + lane;
           const bool valid = i < n;
           const float xi = valid ? xbuf[i] : __int_as_float(0x7F800000);
-          // elements of earlier chunks come first on ties, later chunks never; this chunk: warp_rank
-          uint32_t rank = warp_rank(xi, lt_mask);
+          float r0 = 0.f, r1 = 0.f;
           for (uint32_t j = 0; j < c0; j += 4u) {
             const float4 v = *reinterpret_cast<const float4*>(xbuf + j);
-            rank += (v.x <= xi ? 1u : 0u) + (v.y <= xi ? 1u : 0u) + (v.z <= xi ? 1u : 0u) + (v.w <= xi ? 1u : 0u);
+            r0 += le(v.x, xi); r1 += le(v.y, xi);
+            r0 += le(v.z, xi); r1 += le(v.w, xi);
           }
-          for (uint32_t j = c0 + 32u; j < npad; j += 4u) {
+          for (uint32_t j = c0; j < npad; j += 4u) {
             const float4 v = *reinterpret_cast<const float4*>(xbuf + j);
-            rank += (v.x < xi ? 1u : 0u) + (v.y < xi ? 1u : 0u) + (v.z < xi ? 1u : 0u) + (v.w < xi ? 1u : 0u);
+            r0 += lt(v.x, xi); r1 += lt(v.y, xi);
+            r0 += lt(v.z, xi); r1 += lt(v.w, xi);
           }
+          const uint32_t ties = __match_any_sync(0xFFFFFFFFu, __float_as_uint(xi + 0.0f));      // -0 == +0
+          const uint32_t rank = (uint32_t)(r0 + r1) + __popc(ties & lt_mask);
+          const uint32_t rwi = valid ? wbuf[i] : 0u;
+          const uint32_t es = __shfl_sync(0xFFFFFFFFu, e_r, (int)(rwi >> 16));
+          const uint32_t cs = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)(rwi >> 16));
           if (valid) {
-            const uint32_t rwi = wbuf[i];
             const uint32_t s = sa + (rwi >> 16);
             const float4 A = __ldg(a.g.sector_rows + 2 * s), B = __ldg(a.g.sector_rows + 2 * s + 1);
             const size_t P = P0 + rank;
             a.x[P] = xi; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
             a.id[P] = (__float_as_uint(B.y) << 9) | (rwi & 0x1FFu);
-            if (view) wbuf[i] = (rwi & 0xFFFF0000u) | rank;          // (sector in group, rank) for the view below
-          }
-        }
-        if (view) {
-          // per-sector view: the fill order is sector-major, so the entries of sector r are elements
-          // [e_r, e_r + cnt_r) of the buffer; the position inside the run is the rank among them
-          __syncwarp();
-          for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
-            const uint32_t i = c0 + lane;
-            const bool valid = i < n;
-            const uint32_t rwi = valid ? wbuf[i] : 0u;
-            const uint32_t rank = rwi & 0xFFFFu;
-            const uint32_t es = __shfl_sync(0xFFFFFFFFu, e_r, (int)(rwi >> 16));
-            const uint32_t cs = __shfl_sync(0xFFFFFFFFu, cnt_r, (int)(rwi >> 16));
-            if (valid) {
+            if (view) {
+              // per-sector view: the fill order is sector-major, so the sector's words are elements [es, es + cs) of
+              // the buffer; the place inside the sector's run is the rank among them
               uint32_t pos = 0;
-              for (uint32_t j = es; j < es + cs; ++j) pos += (wbuf[j] & 0xFFFFu) < rank ? 1u : 0u;
+              for (uint32_t j = es; j < es + cs; ++j) pos += before(xbuf[j], j, xi, i);
               const size_t Q = P0 + es + pos;
-              a.sx[Q] = xbuf[i];
+              a.sx[Q] = xi;
               a.si[Q] = (uint16_t)(gstart + rank);
             }
           }
@@ -393,6 +507,14 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
         __syncwarp();                                   // the buffer is reused by the warp's next group
       } else {
         // ---- generic path (group larger than the sort buffer): rank by recomputation, O(n^2) --------------
+        if (!have_base) {
+          while (ld_volatile_shared_u32(&s_ready) == 0u) {}
+          __threadfence_block();
+          base = *reinterpret_cast<volatile uint32_t*>(&s_base);
+          have_base = true;
+        }
+        if ((unsigned long long)base + tot > a.capacity) continue;
+        const size_t P0 = (size_t)base + gstart;
         for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
           const uint32_t i = c0 + lane;
           int r = 0;
@@ -445,11 +567,11 @@ __global__ void __launch_bounds__(512) ut_decode_kernel(const DecodeArgs a) {
   }
 }
 
-static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, uint32_t sort_buf, int block) {
-  size_t b = align16(raw_stage);
-  b += align16((size_t)(ng + 1) * 2);
-  b += 2 * align16((size_t)ns * 4) + align16((size_t)ng * 4);
-  b += 2 * align16((size_t)(block / 32) * sort_buf * 4);
+static size_t decode_smem_bytes(uint32_t ns, uint32_t ng, uint32_t raw_stage, uint32_t hit_stage, uint32_t buf_elems) {
+  size_t b = align16(std::max<size_t>(raw_stage, 4 * (size_t)hit_stage));
+  b += align16((size_t)(ng + 1) * 2) + align16((size_t)(ng + 1) * 4) + align16((size_t)ns);
+  b += align16((size_t)(ns + 1) * 4) + align16((size_t)ns * 4);
+  b += 2 * align16((size_t)buf_elems * 4);
   return b;
 }
 
@@ -482,25 +604,51 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   const unsigned long long stage_hits = std::min<unsigned long long>(((avg + 255) / 256) * 256 + 256, 1u << 16);
   uint32_t raw_stage = (uint32_t)align16(8u * ns + 2u * stage_hits + 32u);
   raw_stage = (uint32_t)tuned(tune.decode_raw_stage_bytes, (int)raw_stage) & ~15u;
-  // per-warp sort buffer: twice the mean group size, at least 64, a multiple of 32
+  // the capacity bound counts the pad half-word of every odd bank as a hit: about n_sectors / 2 per event
+  const unsigned long long est = avg > ns ? avg - ns / 2 : avg;
+  // 12 warps order an event together (measured on config 3: 256 threads 72 us, 384 59 us, 512 63 us); busy events get 16
+  int block = tuned(tune.decode_block, avg > 4096 ? 512 : 384);
+  block = std::max(64, std::min(512, (block / 32) * 32));
+  const uint32_t nwarps = (uint32_t)block / 32u;
+  // the warp-per-group path (UT_ORDER_Y, oversize events) slices the same buffers: twice the mean group, at least 64
   uint32_t sort_buf = (uint32_t)std::min<unsigned long long>(((2 * avg / ng + 31) / 32) * 32 + 32, 1024);
   sort_buf = std::max(64u, sort_buf);
   sort_buf = ((uint32_t)tuned(tune.decode_sort_buf, (int)sort_buf) + 31u) & ~31u;
-  // 5-warp CTAs keep a 1000-event batch resident at once (7 per SM); busy events get 8 warps per event
-  int block = tuned(tune.decode_block, avg > 4096 ? 256 : 160);
-  block = std::max(64, std::min(512, (block / 32) * 32));
-  size_t smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
   const size_t budget = (size_t)max_smem;
+  // CTA-wide order: the event's padded fill order (<= 3 pad slots per group) with 1/8 (else 1/16) of slack; the smaller
+  // slack is taken when it lets one more CTA stay resident
+  auto stage_for = [&](unsigned long long slack_div, unsigned long long slack_min) {
+    return (uint32_t)std::min<unsigned long long>(((est + est / slack_div + slack_min + 3ull * ng + 31) / 32) * 32, 1u << 16);
+  };
+  uint32_t hit_stage = stage_for(8, 128);
+  if (hits->order == UT_ORDER_Y) hit_stage = 0;
+  else if (tune.decode_hit_stage >= 0) hit_stage = ((uint32_t)tune.decode_hit_stage + 31u) & ~31u;
+  else {
+    const uint32_t tight = stage_for(16, 64);
+    const size_t s8 = decode_smem_bytes(ns, ng, raw_stage, hit_stage, std::max(hit_stage, nwarps * sort_buf)) + 1024;
+    const size_t s16 = decode_smem_bytes(ns, ng, raw_stage, tight, std::max(tight, nwarps * sort_buf)) + 1024;
+    if ((size_t)dev.smem_per_sm / s16 > (size_t)dev.smem_per_sm / s8 || s8 - 1024 > budget) hit_stage = tight;
+  }
+  auto smem_of = [&]() { return decode_smem_bytes(ns, ng, raw_stage, hit_stage, std::max(hit_stage, nwarps * sort_buf)); };
+  size_t smem = smem_of();
+  if (smem > budget && tune.decode_hit_stage < 0) { hit_stage = 0; smem = smem_of(); }   // events too large to order as a whole
   while (smem > budget && raw_stage > 4096) {            // oversize events read their banks from global memory
     raw_stage = (raw_stage / 2) & ~15u;
-    smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
+    smem = smem_of();
   }
   while (smem > budget && sort_buf > 32) {
     sort_buf -= 32;
-    smem = decode_smem_bytes(ns, ng, raw_stage, sort_buf, block);
+    smem = smem_of();
+  }
+  while (smem > budget && hit_stage > 0) {
+    hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
+    smem = smem_of();
   }
   if (smem > budget) return UT_ERR_LIMIT;
-  a.raw_stage_bytes = raw_stage; a.sort_buf = sort_buf;
+  a.raw_stage_bytes = raw_stage; a.hit_stage = hit_stage;
+  a.buf_elems = std::max(hit_stage, nwarps * sort_buf);
+  if (tune.decode_sort_buf < 0) sort_buf = std::min(1024u, (a.buf_elems / nwarps) & ~31u);   // the slices take what is there
+  a.sort_buf = sort_buf;
 
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ut_decode_kernel, block, smem));
@@ -511,7 +659,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   UTC_CUDA(cudaGetLastError());
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.decode_grid = grid; li.decode_block = block; li.decode_smem_bytes = (int)smem;
-  li.decode_raw_stage_bytes = (int)raw_stage; li.decode_sort_buf = (int)sort_buf;
+  li.decode_raw_stage_bytes = (int)raw_stage; li.decode_sort_buf = (int)sort_buf; li.decode_hit_stage = (int)hit_stage;
   return UT_OK;
 }
 

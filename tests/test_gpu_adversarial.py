@@ -202,7 +202,7 @@ def test_guard_bands(gpu, geom, wl, case):
         g, b, p = wl(4, 12)
     elif case == "generic_paths":
         g, b, p = wl(2, 12)
-        B.ut_tuning_set(decode_sort_buf=32, decode_raw_stage_bytes=4096, compass_hit_stage=512)
+        B.ut_tuning_set(decode_sort_buf=32, decode_raw_stage_bytes=4096, compass_hit_stage=512, decode_hit_stage=0)
     elif case == "capacity":
         g, b, p = wl(2, 12)
         cap = int(oracle.decode(b.raw, b.bank_offsets, b.n_events, g, b.hit_capacity).hit_offsets[64 * 7]) + 1

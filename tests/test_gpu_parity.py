@@ -77,6 +77,45 @@ def test_sector_view_contents(gpu, wl):
         check_sector_view(gpu, geom, b, hits, h_ref)
 
 
+@pytest.mark.parametrize("tuning", [dict(), dict(decode_hit_stage=0), dict(decode_hit_stage=1024),
+                                    dict(decode_block=64), dict(decode_block=512, decode_raw_stage_bytes=4096),
+                                    dict(decode_hit_stage=0, decode_sort_buf=64, decode_block=96)],
+                         ids=["cta", "warp_per_group", "stage_too_small", "block64", "block512_raw_global", "slices64"])
+def test_decode_data_paths(gpu, wl, tuning):
+    """Every way ut_decode can order an event gives the oracle's container and the same per-sector view: the CTA-wide
+    order (thread per hit), the warp-per-group order (events that do not fit, UT_ORDER_Y), small and large CTAs, raw
+    banks read from global memory.  Config 2 and config 4 events plus hand-built ties across sectors and chunks."""
+    from gpu_helpers import compare_decode
+    gpu.B.ut_tuning_set(**tuning) if tuning else gpu.B.ut_tuning_set(None)
+    try:
+        for c, n in ((2, 30), (4, 6)):
+            geom, b, p = wl(c, n)
+            h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+            hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+            got, off, st = gpu.hits_numpy(hits, b.n_events)
+            compare_decode(h_ref, got, off, st)
+            li = gpu.B.last_launch_info()
+            if "decode_hit_stage" in tuning:
+                assert li["decode_hit_stage"] == tuning["decode_hit_stage"]
+            if tuning.get("decode_hit_stage", -1) != 1024 and tuning.get("decode_sort_buf", -1) != 64:
+                check_sector_view(gpu, geom, b, hits, h_ref)     # (undersized buffers may leave an event without a view)
+        # equal x in different rows of one column (X layer: same strip and frac), 70 copies of 5 strips: ties inside a
+        # 32-hit chunk, across chunks and across sectors
+        geom = gpu.tables
+        k = np.arange(70)
+        sec = G.dense_sector(0, 5, 0) + k % 14
+        strip = 100 + k // 14
+        rng = np.random.default_rng(3)
+        perm = rng.permutation(k.size)
+        b = assemble_batch(geom, [_one_event(geom, sec[perm], strip[perm], np.ones(k.size, int), rng.permutation(896))])
+        h_ref = oracle.decode(b.raw, b.bank_offsets, b.n_events, geom, b.hit_capacity)
+        hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+        got, off, st = gpu.hits_numpy(hits, b.n_events)
+        compare_decode(h_ref, got, off, st)
+    finally:
+        gpu.B.ut_tuning_set(None)
+
+
 @pytest.mark.parametrize("split", [1, 2, 4])
 @pytest.mark.parametrize("view", [True, False])
 def test_compass_data_paths(gpu, wl, view, split):
@@ -271,7 +310,7 @@ def test_small_staging_takes_generic_paths(gpu, wl):
     """Force the events through the non-staged decode path and the global-memory Compass path (ut_tuning_set:
     the library reads its environment knobs once, so the launch shapes are set through the API)."""
     geom, b, p = wl(2, 12)
-    gpu.B.ut_tuning_set(decode_sort_buf=32, decode_raw_stage_bytes=4096, compass_hit_stage=512)
+    gpu.B.ut_tuning_set(decode_sort_buf=32, decode_raw_stage_bytes=4096, compass_hit_stage=512, decode_hit_stage=0)
     try:
         t = gpu.B.ut_tuning_get()
         assert (t.decode_sort_buf, t.decode_raw_stage_bytes, t.compass_hit_stage, t.compass_block) == (32, 4096, 512, -1)
