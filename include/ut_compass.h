@@ -282,6 +282,18 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_banks_host, size
                              const uint32_t* velo_offsets_host, uint32_t n_velo_total, int32_t n_events,
                              const compass_config* config, ut_tracks* tracks_host, uint32_t* status_host,
                              uint32_t* n_hits_host, ut_stream_t stream);
+/* Device-side timeline of the most recent ut_pipeline_run_host on `p`, read after the stream was synchronised
+ * (tracing aid; bench.py reports it): ms_out[k*5 + q] = milliseconds from the start of the call to the point where
+ * chunk k had q = 0: its raw banks and offsets on the device, 1: its VELO states, 2: been decoded, 3: been tracked,
+ * 4: its tracks on the host; *n_chunks_out = chunks the call used (<= 4; ms_out holds 20 floats); -1 = not recorded
+ * (zero-copy runs record no copy-in point). */
+int32_t ut_pipeline_timeline(ut_pipeline* p, float* ms_out, int32_t* n_chunks_out);
+/* Page-locked HOST memory for the buffers handed to ut_pipeline_run_host (cudaHostAlloc, portable and mapped; 256-byte
+ * aligned).  Any pinned memory works; this is the allocation the copy engines were measured at full PCIe rate with
+ * on the bench box (other pinned allocations of the same size copied at a quarter of it in some processes).
+ * ut_host_free releases it (never free() it).  Returns UT_ERR_CUDA when the allocation fails. */
+int32_t ut_host_alloc(void** out, size_t bytes);
+int32_t ut_host_free(void* p);
 /* Device views of the arena (valid after a run): decoded hits and offsets, for inspection. */
 int32_t ut_pipeline_device_hits(ut_pipeline* p, ut_hits* hits_out, const uint32_t** hit_offsets_out);
 

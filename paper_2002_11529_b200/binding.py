@@ -92,7 +92,7 @@ EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get"
            "ut_sector_offsets_stride", "compass_search_windows", "compass_tracklets_from_windows", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
            "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
-           "ut_pipeline_device_hits"]
+           "ut_pipeline_device_hits", "ut_host_alloc", "ut_host_free", "ut_pipeline_timeline"]
 
 _lib.ut_version.restype = C.c_char_p
 _lib.ut_last_error.restype = C.c_char_p
@@ -123,6 +123,9 @@ _lib.ut_pipeline_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_vo
                                       C.c_void_p, C.c_uint32, C.c_int32, C.POINTER(compass_config),
                                       C.POINTER(ut_tracks), C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ut_pipeline_device_hits.argtypes = [C.c_void_p, C.POINTER(ut_hits), C.POINTER(C.c_void_p)]
+_lib.ut_pipeline_timeline.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+_lib.ut_host_alloc.argtypes = [C.POINTER(C.c_void_p), C.c_size_t]
+_lib.ut_host_free.argtypes = [C.c_void_p]
 _lib.ut_last_launch_info.argtypes = [C.POINTER(ut_launch_info)]
 _lib.ut_sector_offsets_stride.restype = C.c_uint32
 _lib.ut_sector_offsets_stride.argtypes = [C.POINTER(ut_geometry)]
@@ -405,6 +408,48 @@ def last_launch_info() -> dict:
     return {n: getattr(li, n) for n, _ in ut_launch_info._fields_}
 
 
+class _HostBlock:
+    """One ut_host_alloc allocation; freed when the last tensor that views it is gone."""
+
+    def __init__(self, nbytes: int):
+        self.p = C.c_void_p()
+        _check(_lib.ut_host_alloc(C.byref(self.p), max(int(nbytes), 1)), "ut_host_alloc")
+        self.buf = (C.c_uint8 * max(int(nbytes), 1)).from_address(self.p.value)
+
+    def __del__(self):
+        try:
+            if self.p:
+                _lib.ut_host_free(self.p)
+                self.p = C.c_void_p()
+        except Exception:
+            pass
+
+
+def host_tensor(n: int, dtype: torch.dtype) -> torch.Tensor:
+    """A HOST tensor of n elements in ut_host_alloc memory (page-locked), for ut_pipeline_run_host."""
+    blk = _HostBlock(n * torch.empty(0, dtype=dtype).element_size())
+    arr = np.frombuffer(blk.buf, dtype=np.uint8)
+    t = torch.from_numpy(arr).view(dtype)[:n] if n > 0 else torch.empty(0, dtype=dtype)
+    _host_blocks[t.data_ptr()] = blk            # the block lives as long as the process keeps the key; see host_free
+    return t
+
+
+def host_free(t: torch.Tensor) -> None:
+    _host_blocks.pop(t.data_ptr(), None)
+
+
+_host_blocks: dict = {}
+
+
+def to_host_pinned(a) -> torch.Tensor:
+    """Copy of a numpy array in ut_host_alloc memory."""
+    a = np.ascontiguousarray(a)
+    t = host_tensor(a.size, torch.from_numpy(a[:0].copy()).dtype if a.size == 0 else torch.from_numpy(a.ravel()[:1].copy()).dtype)
+    if a.size:
+        t.numpy()[:] = a.ravel()
+    return t
+
+
 class Pipeline:
     """ut_pipeline_*: host buffers in, host track SoA out (copies inside the call)."""
 
@@ -426,6 +471,14 @@ class Pipeline:
                                          velo_offsets_h.data_ptr(), n_velo, n_events, C.byref(config), C.byref(tr),
                                          out_h["status"].data_ptr(), out_h["n_hits_total"].data_ptr(),
                                          _stream_ptr(stream)), "ut_pipeline_run_host")
+
+    def timeline(self) -> list:
+        """Per chunk of the last run_host (after a sync): ms from the call's start to copy-in, VELO-in, decoded, tracked, out."""
+        ms = (C.c_float * 20)()
+        n = C.c_int32(0)
+        _check(_lib.ut_pipeline_timeline(self.h, ms, C.byref(n)), "ut_pipeline_timeline")
+        keys = ("banks_in", "velo_in", "decoded", "tracked", "tracks_out")
+        return [{k: round(float(ms[c * 5 + q]), 4) for q, k in enumerate(keys)} for c in range(n.value)]
 
     def destroy(self):
         if self.h:

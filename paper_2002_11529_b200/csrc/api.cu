@@ -16,7 +16,7 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
                       unsigned long long hits_hint);
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint);
+                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint, uint32_t* ticket = nullptr);
 
 size_t consolidate_workspace_bytes(uint32_t max_velo);
 int32_t launch_consolidate(const ut_tracks* tracks, const uint32_t* velo_offsets, int32_t n_events, uint32_t n_velo_hint,
@@ -431,8 +431,10 @@ struct ut_pipeline {
   ut_hits hits;
   ut_tracks tracks;
   // chunked overlap of copies and kernels: copy-in stream, copy-out stream, per-chunk events
-  cudaStream_t s_in, s_out, s_cmp;
-  cudaEvent_t ev_start, ev_out, ev_in[4], ev_velo[4], ev_done[4], ev_dec[4];
+  cudaStream_t s_in, s_in2, s_out, s_cmp, s_cmp2;
+  cudaEvent_t ev_start, ev_out, ev_in[4], ev_velo[4], ev_done[4], ev_dec[4], ev_d2h[4];
+  int last_chunks;               // chunks of the most recent run (ut_pipeline_timeline)
+  bool last_zero_copy;
 };
 
 int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_raw_bytes, uint64_t max_hits,
@@ -470,15 +472,15 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   p->tracks.status = p->status + 4;                    // 4 words: status + the kernel's work ticket
   if (cudaMemset(p->block, 0, total) != cudaSuccess) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
   bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&p->s_in2, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&p->s_cmp, cudaStreamNonBlocking) == cudaSuccess &&
-            cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) == cudaSuccess &&
-            cudaEventCreateWithFlags(&p->ev_out, cudaEventDisableTiming) == cudaSuccess;
-  for (int k = 0; k < 4 && ok; ++k)
-    ok = cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming) == cudaSuccess &&
-         cudaEventCreateWithFlags(&p->ev_velo[k], cudaEventDisableTiming) == cudaSuccess &&
-         cudaEventCreateWithFlags(&p->ev_done[k], cudaEventDisableTiming) == cudaSuccess &&
-         cudaEventCreateWithFlags(&p->ev_dec[k], cudaEventDisableTiming) == cudaSuccess;
+            cudaStreamCreateWithFlags(&p->s_cmp2, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreate(&p->ev_start) == cudaSuccess && cudaEventCreate(&p->ev_out) == cudaSuccess;
+  for (int k = 0; k < 4 && ok; ++k)         // (timing events: ut_pipeline_timeline reads them)
+    ok = cudaEventCreate(&p->ev_in[k]) == cudaSuccess && cudaEventCreate(&p->ev_velo[k]) == cudaSuccess &&
+         cudaEventCreate(&p->ev_done[k]) == cudaSuccess && cudaEventCreate(&p->ev_dec[k]) == cudaSuccess &&
+         cudaEventCreate(&p->ev_d2h[k]) == cudaSuccess;
   if (!ok) { cudaFree(p->block); delete p; return UT_ERR_CUDA; }
   *out = p;
   return UT_OK;
@@ -487,13 +489,16 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
 int32_t ut_pipeline_destroy(ut_pipeline* p) {
   if (!p) return UT_ERR_NULL;
   cudaStreamSynchronize(p->s_in);
+  cudaStreamSynchronize(p->s_in2);
   cudaStreamSynchronize(p->s_out);
   cudaStreamSynchronize(p->s_cmp);
+  cudaStreamSynchronize(p->s_cmp2);
   for (int k = 0; k < 4; ++k) {
     cudaEventDestroy(p->ev_in[k]); cudaEventDestroy(p->ev_velo[k]); cudaEventDestroy(p->ev_done[k]); cudaEventDestroy(p->ev_dec[k]);
+    cudaEventDestroy(p->ev_d2h[k]);
   }
   cudaEventDestroy(p->ev_start); cudaEventDestroy(p->ev_out);
-  cudaStreamDestroy(p->s_in); cudaStreamDestroy(p->s_out); cudaStreamDestroy(p->s_cmp);
+  cudaStreamDestroy(p->s_in); cudaStreamDestroy(p->s_in2); cudaStreamDestroy(p->s_out); cudaStreamDestroy(p->s_cmp); cudaStreamDestroy(p->s_cmp2);
   cudaFree(p->block);
   delete p;
   return UT_OK;
@@ -512,14 +517,16 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   // The batch is cut into up to 4 chunks of events: chunk k+1 is copied in while chunk k is decoded and
   // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
   // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
-  const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 500);
-  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 500);
+  const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 334);
+  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 334);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
-  bool ok = cudaMemsetAsync(p->status, 0, 32, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
+  bool ok = cudaMemsetAsync(p->status, 0, 64, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&
+            cudaStreamWaitEvent(p->s_in2, p->ev_start, 0) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_out, p->ev_start, 0) == cudaSuccess &&
-            cudaStreamWaitEvent(p->s_cmp, p->ev_start, 0) == cudaSuccess;
-  if (!ok) return UT_ERR_CUDA;
+            cudaStreamWaitEvent(p->s_cmp, p->ev_start, 0) == cudaSuccess &&
+            cudaStreamWaitEvent(p->s_cmp2, p->ev_start, 0) == cudaSuccess;
+  if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
   // Zero copy (ut_tuning.pipeline_zero_copy = 1, off by default): when the raw banks and their offsets sit in mapped
   // pinned host memory the decode kernel reads them over PCIe itself (bulk copies and coalesced loads straight from
   // the host buffer, no staging copy) and Compass runs on a second stream, so that chunk k is tracked while chunk
@@ -538,7 +545,7 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
       cudaGetLastError();                          // not mapped pinned memory: staged copies
     }
   }
-  cudaStream_t sc = raw_z ? p->s_cmp : s;         // stream of the Compass launches
+  p->last_zero_copy = raw_z != nullptr;
   if (n_events == 0) {
     ok = cudaMemsetAsync(p->hit_offsets, 0, 4, s) == cudaSuccess;
     if (status_h) ok = ok && cudaMemcpyAsync(status_h, p->status, 4, cudaMemcpyDeviceToHost, s) == cudaSuccess &&
@@ -554,23 +561,60 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   auto d2h = [&](void* h, const void* d, size_t n) {
     return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
   };
+  // `rows` arrays of `n` bytes each, `hpitch` / `dpitch` bytes apart: one strided copy when the host arrays are evenly
+  // spaced (every copy costs ~10 us of engine latency on top of its bytes), else one copy per array
+  auto rows_copy = [&](void* const* hp, ptrdiff_t hpitch, unsigned char* d, size_t dpitch, size_t n, int rows, bool to_host,
+                       cudaStream_t st) {
+    if (n == 0) return true;
+    if (hpitch >= (ptrdiff_t)n) {
+      if ((to_host ? cudaMemcpy2DAsync(hp[0], (size_t)hpitch, d, dpitch, n, (size_t)rows, cudaMemcpyDeviceToHost, st)
+                   : cudaMemcpy2DAsync(d, dpitch, hp[0], (size_t)hpitch, n, (size_t)rows, cudaMemcpyHostToDevice, st)) == cudaSuccess)
+        return true;
+      cudaGetLastError();          // evenly spaced, but not rows of ONE page-locked allocation: the call refuses; copy per array
+    }
+    bool good = true;
+    for (int r = 0; r < rows && good; ++r)
+      good = (to_host ? cudaMemcpyAsync(hp[r], d + (size_t)r * dpitch, n, cudaMemcpyDeviceToHost, st)
+                      : cudaMemcpyAsync(d + (size_t)r * dpitch, hp[r], n, cudaMemcpyHostToDevice, st)) == cudaSuccess;
+    return good;
+  };
+  // spacing of evenly spaced host arrays (0: not evenly spaced)
+  auto pitch_of = [](const void* a0, const void* a1, const void* a2, const void* a3) -> ptrdiff_t {
+    const ptrdiff_t d = (const unsigned char*)a1 - (const unsigned char*)a0;
+    if (d <= 0 || (const unsigned char*)a2 - (const unsigned char*)a1 != d) return 0;
+    if (a3 && (const unsigned char*)a3 - (const unsigned char*)a2 != d) return 0;
+    return d;
+  };
   velo_states vd = {p->vx, p->vy, p->vtx, p->vty, velo_h->z};
+  const size_t dv_pitch = (size_t)((unsigned char*)p->vy - (unsigned char*)p->vx);
+  // The VELO states and their offsets (15 % of the input bytes) go in at once on a second copy-in stream, beside the first
+  // chunk's banks: Compass needs them only after the first decode.
+  {
+    void* const hv[4] = {const_cast<float*>(velo_h->x), const_cast<float*>(velo_h->y), const_cast<float*>(velo_h->tx),
+                         const_cast<float*>(velo_h->ty)};
+    ok = cudaMemcpyAsync(p->velo_offsets, vo_h, ((size_t)n_events + 1) * 4, cudaMemcpyHostToDevice, p->s_in2) == cudaSuccess &&
+         rows_copy(hv, pitch_of(hv[0], hv[1], hv[2], hv[3]), (unsigned char*)p->vx, dv_pitch, (size_t)n_velo * 4, 4, false, p->s_in2) &&
+         cudaEventRecord(p->ev_velo[0], p->s_in2) == cudaSuccess && cudaStreamWaitEvent(p->s_cmp, p->ev_velo[0], 0) == cudaSuccess &&
+         cudaStreamWaitEvent(p->s_cmp2, p->ev_velo[0], 0) == cudaSuccess;
+    if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
+  }
+  const ptrdiff_t ht_pitch = pitch_of(tracks_h->n_hits, tracks_h->qop, tracks_h->chi2, nullptr);
+  const size_t dt_pitch = (size_t)((unsigned char*)p->tracks.qop - (unsigned char*)p->tracks.n_hits);
   int launched = 0;
+  // Chunk sizes fall linearly (K = 4: 40 / 30 / 20 / 10 % of the events).  The copy-in is the longest stage (PCIe), every
+  // chunk's kernels hide behind the next chunk's copy, and what remains exposed at the end is the last chunk's decode +
+  // Compass + copy-out: the smaller that chunk, the shorter the call.
+  auto chunk_begin = [&](int k) { return (int)((long long)n_events * k * (2 * K - k + 1) / ((long long)K * (K + 1))); };
   for (int k = 0; k < K; ++k) {
-    const int e0 = (int)((long long)n_events * k / K), e1 = (int)((long long)n_events * (k + 1) / K), ne = e1 - e0;
+    const int e0 = chunk_begin(k), e1 = k == K - 1 ? n_events : chunk_begin(k + 1), ne = e1 - e0;
     const size_t r0 = k == 0 ? 0 : bo_h[(size_t)e0 * ns], r1 = k == K - 1 ? raw_bytes : bo_h[(size_t)e1 * ns];
     const uint32_t v0 = vo_h[e0], v1 = vo_h[e1];
     if (r1 < r0 || r1 > raw_bytes || v1 < v0 || v1 > n_velo) return UT_ERR_ARG;
-    // the decode only needs the banks and their offsets: the VELO states follow while it runs
-    ok = (raw_z != nullptr ||
-          (h2d(p->raw + r0, raw_h + r0, r1 - r0) &&
-           h2d(p->bank_offsets + (size_t)e0 * ns, bo_h + (size_t)e0 * ns, ((size_t)ne * ns + 1) * 4) &&
-           cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess)) &&
-         h2d(p->velo_offsets + e0, vo_h + e0, ((size_t)ne + 1) * 4) &&
-         h2d(p->vx + v0, velo_h->x + v0, (size_t)(v1 - v0) * 4) && h2d(p->vy + v0, velo_h->y + v0, (size_t)(v1 - v0) * 4) &&
-         h2d(p->vtx + v0, velo_h->tx + v0, (size_t)(v1 - v0) * 4) && h2d(p->vty + v0, velo_h->ty + v0, (size_t)(v1 - v0) * 4) &&
-         cudaEventRecord(p->ev_velo[k], p->s_in) == cudaSuccess;
-    if (!ok) return UT_ERR_CUDA;
+    ok = raw_z != nullptr ||
+         (h2d(p->raw + r0, raw_h + r0, r1 - r0) &&
+          h2d(p->bank_offsets + (size_t)e0 * ns, bo_h + (size_t)e0 * ns, ((size_t)ne * ns + 1) * 4) &&
+          cudaEventRecord(p->ev_in[k], p->s_in) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_in[k], 0) == cudaSuccess);
+    if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
     uint32_t* ho = p->hit_offsets + (size_t)e0 * ng;
     // upper bound of this chunk's hits from its raw size alone (sizes the on-chip staging like a whole call)
     const size_t hdr = 6 * (size_t)ne * ns;
@@ -581,25 +625,61 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
                                k == 0 ? nullptr : ho, hint);
     if (rc) return rc;
     launched += launch_info().kernels_launched;
-    if (raw_z && (cudaEventRecord(p->ev_dec[k], s) != cudaSuccess || cudaStreamWaitEvent(sc, p->ev_dec[k], 0) != cudaSuccess))
-      return UT_ERR_CUDA;
-    if (cudaStreamWaitEvent(sc, p->ev_velo[k], 0) != cudaSuccess) return UT_ERR_CUDA;
-    rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, sc, n_velo, hint);
+    // Compass runs beside the decode stream, chunks alternating between two streams (each launch with its own work
+    // ticket): chunk k is tracked while chunk k + 1 is decoded and chunk k + 2 streams in, and the short last chunks,
+    // which cost one event's latency whatever their size, overlap each other.  Both kernels leave issue slots idle alone.
+    cudaStream_t sc = (k & 1) ? p->s_cmp2 : p->s_cmp;
+    if (cudaEventRecord(p->ev_dec[k], s) != cudaSuccess || cudaStreamWaitEvent(sc, p->ev_dec[k], 0) != cudaSuccess)
+      return cuda_fail("ut_pipeline_run_host (events)", cudaGetLastError());
+    rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, sc, n_velo, hint, p->status + 8 + 2 * (k & 1));
     if (rc) return rc;
     launched += launch_info().kernels_launched;
     ok = cudaEventRecord(p->ev_done[k], sc) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess;
-    for (int l = 0; l < 4 && ok; ++l)
-      ok = d2h(tracks_h->hit_idx + (size_t)l * n_velo + v0, p->tracks.hit_idx + (size_t)l * n_velo + v0, (size_t)(v1 - v0) * 4);
-    ok = ok && d2h(tracks_h->n_hits + v0, p->tracks.n_hits + v0, (size_t)(v1 - v0) * 4) &&
-         d2h(tracks_h->qop + v0, p->tracks.qop + v0, (size_t)(v1 - v0) * 4) &&
-         d2h(tracks_h->chi2 + v0, p->tracks.chi2 + v0, (size_t)(v1 - v0) * 4);
-    if (!ok) return UT_ERR_CUDA;
+    {
+      void* const hi[4] = {tracks_h->hit_idx + v0, tracks_h->hit_idx + (size_t)n_velo + v0, tracks_h->hit_idx + 2 * (size_t)n_velo + v0,
+                           tracks_h->hit_idx + 3 * (size_t)n_velo + v0};
+      void* const hr[3] = {tracks_h->n_hits + v0, tracks_h->qop + v0, tracks_h->chi2 + v0};
+      ok = ok && rows_copy(hi, (ptrdiff_t)n_velo * 4, (unsigned char*)(p->tracks.hit_idx + v0), (size_t)n_velo * 4, (size_t)(v1 - v0) * 4, 4,
+                           true, p->s_out) &&
+           rows_copy(hr, ht_pitch, (unsigned char*)(p->tracks.n_hits + v0), dt_pitch, (size_t)(v1 - v0) * 4, 3, true, p->s_out) &&
+           cudaEventRecord(p->ev_d2h[k], p->s_out) == cudaSuccess;
+    }
+    if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
   }
+  p->last_chunks = K;
   launch_info().kernels_launched = launched;
   if (status_h) ok = ok && d2h(status_h, p->status, 4) && d2h(status_h + 1, p->status + 4, 4);
   if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * ng, 4);
   ok = ok && cudaEventRecord(p->ev_out, p->s_out) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_out, 0) == cudaSuccess;
-  return ok ? UT_OK : UT_ERR_CUDA;
+  return ok ? UT_OK : cuda_fail("ut_pipeline_run_host (copy out)", cudaGetLastError());
+}
+
+int32_t ut_pipeline_timeline(ut_pipeline* p, float* ms_out, int32_t* n_chunks_out) {
+  if (!p || !ms_out || !n_chunks_out) return UT_ERR_NULL;
+  *n_chunks_out = p->last_chunks;
+  for (int k = 0; k < p->last_chunks; ++k) {
+    cudaEvent_t ev[5] = {p->ev_in[k], p->ev_velo[0], p->ev_dec[k], p->ev_done[k], p->ev_d2h[k]};   // (VELO states: one copy per call)
+    for (int q = 0; q < 5; ++q) {
+      float ms = -1.f;
+      if (q == 0 && p->last_zero_copy) { ms_out[k * 5] = -1.f; continue; }
+      if (cudaEventElapsedTime(&ms, p->ev_start, ev[q]) != cudaSuccess) { cudaGetLastError(); ms = -1.f; }
+      ms_out[k * 5 + q] = ms;
+    }
+  }
+  return UT_OK;
+}
+
+int32_t ut_host_alloc(void** out, size_t bytes) {
+  if (!out) return UT_ERR_NULL;
+  *out = nullptr;
+  const cudaError_t err = cudaHostAlloc(out, bytes ? bytes : 1, cudaHostAllocPortable | cudaHostAllocMapped);
+  return err == cudaSuccess ? UT_OK : cuda_fail("cudaHostAlloc", err);
+}
+
+int32_t ut_host_free(void* p) {
+  if (!p) return UT_OK;
+  const cudaError_t err = cudaFreeHost(p);
+  return err == cudaSuccess ? UT_OK : cuda_fail("cudaFreeHost", err);
 }
 
 int32_t ut_pipeline_device_hits(ut_pipeline* p, ut_hits* hits_out, const uint32_t** hit_offsets_out) {

@@ -81,7 +81,8 @@ struct CompassArgs {
   compass_config c;
   int32_t *out_idx, *out_n;
   float *out_qop, *out_chi2;
-  uint32_t* status;                    // [0] status word, [1] next work item, [2] CTAs done
+  uint32_t* status;                    // [0] status word
+  uint32_t* ticket;                    // [0] next work item, [1] CTAs done (one pair per launch that may run at a time)
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
   uint32_t trk_stage;                  // tracks of an item that can be ordered by radius (0: never)
   unsigned long long capacity;         // elements of the hit arrays (bulk copies never read past it)
@@ -758,7 +759,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   __shared__ uint32_t s_item[2];                   // double-buffered: a slow thread still reads the previous ticket
   for (int k = 0;; ++k) {
     // work items are dealt out dynamically: CTAs that finish early take more
-    if (tid == 0) s_item[k & 1] = atomicAdd(a.status + 1, 1u);
+    if (tid == 0) s_item[k & 1] = atomicAdd(a.ticket, 1u);
     __syncthreads();                               // tables staged / previous item fully consumed
     const uint32_t item = s_item[k & 1];
     if (item >= n_items) break;
@@ -972,7 +973,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   }
   if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
     __threadfence();
-    if (atomicAdd(a.status + 2, 1u) == gridDim.x - 1) { a.status[1] = 0; a.status[2] = 0; __threadfence(); }
+    if (atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1) { a.ticket[0] = 0; a.ticket[1] = 0; __threadfence(); }
   }
 }
 
@@ -999,7 +1000,7 @@ static const void* const kKernels[2][2][2] = {     // [large CTAs][interval sear
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
-                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint) {
+                       cudaStream_t stream, uint32_t idx_stride, unsigned long long hits_hint, uint32_t* ticket) {
   DeviceInfo dev;
   int max_smem = 0, max_smem_large = 0;               // largest dynamic size a CTA may ask for on this device
   if (const int32_t rc = device_info(&dev)) return rc;
@@ -1041,6 +1042,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.capacity = hits->capacity;
   a.bulk_ok = ((reinterpret_cast<uintptr_t>(hits->x_at_y0) | reinterpret_cast<uintptr_t>(hits->id)) & 15u) == 0 ? 1u : 0u;
   a.out_idx = out->hit_idx; a.out_n = out->n_hits; a.out_qop = out->qop; a.out_chi2 = out->chi2; a.status = out->status;
+  a.ticket = ticket ? ticket : out->status + 1;      // (ut_tracks.status is 4 words: status, ticket pair, spare)
 
   const int C = cfg->max_candidates_per_layer;
   const uint32_t ns = geom->n_sectors, ng = geom->n_groups;
