@@ -991,11 +991,12 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32
 // Two register budgets: CTAs of <= 224 threads at 4 per SM (72 registers), and larger CTAs (big events / C = 32,
 // where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
 constexpr int kSmallBlock = 224;
+constexpr int kLargeBlock = 640;             // (a 768-thread bound caps the kernel at 80 registers and it spills; 640: 84-88, none)
 #define UTC_K(T, B, I, K) reinterpret_cast<const void*>(&compass_kernel<T, B, I, K>)
 static const void* const kKernels[2][2][2] = {     // [large CTAs][interval search][kick table]
     {{UTC_K(kSmallBlock, 4, false, false), UTC_K(kSmallBlock, 4, false, true)},
      {UTC_K(kSmallBlock, 4, true, false), UTC_K(kSmallBlock, 4, true, true)}},
-    {{UTC_K(768, 1, false, false), UTC_K(768, 1, false, true)}, {UTC_K(768, 1, true, false), UTC_K(768, 1, true, true)}}};
+    {{UTC_K(kLargeBlock, 1, false, false), UTC_K(kLargeBlock, 1, false, true)}, {UTC_K(kLargeBlock, 1, true, false), UTC_K(kLargeBlock, 1, true, true)}}};
 #undef UTC_K
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
@@ -1058,7 +1059,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   int block = tuned(tune.compass_block, 0);
   if (block <= 0) {
     int best_warps = -1;
-    for (int b = 192; b <= 768; b += 32) {
+    for (int b = 192; b <= kLargeBlock; b += 32) {
       const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
@@ -1068,7 +1069,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     }
     if (block <= 0) block = 192;
   }
-  block = std::max(32, std::min(768, (block / 32) * 32));
+  block = std::max(32, std::min(kLargeBlock, (block / 32) * 32));
   size_t smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
   while (smem > budget && block > 64) {             // fewer warps before giving up staging
     block -= 32;
