@@ -517,8 +517,8 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   // The batch is cut into up to 4 chunks of events: chunk k+1 is copied in while chunk k is decoded and
   // tracked, and the tracks of chunk k go out while chunk k+1 is computed.  Results are those of one call:
   // the decode of chunk k starts its hit prefix from the total chunk k-1 left in hit_offsets.
-  const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 334);
-  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 334);
+  const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 333);
+  int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 333);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
   bool ok = cudaMemsetAsync(p->status, 0, 64, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&

@@ -383,6 +383,54 @@ def test_host_pipeline_matches_oracle(gpu, wl, n_events, zero_copy):
     gpu.B.ut_tuning_set(None)
 
 
+@pytest.mark.parametrize("chunk", [333, 120])
+def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk):
+    """ut_pipeline_run_host with buffers from ut_host_alloc: the four VELO arrays are rows of one allocation and so are
+    n_hits / qop / chi2, which the call moves as one strided copy each (separate torch-pinned tensors, the test above,
+    take one copy per array); 3 and 4 chunks of linearly falling size.  The result equals the oracle's, and
+    ut_pipeline_timeline reports for every chunk: banks in <= decoded <= tracked <= tracks out."""
+    import torch
+    B = gpu.B
+    B.ut_tuning_set(pipeline_chunk_events=chunk)
+    geom, b, p = wl(3, 1000)
+    h_ref, t_ref = oracle_run(b, geom, p)
+    T = b.n_velo_total
+    Tp = (T + 63) // 64 * 64
+    raw_h = B.to_host_pinned(np.concatenate([b.raw, np.zeros(32, np.uint8)]))
+    bo_h, vo_h = B.to_host_pinned(b.bank_offsets.view(np.int32)), B.to_host_pinned(b.velo_offsets.view(np.int32))
+    velo_blk = B.host_tensor(4 * Tp, torch.float32)
+    velo_h = [velo_blk[r * Tp:r * Tp + T] for r in range(4)]
+    for dst, src in zip(velo_h, (b.velo_x, b.velo_y, b.velo_tx, b.velo_ty)):
+        dst.numpy()[:] = src
+    res = B.host_tensor(3 * Tp, torch.int32)
+    res.fill_(-7)
+    out_h = {"hit_idx": B.host_tensor(4 * T, torch.int32), "n_hits": res[0:T], "qop": res[Tp:Tp + T].view(torch.float32),
+             "chi2": res[2 * Tp:2 * Tp + T].view(torch.float32), "status": B.host_tensor(2, torch.int32),
+             "n_hits_total": B.host_tensor(1, torch.int32)}
+    pipe = B.Pipeline(gpu.geom, b.n_events, int(b.raw.size) + 32, b.hit_capacity, T)
+    try:
+        for _ in range(2):
+            pipe.run_host(raw_h, int(b.raw.size), bo_h, velo_h, b.velo_z, vo_h, T, b.n_events, B.make_config(p), out_h)
+            torch.cuda.synchronize()
+            assert int(out_h["n_hits_total"][0]) == h_ref.n_hits and out_h["status"].tolist() == [0, 0]
+            assert np.array_equal(out_h["hit_idx"].numpy().reshape(4, T), t_ref.hit_idx)
+            assert np.array_equal(out_h["n_hits"].numpy(), t_ref.n_hits)
+            assert np.array_equal(out_h["chi2"].numpy().view(np.uint32), t_ref.chi2.view(np.uint32))
+            assert np.array_equal(out_h["qop"].numpy().view(np.uint32), t_ref.qop.view(np.uint32))
+            assert np.all(res.numpy()[T:Tp] == -7) and np.all(res.numpy()[Tp + T:2 * Tp] == -7)   # the pads between the rows
+            tl = pipe.timeline()
+            assert len(tl) == min(4, 1000 // chunk)
+            for c in tl:
+                assert 0 < c["banks_in"] <= c["decoded"] <= c["tracked"] <= c["tracks_out"] and 0 < c["velo_in"] <= c["tracked"]
+            assert all(tl[k]["tracks_out"] <= tl[k + 1]["tracks_out"] for k in range(len(tl) - 1))
+            out_h["n_hits"].fill_(-7)
+    finally:
+        pipe.destroy()
+        B.ut_tuning_set(None)
+        for t_ in (raw_h, bo_h, vo_h, velo_blk, res, out_h["hit_idx"], out_h["status"], out_h["n_hits_total"]):
+            B.host_free(t_)
+
+
 def _consolidate_both(gpu, t_idx, t_n, t_qop, t_chi2, vo, n_events, capacity=None):
     """compass_consolidate on device copies of a dense track SoA vs oracle.consolidate."""
     import torch
