@@ -21,11 +21,12 @@
 //               slot [group start + count] of the sorted order.  Hits with equal x collide there: the
 //               first in fill order keeps the slot, each later one is moved once to slot + (equal hits
 //               in front of it) -- so the result is the stable sort by x         (paper: "find permutation")
-//   -> output, all warps: thread per slot of the sorted order, the 7 SoA arrays by fully coalesced
-//      stores (a warp writes 32 consecutive elements of each array)    (paper: "decode raw banks in order")
+//   -> output, all warps: a warp takes one sector group at a time and walks its slots of the sorted order,
+//      the 7 SoA arrays by fully coalesced stores (32 consecutive elements of each array per step)
+//                                                                     (paper: "decode raw banks in order")
 //      and the hit's entry in the per-sector view for compass_track (ut_hits.x_by_sector ...): the fill
-//      order is sector-major, so a sector's entries are a contiguous run and the position inside the run
-//      is the rank among the bank's own words (a short loop over them)
+//      order is sector-major, so a sector's entries are a contiguous run; a hit goes behind the hits of its
+//      sector that came earlier in the sorted order (running count per sector + match.any among the lanes)
 //
 // Events whose padded fill order does not fit the buffers, and UT_ORDER_Y containers, are ordered warp per
 // sector group instead (ticket inside the CTA): gather into the warp's slice of the same buffers, rank per
@@ -95,7 +96,6 @@ __device__ __forceinline__ float eq(float a, float b) {
   asm("set.eq.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
   return d;
 }
-constexpr uint32_t kTieBit = 0x8000u;   // in the (sector << 16 | word) entry: an earlier hit of the group has the same x
 
 // stable order of the fill sequence: (x, position in the fill order)
 __device__ __forceinline__ uint32_t before(float xj, uint32_t j, float x, uint32_t i) {
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
           for (uint32_t k = 0; k < c; ++k) {
             const uint32_t word = wd[k];
             s_xbuf[p0 + k] = decode_x(word, xp.x, xp.y);
-            s_wbuf[p0 + k] = (sct << 16) | (word & 0x3FFu);   // (ADC bits dropped: bit 15 is kTieBit)
+            s_wbuf[p0 + k] = (sct << 16) | word;
           }
         }
         for (uint32_t g = wt; g < ng; g += nw) {          // pad slots: +inf is never "smaller", kInvalid marks them
@@ -304,6 +304,7 @@ __global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
         }
         asm volatile("bar.sync 1, %0;" ::"r"(nw) : "memory");      // every word is decoded: the raw bytes are dead
         for (uint32_t q = wt; q < ptot; q += nw) s_perm[q] = kInvalid;
+        for (uint32_t q = wt; q < ns; q += nw) s_wpos[q] = 0;       // (word positions are dead too: per-sector counters of the output)
         asm volatile("bar.sync 1, %0;" ::"r"(nw) : "memory");
         // ---- rank: thread per hit, one sweep over its group counts the hits with smaller x ("find permutation",
         //      PAPER.md:273).  Hits with equal x get the same count: the first of them in fill order keeps the slot
@@ -333,39 +334,47 @@ __global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
             }
             for (; j < later; ++j) o0 += eq(s_xbuf[j], x);
             s_perm[pga + rank + (uint32_t)(o0 + o1)] = later;
-            atomicOr(&s_wbuf[later], kTieBit);              // its place in its bank's run needs the exact order
           }
         }
       }
       __syncthreads();                                       // order complete, base known
       base = s_base;
       if ((unsigned long long)base + tot > a.capacity) continue;        // flagged by warp 0; offsets stay exact
-      // ---- output: thread per slot of the sorted order, coalesced SoA stores ("decode raw banks in order",
-      //      PAPER.md:274); the per-sector view entry of the same hit goes to its rank among its own bank's words
-      for (uint32_t q = tid; q < ptot; q += nt) {
-        const uint32_t pi = s_perm[q];
-        if (pi == kInvalid) continue;
-        const uint32_t rw = s_wbuf[pi], sct = rw >> 16;
-        const float x = s_xbuf[pi];
-        const uint32_t g = g_sgrp[sct];
-        const uint32_t pga = s_pstart[g], gfs = s_start[g_gfirst[g]];
-        const uint32_t hpos = gfs + (q - pga);               // place in the event's part of the container
-        const float4 A = __ldg(a.g.sector_rows + 2 * sct), B = __ldg(a.g.sector_rows + 2 * sct + 1);
-        const size_t P = (size_t)base + hpos;
-        a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
-        a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
-        if (view) {
-          const uint32_t es = s_start[sct], cs = s_start[sct + 1] - es, pes = pga + (es - gfs);
-          uint32_t pos = 0;
-          if (rw & kTieBit) { for (uint32_t j = pes; j < pes + cs; ++j) pos += before(s_xbuf[j], j, x, pi); }
-          else {
-            float f = 0.f;
-            for (uint32_t j = pes; j < pes + cs; ++j) f += lt(s_xbuf[j], x);
-            pos = (uint32_t)f;
+      // ---- output: a warp takes one sector group at a time (ticket) and walks its slots of the sorted order, 32 per
+      //      step: coalesced SoA stores ("decode raw banks in order").  The per-sector view entry of a hit
+      //      goes behind the hits of its sector that came earlier in the sorted order: a running count per sector
+      //      (s_wpos, zeroed above) plus the rank among the lanes of the same sector (match.any).
+      for (;;) {
+        uint32_t g = 0;
+        if (lane == 0) g = atomicAdd(&s_gticket, 1u);
+        g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        if (g >= ng) break;
+        const uint32_t pga = s_pstart[g], gfs = s_start[g_gfirst[g]], n = s_start[g_gfirst[g + 1]] - gfs;
+        for (uint32_t c0 = 0; c0 < n; c0 += 32u) {
+          const bool valid = c0 + lane < n;
+          const uint32_t pi = valid ? s_perm[pga + c0 + lane] : 0u;
+          const uint32_t rw = valid ? s_wbuf[pi] : 0xFFFFFFFFu, sct = rw >> 16;
+          const uint32_t peers = __match_any_sync(0xFFFFFFFFu, sct);
+          const uint32_t ahead = __popc(peers & lt_mask);
+          if (valid) {
+            const float x = s_xbuf[pi];
+            const uint32_t hpos = gfs + c0 + lane;             // place in the event's part of the container
+            const float4 A = __ldg(a.g.sector_rows + 2 * sct), B = __ldg(a.g.sector_rows + 2 * sct + 1);
+            const size_t P = (size_t)base + hpos;
+            a.x[P] = x; a.z[P] = A.x; a.yb[P] = A.y; a.ye[P] = A.z; a.dxdy[P] = A.w; a.w[P] = B.x;
+            a.id[P] = (__float_as_uint(B.y) << 9) | (rw & 0x1FFu);
+            if (view) {
+              const uint32_t seen = s_wpos[sct];
+              const size_t Q = (size_t)base + s_start[sct] + seen + ahead;
+              a.sx[Q] = x;
+              a.si[Q] = (uint16_t)hpos;
+              if (n > 32u) {                                   // (a one-step group never reads the count again)
+                __syncwarp(peers);
+                if (ahead == 0) s_wpos[sct] = seen + __popc(peers);
+              }
+            }
           }
-          const size_t Q = (size_t)base + es + pos;
-          a.sx[Q] = x;
-          a.si[Q] = (uint16_t)hpos;
+          __syncwarp();
         }
       }
       continue;
