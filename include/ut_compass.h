@@ -210,7 +210,11 @@ typedef struct {
 /* compass_track -- PAPER.md section V, fused (window search + tracklet finding in one kernel; the
  * paper's CPU port does the same).
  * hits, hit_offsets : as produced by ut_decode (hits->geom gives the group tables).
- * velo_offsets      : device u32 [n_events + 1]; n_velo_total = velo_offsets[n_events] (read on device). */
+ * velo_offsets      : device u32 [n_events + 1]; n_velo_total = velo_offsets[n_events] (read on device).
+ * The kernel is launched with programmatic stream serialization: when the preceding operation of `stream` is the
+ * ut_decode kernel its CTAs may become resident on SMs that kernel has left and stage their geometry tables, and they
+ * wait for its completion (griddepcontrol.wait) before they read hits, offsets or the per-sector view.  Stream order
+ * is otherwise unchanged; behind any other operation the launch is an ordinary one. */
 int32_t compass_track(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                       const uint32_t* velo_offsets, int32_t n_events, const compass_config* config,
                       ut_tracks* tracks_out, ut_stream_t stream);

@@ -756,6 +756,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t K = a.split;
   const uint32_t n_items = (uint32_t)a.n_events * K;
 
+  // Launched with programmatic stream serialization the CTAs may be resident, with their tables staged, while the
+  // preceding kernel of the stream (ut_decode) still runs on other SMs: everything it wrote is read after this point.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   __shared__ uint32_t s_item[2];                   // double-buffered: a slow thread still reads the previous ticket
   for (int k = 0;; ++k) {
     // work items are dealt out dynamically: CTAs that finish early take more
@@ -1108,7 +1111,15 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.split = (uint32_t)split;
   const int grid = std::max(1, (int)std::min<long long>((long long)n_events * split, resident));
   void* params[] = {&a};
-  UTC_CUDA(cudaLaunchKernel(kernel, dim3(grid), dim3(block), params, smem, stream));
+  {
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3(grid); lc.blockDim = dim3(block); lc.dynamicSmemBytes = smem; lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    UTC_CUDA(cudaLaunchKernelExC(&lc, kernel, params));
+  }
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.compass_grid = grid; li.compass_block = block; li.compass_smem_bytes = (int)smem;
   li.compass_hit_stage = (int)hit_stage; li.compass_split = split; li.compass_view = view_ok ? 1 : 0;

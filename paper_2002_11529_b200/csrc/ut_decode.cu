@@ -107,6 +107,9 @@ __global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
   const uint32_t ns = a.g.n_sectors, ng = a.g.n_groups;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
 
+  // a dependent launch (compass_track with programmatic stream serialization) may be scheduled onto free SMs from now
+  // on; it waits for this grid's completion before it reads anything written here
+  asm volatile("griddepcontrol.launch_dependents;");
   Carver cv(smem_raw);
   // raw banks of the event; once every word is decoded the same bytes hold the sorted order (s_perm)
   unsigned char* s_rawstage = cv.take<unsigned char>(max(a.raw_stage_bytes, 4u * a.hit_stage));
