@@ -293,6 +293,35 @@ def test_cuda_graph_replay(gpu, wl):
         assert np.array_equal(compact.track_offsets.cpu().numpy().view(np.uint32), c_ref.track_offsets)
 
 
+def test_two_compass_calls_share_one_container(gpu, wl):
+    """DESIGN.md A21: the work ticket of compass_track lives in the OUTPUT (ut_tracks.status), so two calls that read
+    the same hit container with different configs and outputs may run at the same time on two streams."""
+    import dataclasses
+    import torch
+    from gpu_helpers import compare_tracks
+    B = gpu.B
+    g, b, p = wl(3, 200)
+    p2 = dataclasses.replace(p, min_hits=4, max_candidates_per_layer=8)
+    h_ref, t1 = oracle.run_batch(b, g, p)
+    _, t2 = oracle.run_batch(b, g, p2)
+    hits = gpu.decode(b.raw, b.bank_offsets, b.n_events, b.hit_capacity)
+    velo = B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z)
+    vo = B.to_device_u32(b.velo_offsets)
+    tr = [B.Tracks(b.n_velo_total), B.Tracks(b.n_velo_total)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for _ in range(5):
+        for k, cfg in enumerate((p, p2)):
+            B.compass_track(hits, hits.hit_offsets, velo, vo, b.n_events, B.make_config(cfg), tr[k], stream=streams[k])
+    torch.cuda.synchronize()
+    for k, ref in enumerate((t1, t2)):
+        idx, nh, qop, chi2 = tr[k].numpy()
+        got = dict(hit_idx=idx, n_hits=nh, qop=qop, chi2=chi2, status=int(tr[k].status[0].item()))
+        n_diff, _ = compare_tracks(ref, got)
+        assert n_diff == 0 and np.array_equal(chi2.view(np.uint32), ref.chi2.view(np.uint32))
+        assert int(tr[k].status[0].item()) == 0
+
+
 def test_two_host_threads(gpu, wl):
     """Two host threads, each with its own stream, container and outputs, call the library at the same time
     (per-device state is built under a lock; launch info and error text are thread-local)."""
