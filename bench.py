@@ -363,6 +363,23 @@ class DeviceWorkload:
         return ([e[0].elapsed_time(e[1]) for e in ev], [e[1].elapsed_time(e[2]) for e in ev],
                 [e[0].elapsed_time(e[2]) for e in ev])
 
+    def timed_steps(self, torch, flush, steps, warmup):
+        """CUDA events around each step, the two calls back to back (compass_track's programmatic launch behind ut_decode
+        needs them adjacent on the stream).  Returns the per-step ms list."""
+        stream = torch.cuda.current_stream()
+        for _ in range(warmup):
+            flush.zero_()
+            self.step()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(steps)]
+        torch.cuda.synchronize()
+        for k in range(steps):
+            flush.zero_()
+            ev[k][0].record(stream)
+            self.step()
+            ev[k][1].record(stream)
+        torch.cuda.synchronize()
+        return [e[0].elapsed_time(e[1]) for e in ev]
+
     def facts(self):
         ne, ng = self.batch.n_events, self.tables.n_groups
         n_hits = int(self.hits.hit_offsets[ne * ng].item()) & 0xFFFFFFFF
@@ -422,7 +439,8 @@ def per_config_report(B, torch, flush, prepared, hbm_peak, steps):
     rows = {}
     for cid, (cfg, geom_t, batch, params) in prepared.items():
         w = DeviceWorkload(B, geom_t, batch, params)
-        t_dec, t_cmp, t_step = w.timed(torch, flush, steps, 3)
+        t_step = w.timed_steps(torch, flush, steps, 3)                # the step: two calls back to back
+        t_dec, t_cmp, _ = w.timed(torch, flush, steps, 0)             # per kernel: an event between the calls
         n_hits, status = w.facts()
         ab = algorithmic_bytes(batch, geom_t, n_hits)
         md, mc, ms = statistics.mean(t_dec), statistics.mean(t_cmp), statistics.mean(t_step)
