@@ -293,6 +293,40 @@ def test_cuda_graph_replay(gpu, wl):
         assert np.array_equal(compact.track_offsets.cpu().numpy().view(np.uint32), c_ref.track_offsets)
 
 
+def test_back_to_back_calls_reuse_one_container(gpu, wl):
+    """ut_decode and compass_track issued back to back on one stream, 40 times, alternating between batches of
+    different sizes in the SAME container: compass_track is launched with programmatic stream serialization behind
+    ut_decode (its CTAs may be resident before the decode completes), and nothing of the previous batch may leak
+    into the next -- hits, offsets and tracks equal the oracle's every time."""
+    import torch
+    B = gpu.B
+    work = [wl(3, 1000), wl(2, 100), wl(3, 333)]
+    refs = [oracle.run_batch(b, g, p) for g, b, p in work]
+    cap = max(b.hit_capacity for _, b, _ in work)
+    hits = B.Hits(cap, 1000, gpu.geom)
+    dev = [(B.to_device_raw(b.raw), B.to_device_u32(b.bank_offsets),
+            B.VeloStates(b.velo_x, b.velo_y, b.velo_tx, b.velo_ty, b.velo_z), B.to_device_u32(b.velo_offsets),
+            B.Tracks(b.n_velo_total), B.make_config(p)) for _, b, p in work]
+    ng = gpu.tables.n_groups
+    for it in range(40):
+        k = it % len(work)
+        b = work[k][1]
+        raw, bo, velo, vo, tracks, cfg = dev[k]
+        B.ut_decode(raw, bo, b.n_events, gpu.geom, hits)
+        B.compass_track(hits, hits.hit_offsets, velo, vo, b.n_events, cfg, tracks)
+        torch.cuda.synchronize()
+        h_ref, t_ref = refs[k]
+        n = h_ref.n_hits
+        assert np.array_equal(hits.hit_offsets[:b.n_events * ng + 1].cpu().numpy().view(np.uint32), h_ref.hit_offsets)
+        assert np.array_equal(hits.x_at_y0[:n].cpu().numpy().view(np.uint32), h_ref.x_at_y0[:n].view(np.uint32))
+        assert np.array_equal(hits.id[:n].cpu().numpy().view(np.uint32), h_ref.id[:n])
+        idx, nh, qop, chi2 = tracks.numpy()
+        assert np.array_equal(idx, t_ref.hit_idx) and np.array_equal(nh, t_ref.n_hits)
+        assert np.array_equal(chi2.view(np.uint32), t_ref.chi2.view(np.uint32))
+        assert np.array_equal(qop.view(np.uint32), t_ref.qop.view(np.uint32))
+        assert int(tracks.status[0].item()) == 0
+
+
 def test_two_compass_calls_share_one_container(gpu, wl):
     """DESIGN.md A21: the work ticket of compass_track lives in the OUTPUT (ut_tracks.status), so two calls that read
     the same hit container with different configs and outputs may run at the same time on two streams."""
