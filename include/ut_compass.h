@@ -93,6 +93,8 @@ typedef struct {
   uint32_t kick_nx, kick_ny;
   float kick_x_lo, kick_y_lo, kick_inv_dx, kick_inv_dy, kick_z_ref;
   const float *kick_kappa, *kick_z_mag;   /* [kick_ny * kick_nx] */
+  float layer_weight[UT_N_LAYERS];        /* filled by ut_geometry_upload: the one weight of the layer's sectors when
+                                             UT_GEOM_LAYER_UNIFORM is set (HOST values inside the struct) */
 } ut_geometry;
 
 /* y_begin and y_end are non-decreasing over the sectors of every group: the sector row a track crosses
@@ -101,6 +103,9 @@ typedef struct {
 /* every group of a layer has the same number of sectors with the same y ranges, row by row: compass_track finds the
  * sector row a track crosses once per layer instead of once per group */
 #define UT_GEOM_ROWS_UNIFORM 2u
+/* every sector of layer l has z == layer_z[l] and the same weight (layer_weight[l]): compass_track takes the z and the
+ * weight of a candidate from the layer instead of from the sector rows (its own kernel variant) */
+#define UT_GEOM_LAYER_UNIFORM 4u
 
 /* Copies HOST tables (`host_tables` holds HOST pointers in the array fields) to the device, checks
  * the contract above and fills `device_out` with device pointers.  Synchronous; call once at set-up. */

@@ -40,7 +40,7 @@ class ut_geometry(C.Structure):
                 ("owner", C.c_void_p),
                 ("kick_nx", C.c_uint32), ("kick_ny", C.c_uint32), ("kick_x_lo", C.c_float), ("kick_y_lo", C.c_float),
                 ("kick_inv_dx", C.c_float), ("kick_inv_dy", C.c_float), ("kick_z_ref", C.c_float),
-                ("kick_kappa", C.c_void_p), ("kick_z_mag", C.c_void_p)]
+                ("kick_kappa", C.c_void_p), ("kick_z_mag", C.c_void_p), ("layer_weight", C.c_float * 4)]
 
 
 class ut_hits(C.Structure):

@@ -218,7 +218,13 @@ int32_t ut_geometry_upload(const ut_geometry* h, ut_geometry* out) {
     return d;
   };
   *out = *h;
-  out->flags = (rows_sorted ? UT_GEOM_ROWS_SORTED : 0u) | (rows_uniform ? UT_GEOM_ROWS_UNIFORM : 0u);
+  bool layer_uniform = true;                 // every sector of a layer at the layer's z, with one weight
+  for (uint32_t g = 0; g < ng; ++g)
+    for (uint32_t s2 = first[g]; s2 < first[g + 1]; ++s2)
+      if (h->z[s2] != h->layer_z[g / gpl] || h->weight[s2] != h->weight[first[(g / gpl) * gpl]]) layer_uniform = false;
+  out->flags = (rows_sorted ? UT_GEOM_ROWS_SORTED : 0u) | (rows_uniform ? UT_GEOM_ROWS_UNIFORM : 0u) |
+               (layer_uniform ? UT_GEOM_LAYER_UNIFORM : 0u);
+  for (uint32_t l = 0; l < UT_N_LAYERS; ++l) out->layer_weight[l] = layer_uniform ? h->weight[first[l * gpl]] : 0.f;
   out->id_to_sector = (const uint32_t*)put(h->id_to_sector, h->id_table_size * 4, sz_id);
   out->sector_raw_id = (const uint32_t*)put(h->sector_raw_id, ns * 4, sz_s);
   out->sector_group = (const uint32_t*)put(h->sector_group, ns * 4, sz_s);

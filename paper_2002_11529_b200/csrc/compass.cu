@@ -78,6 +78,7 @@ struct CompassArgs {
   const uint32_t *id_to_sector, *group_first_sector;
   const float *group_xmin, *group_xmax, *sec_yb, *sec_ye, *sec_dxdy, *sec_z, *sec_w;
   float layer_z[4], layer_dxdy[4];
+  float layer_w[4];                    // UT_GEOM_LAYER_UNIFORM: the one weight of the layer's sectors (LU kernels)
   compass_config c;
   int32_t *out_idx, *out_n;
   float *out_qop, *out_chi2;
@@ -192,7 +193,8 @@ __device__ __forceinline__ void note_zw(const CompassArgs& a, int s, bool first,
 // ---- phase 1: candidate list of one (track, layer) -------------------------------------
 // Group and sector row are found from a linear guess corrected against the tables (exact lower bound of
 // the same predicates the oracle's search uses; O(1) on a regular layout, any sorted layout works).
-template <bool BUCKETED>
+// LU: layer-uniform geometry (UT_GEOM_LAYER_UNIFORM): z and weight of a candidate are its layer's, nothing to note
+template <bool BUCKETED, bool LU>
 __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
                                               int l, float x_e, float y_e, uint32_t h0, float& zu, float& wu) {
   const int C = a.c.max_candidates_per_layer;
@@ -328,7 +330,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
             ++n;
           }
         }
-        if (n != n_before || took_any) note_zw(a, s, n_before == 0, zu, wu);
+        if (!LU && (n != n_before || took_any)) note_zw(a, s, n_before == 0, zu, wu);
       }
     } else if (a.order_y) {
       // Y-sorted group: "two binary searches over the Y axis, one to delimit the beginning of the
@@ -353,7 +355,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;
         const bool first_cand = n == 0;
-        if (cand_insert(wa, slot, n, C, d, (h << 16) | s)) note_zw(a, (int)s, first_cand, zu, wu);
+        if (cand_insert(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
       }
     } else {
       const float* X = a.hx + h0;
@@ -372,7 +374,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;             // reported by the staging pass of the bucketed path only
         const bool first_cand = n == 0;
-        if (cand_insert(wa, slot, n, C, d, (h << 16) | s)) note_zw(a, (int)s, first_cand, zu, wu);
+        if (cand_insert(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
       }
     }
   }
@@ -596,7 +598,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
 }
 
 // The warps of the CTA pull 8-track batches of the item: track m of the item is VELO track t0 + m * K + part.
-template <bool BUCKETED, bool INTERVAL, bool KICK>
+template <bool BUCKETED, bool INTERVAL, bool KICK, bool LU>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
                                            uint32_t h0, uint32_t t0, uint32_t nTk, uint32_t part, uint32_t T,
                                            const uint16_t* perm) {
@@ -614,13 +616,13 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     const uint32_t tg = t0 + (active ? (perm ? (uint32_t)perm[ti] : ti) * a.split + part : 0u);
     // ---------------- phase 1: window search, lane = (track, layer) ---------------------------------------
     int n_st = 0;
-    float zu = 0.f, wu = 0.f;
+    float zu = LU ? a.layer_z[l] : 0.f, wu = LU ? a.layer_w[l] : 0.f;
     if (active) {
       const float vx = __ldg(a.vx + tg), vy = __ldg(a.vy + tg), vtx = __ldg(a.vtx + tg), vty = __ldg(a.vty + tg);
       const float dzv = __fsub_rn(a.layer_z[l], a.vz);
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
-      n_st = collect_window<BUCKETED>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
+      n_st = collect_window<BUCKETED, LU>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
       if (KICK && l == 0) track_kick(a.kick, a.c, vx, vy, vtx, vty, a.vz, wa.tkap[lane >> 2], wa.tzm[lane >> 2]);
     } else if (KICK && l == 0) {
       wa.tkap[lane >> 2] = a.c.kappa;
@@ -637,12 +639,12 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       wa.srt[lane] = srt;
     }
     if (lane < kTPW) wa.best[lane] = kNoKey;
-    const bool uni = __all_sync(0xFFFFFFFFu, zu == zu);      // every list of the batch has one z and one weight
+    const bool uni = LU || __all_sync(0xFFFFFFFFu, zu == zu);      // every list of the batch has one z and one weight
     __syncwarp();
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
     const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    if (uni) find_tracklets<true, INTERVAL, KICK>(a, wa, lane, todo);
+    if (LU || uni) find_tracklets<true, INTERVAL, KICK>(a, wa, lane, todo);
     else find_tracklets<false, false, KICK>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
@@ -664,8 +666,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
           if (pr[k]) {
             const uint32_t hs = wa.chs[(q4 + k) * CS + pp[k]];
             d[k] = wa.cd[(q4 + k) * CS + pp[k]];
-            z[k] = __ldg(a.sec_z + (hs & 0xFFFFu));
-            w[k] = __ldg(a.sec_w + (hs & 0xFFFFu));
+            z[k] = LU ? a.layer_z[k] : __ldg(a.sec_z + (hs & 0xFFFFu));
+            w[k] = LU ? a.layer_w[k] : __ldg(a.sec_w + (hs & 0xFFFFu));
             if (k == l) hidx = (int)(h0 + (hs >> 16));
           }
         }
@@ -684,7 +686,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
 // max_candidates_per_layer allows long lists; the kernel without it is the faster one for short lists).
 // KICK: per-track kappa / z_mag from the kick table (ut_geometry.kick_*); without it the config's constants come
 // straight from the kernel parameters.
-template <int MAXT, int MINB, bool INTERVAL, bool KICK>
+template <int MAXT, int MINB, bool INTERVAL, bool KICK, bool LU>
 __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -969,9 +971,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     __syncthreads();                               // order and staged data visible; scratch is dead from here on
     if (staged) {
-      track_loop<true, INTERVAL, KICK>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<true, INTERVAL, KICK, LU>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false, INTERVAL, KICK>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<false, INTERVAL, KICK, LU>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     }
   }
   if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
@@ -995,11 +997,13 @@ static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32
 // where shared memory allows one CTA per SM and only more warps per CTA raise the occupancy).
 constexpr int kSmallBlock = 224;
 constexpr int kLargeBlock = 640;             // (a 768-thread bound caps the kernel at 80 registers and it spills; 640: 84-88, none)
-#define UTC_K(T, B, I, K) reinterpret_cast<const void*>(&compass_kernel<T, B, I, K>)
-static const void* const kKernels[2][2][2] = {     // [large CTAs][interval search][kick table]
-    {{UTC_K(kSmallBlock, 4, false, false), UTC_K(kSmallBlock, 4, false, true)},
-     {UTC_K(kSmallBlock, 4, true, false), UTC_K(kSmallBlock, 4, true, true)}},
-    {{UTC_K(kLargeBlock, 1, false, false), UTC_K(kLargeBlock, 1, false, true)}, {UTC_K(kLargeBlock, 1, true, false), UTC_K(kLargeBlock, 1, true, true)}}};
+#define UTC_K(T, B, I, K, U) reinterpret_cast<const void*>(&compass_kernel<T, B, I, K, U>)
+// [large CTAs][interval search][2: kick table, 1: layer-uniform geometry (UT_GEOM_LAYER_UNIFORM) without kick table, 0: neither]
+static const void* const kKernels[2][2][3] = {
+    {{UTC_K(kSmallBlock, 4, false, false, false), UTC_K(kSmallBlock, 4, false, false, true), UTC_K(kSmallBlock, 4, false, true, false)},
+     {UTC_K(kSmallBlock, 4, true, false, false), UTC_K(kSmallBlock, 4, true, false, true), UTC_K(kSmallBlock, 4, true, true, false)}},
+    {{UTC_K(kLargeBlock, 1, false, false, false), UTC_K(kLargeBlock, 1, false, false, true), UTC_K(kLargeBlock, 1, false, true, false)},
+     {UTC_K(kLargeBlock, 1, true, false, false), UTC_K(kLargeBlock, 1, true, false, true), UTC_K(kLargeBlock, 1, true, true, false)}}};
 #undef UTC_K
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
@@ -1011,9 +1015,11 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   const ut_tuning tune = tuning_snapshot();
   const int interval_min = tuned(tune.compass_interval_min, 16);
   const int iv = cfg->max_candidates_per_layer > interval_min ? 1 : 0;    // long partner lists are possible
-  const int kk = hits->geom->kick_nx != 0 ? 1 : 0;                        // per-track kick from the table
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[0][iv][kk], kSlotCompassSmall + 2 * iv + kk, &max_smem)) return rc;
-  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[1][iv][kk], kSlotCompassLarge + 2 * iv + kk, &max_smem_large)) return rc;
+  // kernel variant: 2 = per-track kick from the table, 1 = layer-uniform geometry (z and weight of a candidate are its
+  // layer's), 0 = the general kernel
+  const int kk = hits->geom->kick_nx != 0 ? 2 : ((hits->geom->flags & UT_GEOM_LAYER_UNIFORM) ? 1 : 0);
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[0][iv][kk], kSlotCompassSmall + 3 * iv + kk, &max_smem)) return rc;
+  if (const int32_t rc = kernel_max_dynamic_smem(kKernels[1][iv][kk], kSlotCompassLarge + 3 * iv + kk, &max_smem_large)) return rc;
   max_smem = std::min(max_smem, max_smem_large);
   const int n_sm = dev.n_sm, sm_smem = dev.smem_per_sm;
   const ut_geometry* geom = hits->geom;
@@ -1037,7 +1043,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   a.id_to_sector = geom->id_to_sector; a.group_first_sector = geom->group_first_sector;
   a.group_xmin = geom->group_xmin; a.group_xmax = geom->group_xmax;
   a.sec_yb = geom->y_begin; a.sec_ye = geom->y_end; a.sec_dxdy = geom->dxdy; a.sec_z = geom->z; a.sec_w = geom->weight;
-  for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; }
+  for (int l = 0; l < 4; ++l) { a.layer_z[l] = geom->layer_z[l]; a.layer_dxdy[l] = geom->layer_dxdy[l]; a.layer_w[l] = geom->layer_weight[l]; }
   a.c = *cfg;
   a.kick = make_kick_table(geom);
   a.slope_lim = cfg->max_slope * (1.0f + kFilterEps);
