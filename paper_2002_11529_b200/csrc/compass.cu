@@ -382,13 +382,14 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
 }
 
 // z of candidate `i` of `slot` (UNI: every list of the batch has one z, kept per slot)
-template <bool UNI>
+// (LU: layer-uniform geometry, the z of slot's layer straight from the kernel parameters)
+template <bool UNI, bool LU = false>
 __device__ __forceinline__ float cand_z(const CompassArgs& a, const WarpArea& wa, int slot, int i) {
-  return UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * wa.CS + i] & 0xFFFFu));
+  return LU ? a.layer_z[slot & 3] : (UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * wa.CS + i] & 0xFFFFu)));
 }
 
 // ---- phase 2 (b) + (c): `cnt` queued seeds, one per lane, then all their 3/4-hit combinations --------------
-template <bool UNI, bool KICK>
+template <bool UNI, bool KICK, bool LU>
 __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpArea& wa, int lane, int cnt, int qhead,
                                               int dir) {
   const int LA = dir ? 3 : 0, LB = dir ? 1 : 2, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
@@ -408,7 +409,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
       const uint32_t sd = wa.seedq[(qhead + q) & (kSeedQ - 1)];
       const int j4 = (int)(sd >> 10) * 4, ia = (sd >> 5) & 31, ib = sd & 31;
       const float da = wa.cd[(j4 + LA) * CS + ia], db = wa.cd[(j4 + LB) * CS + ib];
-      const float za = cand_z<UNI>(a, wa, j4 + LA, ia), zb = cand_z<UNI>(a, wa, j4 + LB, ib);
+      const float za = cand_z<UNI, LU>(a, wa, j4 + LA, ia), zb = cand_z<UNI, LU>(a, wa, j4 + LB, ib);
       const float bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
       const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, KICK ? wa.tzm[sd >> 10] : a.c.z_mag)));
       ok = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
@@ -417,8 +418,8 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
         const float* cC = wa.cd + (j4 + LC) * CS;
         const float* cDl = wa.cd + (j4 + LD) * CS;
         if (UNI) {
-          const float predC = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(wa.zs[j4 + LC], za)));
-          const float predD = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(wa.zs[j4 + LD], za)));
+          const float predC = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(LU ? a.layer_z[LC] : wa.zs[j4 + LC], za)));
+          const float predD = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(LU ? a.layer_z[LD] : wa.zs[j4 + LD], za)));
           for (int i = sub; i < nC; i += 4)
             if (fabsf(__fsub_rn(cC[i], predC)) <= a.c.seed_tol) pC |= 1u << i;
           for (int i = sub; i < nD; i += 4)
@@ -483,7 +484,8 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
         if (pr[l]) {
           const int slot = j * 4 + l;
           d[l] = wa.cd[slot * CS + pos[l]];
-          if (UNI) { z[l] = wa.zs[slot]; w[l] = wa.ws[slot]; }
+          if (LU) { z[l] = a.layer_z[l]; w[l] = a.layer_w[l]; }
+          else if (UNI) { z[l] = wa.zs[slot]; w[l] = wa.ws[slot]; }
           else {
             const uint32_t s = wa.chs[slot * CS + pos[l]] & 0xFFFFu;
             z[l] = __ldg(a.sec_z + s);
@@ -503,7 +505,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 // ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
 // (process_seeds has ONE call site per variant: the kernel's code size decides how well it stays in the
 //  instruction cache)
-template <bool UNI, bool INTERVAL, bool KICK>
+template <bool UNI, bool INTERVAL, bool KICK, bool LU>
 __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
   const int j = lane & 7;
   const int CS = wa.CS;
@@ -531,9 +533,9 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
       float da = 0.f, za = 0.f, zam = 0.f, rinv = 0.f, lim0 = 0.f;
       if (i < total) {
         da = wa.cd[sA * CS + ia];
-        za = cand_z<UNI>(a, wa, sA, (int)ia);
+        za = cand_z<UNI, LU>(a, wa, sA, (int)ia);
         zam = za - (KICK ? wa.tzm[jj] : a.c.z_mag);
-        if (UNI) rinv = rcp_approx(wa.zs[sB] - za);
+        if (UNI) rinv = rcp_approx((LU ? a.layer_z[LB] : wa.zs[sB]) - za);
         lim0 = a.c.kink_tol + kFilterEps * (a.c.kink_tol + fabsf(da));
       } else {
         nBj = 0;
@@ -545,7 +547,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         // can pass the slope and kink cuts are an interval of d, found by two searches instead of a walk over the
         // whole list.  [lo, hi] contains every db the cuts accept (real arithmetic widened by 1e-5 relative; a NaN
         // bound opens the interval), the filter below and the exact cuts still decide.
-        const float dz = wa.zs[sB] - za, sdz = a.slope_lim * fabsf(dz);
+        const float dz = (LU ? a.layer_z[LB] : wa.zs[sB]) - za, sdz = a.slope_lim * fabsf(dz);
         const float rho = zam * rinv, rr = rcp_approx(rho);
         const float k1 = a.c.kink_tol * (1.f + 1e-5f);
         const float qa = (da - k1) * rr, qb = (da + k1) * rr;
@@ -585,7 +587,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         while (qn >= 32 || (last && qn > 0)) {  // a full queue, or the rest after the last pair
           __syncwarp();
           const int cnt = min(qn, 32);
-          process_seeds<UNI, KICK>(a, wa, lane, cnt, qhead, dir);
+          process_seeds<UNI, KICK, LU>(a, wa, lane, cnt, qhead, dir);
           qhead += cnt;
           qn -= cnt;
           __syncwarp();
@@ -629,8 +631,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       wa.tzm[lane >> 2] = a.c.z_mag;
     }
     wa.n[lane] = n_st;
-    wa.zs[lane] = zu;
-    wa.ws[lane] = wu;
+    if (!LU) { wa.zs[lane] = zu; wa.ws[lane] = wu; }
     // long lists that ascend in d (one x-sorted run, or runs of x-disjoint sectors) are searched, not walked
     if (INTERVAL && __any_sync(0xFFFFFFFFu, n_st > a.interval_min)) {
       int srt = 1;
@@ -644,8 +645,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
     const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    if (LU || uni) find_tracklets<true, INTERVAL, KICK>(a, wa, lane, todo);
-    else find_tracklets<false, false, KICK>(a, wa, lane, todo);
+    if (LU || uni) find_tracklets<true, INTERVAL, KICK, LU>(a, wa, lane, todo);
+    else find_tracklets<false, false, KICK, false>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
       const int q4 = lane & ~3;
