@@ -43,7 +43,7 @@ int32_t cuda_fail(const char* what, cudaError_t err);
 // devices and host threads may call into the library.
 struct DeviceInfo { int device, n_sm, smem_optin, smem_per_sm; };
 enum KernelSlot { kSlotDecode = 0, kSlotCompassSmall = 1, kSlotCompassLarge = 7, kSlotWindows = 13, kSlotTracklets = 14,
-                  kNumKernelSlots = 16 };     // (6 Compass slots each: interval search x {general, layer-uniform, kick table})
+                  kSlotCompassC16 = 15, kNumKernelSlots = 16 };     // (6 Compass slots each: interval search x {general, layer-uniform, kick table})
 int32_t device_info(DeviceInfo* out);
 // largest dynamic shared-memory size `kernel` may ask for on the current device (opted in on its first use there)
 int32_t kernel_max_dynamic_smem(const void* kernel, int slot, int* max_dyn);

@@ -125,15 +125,19 @@ struct WarpArea {
 };
 
 __host__ __device__ inline int cand_stride(int C) { return C | 1; }
+// CC: max_candidates_per_layer as a compile-time constant (0: the run-time value): strides and caps fold into the code
+template <int CC>
+__device__ __forceinline__ int stride_of(const WarpArea& wa) { return CC ? (CC | 1) : wa.CS; }
 __host__ __device__ inline size_t warp_area_bytes(int C) {
   return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 4 + kTPW * 4 * 2;
 }
 
 // Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
 // Returns false when the list is full and the new hit is not closer than its worst entry.
+template <int CC>
 __device__ __forceinline__ bool cand_insert(const WarpArea& wa, int slot, int& n, int C, float d, uint32_t hs) {
-  float* cd = wa.cd + slot * wa.CS;
-  uint32_t* chs = wa.chs + slot * wa.CS;
+  float* cd = wa.cd + slot * stride_of<CC>(wa);
+  uint32_t* chs = wa.chs + slot * stride_of<CC>(wa);
   if (n == C) {
     int worst = 0;
     float wabs = fabsf(cd[0]);
@@ -194,16 +198,16 @@ __device__ __forceinline__ void note_zw(const CompassArgs& a, int s, bool first,
 // Group and sector row are found from a linear guess corrected against the tables (exact lower bound of
 // the same predicates the oracle's search uses; O(1) on a regular layout, any sorted layout works).
 // LU: layer-uniform geometry (UT_GEOM_LAYER_UNIFORM): z and weight of a candidate are its layer's, nothing to note
-template <bool BUCKETED, bool LU>
+template <bool BUCKETED, bool LU, int CC>
 __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
                                               int l, float x_e, float y_e, uint32_t h0, float& zu, float& wu) {
-  const int C = a.c.max_candidates_per_layer;
+  const int C = CC ? CC : a.c.max_candidates_per_layer;
   const float D = a.c.win_half[l], negD = -D;
   const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
   const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
   const int g0 = l * (int)a.gpl, g1 = g0 + (int)a.gpl;
-  float* cd = wa.cd + slot * wa.CS;
-  uint32_t* chs = wa.chs + slot * wa.CS;
+  float* cd = wa.cd + slot * stride_of<CC>(wa);
+  uint32_t* chs = wa.chs + slot * stride_of<CC>(wa);
   const int pad = 2 * l;                            // bank padding of the group tables
   int g;
   {                                                 // first group with group_xmax >= lo
@@ -317,7 +321,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
           const bool acc = d >= negD;
           const uint32_t hs = ((uint32_t)S.hh[p] << 16) | (uint32_t)s;
           if (acc && (n >= C || (n > 0 && hs <= last))) {   // rare: cap reached or out of hit order
-            const bool took = cand_insert(wa, slot, n, C, d, hs);
+            const bool took = cand_insert<CC>(wa, slot, n, C, d, hs);
             took_any |= took;
             last = chs[n - 1];
             if (!took && d >= 0.f) break;           // full list, positive side: every later hit is further still
@@ -355,7 +359,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;
         const bool first_cand = n == 0;
-        if (cand_insert(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
+        if (cand_insert<CC>(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
       }
     } else {
       const float* X = a.hx + h0;
@@ -374,7 +378,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
         const uint32_t s = rid < a.id_table_size ? __ldg(a.id_to_sector + rid) : kInvalid;
         if (s >= a.n_sectors) continue;             // reported by the staging pass of the bucketed path only
         const bool first_cand = n == 0;
-        if (cand_insert(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
+        if (cand_insert<CC>(wa, slot, n, C, d, (h << 16) | s) && !LU) note_zw(a, (int)s, first_cand, zu, wu);
       }
     }
   }
@@ -383,17 +387,17 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
 
 // z of candidate `i` of `slot` (UNI: every list of the batch has one z, kept per slot)
 // (LU: layer-uniform geometry, the z of slot's layer straight from the kernel parameters)
-template <bool UNI, bool LU = false>
+template <bool UNI, bool LU = false, int CC = 0>
 __device__ __forceinline__ float cand_z(const CompassArgs& a, const WarpArea& wa, int slot, int i) {
-  return LU ? a.layer_z[slot & 3] : (UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * wa.CS + i] & 0xFFFFu)));
+  return LU ? a.layer_z[slot & 3] : (UNI ? wa.zs[slot] : __ldg(a.sec_z + (wa.chs[slot * stride_of<CC>(wa) + i] & 0xFFFFu)));
 }
 
 // ---- phase 2 (b) + (c): `cnt` queued seeds, one per lane, then all their 3/4-hit combinations --------------
-template <bool UNI, bool KICK, bool LU>
+template <bool UNI, bool KICK, bool LU, int CC>
 __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpArea& wa, int lane, int cnt, int qhead,
                                               int dir) {
   const int LA = dir ? 3 : 0, LB = dir ? 1 : 2, LC = dir ? 2 : 1, LD = dir ? 0 : 3;
-  const int CS = wa.CS;
+  const int CS = stride_of<CC>(wa);
   const bool min3 = a.c.min_hits == 3;
   // (b) 4 lanes share one seed (8 seeds per round): the exact cuts of step 5, then every 4th hit of the two
   //     other layers per lane; the masks of compatible hits end up in lane = seed index
@@ -409,7 +413,7 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
       const uint32_t sd = wa.seedq[(qhead + q) & (kSeedQ - 1)];
       const int j4 = (int)(sd >> 10) * 4, ia = (sd >> 5) & 31, ib = sd & 31;
       const float da = wa.cd[(j4 + LA) * CS + ia], db = wa.cd[(j4 + LB) * CS + ib];
-      const float za = cand_z<UNI, LU>(a, wa, j4 + LA, ia), zb = cand_z<UNI, LU>(a, wa, j4 + LB, ib);
+      const float za = cand_z<UNI, LU, CC>(a, wa, j4 + LA, ia), zb = cand_z<UNI, LU, CC>(a, wa, j4 + LB, ib);
       const float bs = __fdiv_rn(__fsub_rn(db, da), __fsub_rn(zb, za));
       const float a0 = __fsub_rn(da, __fmul_rn(bs, __fsub_rn(za, KICK ? wa.tzm[sd >> 10] : a.c.z_mag)));
       ok = fabsf(bs) <= a.c.max_slope && fabsf(a0) <= a.c.kink_tol;
@@ -426,12 +430,12 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
             if (fabsf(__fsub_rn(cDl[i], predD)) <= a.c.seed_tol) pD |= 1u << i;
         } else {
           for (int i = sub; i < nC; i += 4) {
-            const float zc = cand_z<false>(a, wa, j4 + LC, i);
+            const float zc = cand_z<false, false, CC>(a, wa, j4 + LC, i);
             const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zc, za)));
             if (fabsf(__fsub_rn(cC[i], pred)) <= a.c.seed_tol) pC |= 1u << i;
           }
           for (int i = sub; i < nD; i += 4) {
-            const float zd = cand_z<false>(a, wa, j4 + LD, i);
+            const float zd = cand_z<false, false, CC>(a, wa, j4 + LD, i);
             const float pred = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(zd, za)));
             if (fabsf(__fsub_rn(cDl[i], pred)) <= a.c.seed_tol) pD |= 1u << i;
           }
@@ -505,10 +509,10 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
 // ---- phase 2 (a): seed rows of the batch, conservative filter of the slope + kink cuts, seed queue -----------
 // (process_seeds has ONE call site per variant: the kernel's code size decides how well it stays in the
 //  instruction cache)
-template <bool UNI, bool INTERVAL, bool KICK, bool LU>
+template <bool UNI, bool INTERVAL, bool KICK, bool LU, int CC>
 __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpArea& wa, int lane, uint32_t todo) {
   const int j = lane & 7;
-  const int CS = wa.CS;
+  const int CS = stride_of<CC>(wa);
   const uint32_t lt_mask = (1u << lane) - 1u;
   for (int dir = 0; dir < 2 && todo; ++dir) {     // forward seeds (L0, L2), then backward (L3, L1)
     const int LA = dir ? 3 : 0, LB = dir ? 1 : 2;
@@ -533,7 +537,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
       float da = 0.f, za = 0.f, zam = 0.f, rinv = 0.f, lim0 = 0.f;
       if (i < total) {
         da = wa.cd[sA * CS + ia];
-        za = cand_z<UNI, LU>(a, wa, sA, (int)ia);
+        za = cand_z<UNI, LU, CC>(a, wa, sA, (int)ia);
         zam = za - (KICK ? wa.tzm[jj] : a.c.z_mag);
         if (UNI) rinv = rcp_approx((LU ? a.layer_z[LB] : wa.zs[sB]) - za);
         lim0 = a.c.kink_tol + kFilterEps * (a.c.kink_tol + fabsf(da));
@@ -573,7 +577,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         bool pass = false;
         const int ib = INTERVAL ? ib0 + ik : ik;
         if (ik < nBj) {
-          if (!UNI) rinv = rcp_approx(cand_z<false>(a, wa, sB, ib) - za);
+          if (!UNI) rinv = rcp_approx(cand_z<false, false, CC>(a, wa, sB, ib) - za);
           const float bsa = (cB[ib] - da) * rinv;
           const float t = bsa * zam;
           pass = fabsf(bsa) <= a.slope_lim && fabsf(da - t) <= __fmaf_rn(kFilterEps, fabsf(t), lim0);
@@ -587,7 +591,7 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
         while (qn >= 32 || (last && qn > 0)) {  // a full queue, or the rest after the last pair
           __syncwarp();
           const int cnt = min(qn, 32);
-          process_seeds<UNI, KICK, LU>(a, wa, lane, cnt, qhead, dir);
+          process_seeds<UNI, KICK, LU, CC>(a, wa, lane, cnt, qhead, dir);
           qhead += cnt;
           qn -= cnt;
           __syncwarp();
@@ -600,14 +604,14 @@ __device__ __forceinline__ void find_tracklets(const CompassArgs& a, const WarpA
 }
 
 // The warps of the CTA pull 8-track batches of the item: track m of the item is VELO track t0 + m * K + part.
-template <bool BUCKETED, bool INTERVAL, bool KICK, bool LU>
+template <bool BUCKETED, bool INTERVAL, bool KICK, bool LU, int CC>
 __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int* s_ticket,
                                            uint32_t h0, uint32_t t0, uint32_t nTk, uint32_t part, uint32_t T,
                                            const uint16_t* perm) {
   const int lane = threadIdx.x & 31;
   const int l = lane & 3;                         // layer of this lane in phase 1 and in the output
   const int j = lane & 7;                         // track-in-batch this lane does the bookkeeping for (lanes 0..7)
-  const int CS = wa.CS;
+  const int CS = stride_of<CC>(wa);
   for (;;) {
     int batch = 0;
     if (lane == 0) batch = atomicAdd(s_ticket, 1);
@@ -624,7 +628,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
       const float dzv = __fsub_rn(a.layer_z[l], a.vz);
       const float x_e = __fadd_rn(vx, __fmul_rn(vtx, dzv));
       const float y_e = __fadd_rn(vy, __fmul_rn(vty, dzv));
-      n_st = collect_window<BUCKETED, LU>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
+      n_st = collect_window<BUCKETED, LU, CC>(a, wa, S, lane, l, x_e, y_e, h0, zu, wu);
       if (KICK && l == 0) track_kick(a.kick, a.c, vx, vy, vtx, vty, a.vz, wa.tkap[lane >> 2], wa.tzm[lane >> 2]);
     } else if (KICK && l == 0) {
       wa.tkap[lane >> 2] = a.c.kappa;
@@ -645,8 +649,8 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
     // ---------------- phase 2: tracklet finding, flattened over the warp ---------------
     const int nonempty = (wa.n[4 * j] > 0) + (wa.n[4 * j + 1] > 0) + (wa.n[4 * j + 2] > 0) + (wa.n[4 * j + 3] > 0);
     const uint32_t todo = __ballot_sync(0xFFFFFFFFu, lane < kTPW && nonempty >= a.c.min_hits);
-    if (LU || uni) find_tracklets<true, INTERVAL, KICK, LU>(a, wa, lane, todo);
-    else find_tracklets<false, false, KICK, false>(a, wa, lane, todo);
+    if (LU || uni) find_tracklets<true, INTERVAL, KICK, LU, CC>(a, wa, lane, todo);
+    else find_tracklets<false, false, KICK, false, CC>(a, wa, lane, todo);
     // ---------------- output: the 4 lanes of a track write one layer each ----------------------------------
     if (active) {
       const int q4 = lane & ~3;
@@ -687,7 +691,7 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
 // max_candidates_per_layer allows long lists; the kernel without it is the faster one for short lists).
 // KICK: per-track kappa / z_mag from the kick table (ut_geometry.kick_*); without it the config's constants come
 // straight from the kernel parameters.
-template <int MAXT, int MINB, bool INTERVAL, bool KICK, bool LU>
+template <int MAXT, int MINB, bool INTERVAL, bool KICK, bool LU, int CC = 0>
 __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -972,9 +976,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     }
     __syncthreads();                               // order and staged data visible; scratch is dead from here on
     if (staged) {
-      track_loop<true, INTERVAL, KICK, LU>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<true, INTERVAL, KICK, LU, CC>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     } else {                                       // event larger than the staging size: window search on global memory
-      track_loop<false, INTERVAL, KICK, LU>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
+      track_loop<false, INTERVAL, KICK, LU, CC>(a, wa, S, &s_ticket, h0, t0, nTk, part, T, perm);
     }
   }
   if (tid == 0) {                             // last CTA out re-arms the ticket for the next call
@@ -1006,6 +1010,8 @@ static const void* const kKernels[2][2][3] = {
     {{UTC_K(kLargeBlock, 1, false, false, false), UTC_K(kLargeBlock, 1, false, false, true), UTC_K(kLargeBlock, 1, false, true, false)},
      {UTC_K(kLargeBlock, 1, true, false, false), UTC_K(kLargeBlock, 1, true, false, true), UTC_K(kLargeBlock, 1, true, true, false)}}};
 #undef UTC_K
+// the metric's configuration (small CTAs, layer-uniform geometry, C = 16) with the cap compiled in
+static const void* const kKernelC16 = reinterpret_cast<const void*>(&compass_kernel<kSmallBlock, 4, false, false, true, 16>);
 
 int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const velo_states* velo,
                        const uint32_t* velo_offsets, int32_t n_events, const compass_config* cfg, ut_tracks* out,
@@ -1102,6 +1108,11 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     }
   }
   const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv][kk];
+  if (block <= kSmallBlock && iv == 0 && kk == 1 && C == 16) {
+    int dummy = 0;
+    if (const int32_t rc = kernel_max_dynamic_smem(kKernelC16, kSlotCompassC16, &dummy)) return rc;
+    kernel = kKernelC16;
+  }
   int per_sm = 0;
   UTC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem));
   if (per_sm < 1) return cuda_fail("compass kernel does not fit on an SM", cudaErrorInvalidConfiguration);
