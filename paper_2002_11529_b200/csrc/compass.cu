@@ -125,7 +125,8 @@ struct WarpArea {
 };
 
 __host__ __device__ inline int cand_stride(int C) { return C | 1; }
-// CC: max_candidates_per_layer as a compile-time constant (0: the run-time value): strides and caps fold into the code
+// CC: max_candidates_per_layer as a compile-time constant (0: the run-time value): strides and caps fold into the code;
+// kernels with CC are for row-uniform geometries (UT_GEOM_ROWS_UNIFORM), whose per-sector y search they leave out
 template <int CC>
 __device__ __forceinline__ int stride_of(const WarpArea& wa) { return CC ? (CC | 1) : wa.CS; }
 __host__ __device__ inline size_t warp_area_bytes(int C) {
@@ -219,7 +220,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
   }
   // rows_uniform: the sector rows the track crosses, once for all groups of the layer (rows r0 .. r0 + nr - 1)
   int r0 = 0, nr = 0;
-  if (BUCKETED && a.rows_uniform) {
+  if (BUCKETED && (CC || a.rows_uniform)) {       // (CC kernels are chosen for row-uniform geometries only)
     const int R = (int)a.rows_uniform;
     const float2* yr = S.yr + l * R;
     const float4 grp0 = S.gA[g0 + pad];
@@ -242,7 +243,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
       const uint2 gi = S.gB[g + pad];
       const int sa = (int)(gi.y & 0xFFFFu);
       int s = sa, sb = (int)(gi.y >> 16);
-      const bool per_sector_y = a.rows_uniform == 0;
+      const bool per_sector_y = CC ? false : a.rows_uniform == 0;
       if (!per_sector_y) {
         s = sa + r0;
         sb = s + nr;
@@ -1108,7 +1109,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     }
   }
   const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv][kk];
-  if (block <= kSmallBlock && iv == 0 && kk == 1 && C == 16) {
+  if (block <= kSmallBlock && iv == 0 && kk == 1 && C == 16 && a.rows_uniform != 0) {
     int dummy = 0;
     if (const int32_t rc = kernel_max_dynamic_smem(kKernelC16, kSlotCompassC16, &dummy)) return rc;
     kernel = kKernelC16;
