@@ -203,7 +203,9 @@ template <bool BUCKETED, bool LU, int CC>
 __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpArea& wa, const SmemView& S, int slot,
                                               int l, float x_e, float y_e, uint32_t h0, float& zu, float& wu) {
   const int C = CC ? CC : a.c.max_candidates_per_layer;
-  const float D = a.c.win_half[l], negD = -D;
+  float D = a.c.win_half[l];
+  asm volatile("" : "+f"(D));                     // keep D in a register: the indexed constant load is not redone per hit
+  const float negD = -D;
   const float ctr = __fsub_rn(x_e, __fmul_rn(a.layer_dxdy[l], y_e));
   const float lo = __fsub_rn(__fsub_rn(ctr, D), kGroupEps), hi = __fadd_rn(__fadd_rn(ctr, D), kGroupEps);
   const int g0 = l * (int)a.gpl, g1 = g0 + (int)a.gpl;
