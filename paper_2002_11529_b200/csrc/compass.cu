@@ -143,14 +143,31 @@ __device__ __forceinline__ bool cand_insert(const WarpArea& wa, int slot, int& n
     int worst = 0;
     float wabs = fabsf(cd[0]);
     uint32_t whs = chs[0];
-    for (int i = 1; i < C; ++i) {
-      const float v = fabsf(cd[i]);
-      const uint32_t k = chs[i];
-      if (v > wabs || (v == wabs && k > whs)) { wabs = v; whs = k; worst = i; }
+    // In the kernels with a compile-time cap the compiler would unroll these loops C times; full lists are rare at
+    // their settings and the kernel's code size matters more (config 3: 109.0 -> 106.2 us), so they stay rolled there.
+    // The general kernels serve the long lists of C = 32, where the unrolled loops are the faster ones.
+    if (CC != 0) {
+#pragma unroll 1
+      for (int i = 1; i < C; ++i) {
+        const float v = fabsf(cd[i]);
+        const uint32_t k = chs[i];
+        if (v > wabs || (v == wabs && k > whs)) { wabs = v; whs = k; worst = i; }
+      }
+    } else {
+      for (int i = 1; i < C; ++i) {
+        const float v = fabsf(cd[i]);
+        const uint32_t k = chs[i];
+        if (v > wabs || (v == wabs && k > whs)) { wabs = v; whs = k; worst = i; }
+      }
     }
     const float nabs = fabsf(d);
     if (!(nabs < wabs || (nabs == wabs && hs < whs))) return false;
-    for (int i = worst; i < C - 1; ++i) { cd[i] = cd[i + 1]; chs[i] = chs[i + 1]; }
+    if (CC != 0) {
+#pragma unroll 1
+      for (int i = worst; i < C - 1; ++i) { cd[i] = cd[i + 1]; chs[i] = chs[i + 1]; }
+    } else {
+      for (int i = worst; i < C - 1; ++i) { cd[i] = cd[i + 1]; chs[i] = chs[i + 1]; }
+    }
     n = C - 1;
   }
   int i = n;
