@@ -305,6 +305,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
               uint32_t L = zc, R = zc;                        // the stretch is [L, R)
               float dl = L > p ? fabsf(__fsub_rn(__fadd_rn(S.hx[L - 1], syg), x_e)) : 0.f;
               float dr = R < ub ? fabsf(__fsub_rn(__fadd_rn(S.hx[R], syg), x_e)) : 0.f;
+#pragma unroll 1                                     // (rare, and C may be a compile-time constant: keep the code small)
               for (int k = 0; k < C; ++k) {
                 const bool left = L > p && (R >= ub || dl <= dr);
                 if (left) { --L; dl = L > p ? fabsf(__fsub_rn(__fadd_rn(S.hx[L - 1], syg), x_e)) : 0.f; }
