@@ -285,7 +285,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
             const uint32_t half = cnt >> 1, mid = p + half;
             if (__fsub_rn(__fadd_rn(S.hx[mid], syg), x_e) >= negD) cnt = half; else { p = mid + 1; cnt -= half + 1; }
           }
-          if (n == 0 && p1 - p > (uint32_t)C) {
+          if (__builtin_expect(n == 0 && p1 - p > (uint32_t)C, 0)) {
             // the slot's first run may overflow the cap by itself: of a run that is sorted in d the C closest in
             // (|d|, index) are a contiguous stretch around the zero crossing.  Find the end of the window, then
             // grow the stretch from the zero crossing one hit at a time (ties go to the left: lower index), and
@@ -318,7 +318,7 @@ __device__ __forceinline__ int collect_window(const CompassArgs& a, const WarpAr
                 p1 = R;
               }
             }
-          } else if (p1 - p > (uint32_t)C) {
+          } else if (__builtin_expect(p1 - p > (uint32_t)C, 0)) {
             // a run that can overflow the cap: of the hits on the negative side only the C next to the zero
             // crossing can be among the C closest (each one further out has C closer hits of this very run in
             // front of it), so the scan starts there instead of evicting its way through the run
@@ -445,8 +445,10 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
         if (UNI) {
           const float predC = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(LU ? a.layer_z[LC] : wa.zs[j4 + LC], za)));
           const float predD = __fadd_rn(da, __fmul_rn(bs, __fsub_rn(LU ? a.layer_z[LD] : wa.zs[j4 + LD], za)));
+#pragma unroll 1
           for (int i = sub; i < nC; i += 4)
             if (fabsf(__fsub_rn(cC[i], predC)) <= a.c.seed_tol) pC |= 1u << i;
+#pragma unroll 1
           for (int i = sub; i < nD; i += 4)
             if (fabsf(__fsub_rn(cDl[i], predD)) <= a.c.seed_tol) pD |= 1u << i;
         } else {
