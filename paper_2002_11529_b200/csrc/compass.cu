@@ -108,6 +108,13 @@ __device__ __forceinline__ float rcp_approx(float x) {
   return r;
 }
 
+// n / d for the small counts of the combination index (n < 2^16, d <= 64): (n + 0.5) / d is at least 0.5 / d away from
+// an integer, far more than the error of the approximate reciprocal, so the truncation is the exact quotient -- five
+// instructions instead of the ~20 of an integer division.
+__device__ __forceinline__ uint32_t small_div(uint32_t n, uint32_t d) {
+  return (uint32_t)(((float)n + 0.5f) * rcp_approx((float)d));
+}
+
 // Per-warp working set in shared memory.  Candidate i of lane-slot s (= track-in-batch * 4 + layer) lives at
 // [s * CS + i] with CS odd: the rows (track, hit) and the 4 lanes of a seed in phase 2 read consecutive banks.
 struct WarpArea {
@@ -492,8 +499,8 @@ __device__ __forceinline__ void process_seeds(const CompassArgs& a, const WarpAr
     if (i < K) {
       const uint32_t pc = __popc(mCq);
       uint32_t selC, selD;                           // 0 = none, else 1-based ordinal of the set bit
-      if (min3) { const uint32_t r1 = r + 1, w = pc + 1; selD = r1 / w; selC = r1 - selD * w; }
-      else { selD = r / pc; selC = r - selD * pc + 1; selD += 1; }
+      if (min3) { const uint32_t r1 = r + 1, w = pc + 1; selD = small_div(r1, w); selC = r1 - selD * w; }
+      else { selD = small_div(r, pc); selC = r - selD * pc + 1; selD += 1; }
       int ci = -1, di = -1;
       if (selC) { uint32_t m = mCq; for (uint32_t t = 1; t < selC; ++t) m &= m - 1; ci = __ffs(m) - 1; }
       if (selD) { uint32_t m = mDq; for (uint32_t t = 1; t < selD; ++t) m &= m - 1; di = __ffs(m) - 1; }
