@@ -319,6 +319,7 @@ __global__ void __launch_bounds__(512, 3) ut_decode_kernel(const DecodeArgs a) {
           const uint32_t g = g_sgrp[rw >> 16];
           const uint32_t pga = s_pstart[g], pge = s_pstart[g + 1];
           float r0 = 0.f, r1 = 0.f;
+#pragma unroll 2                                     // (measured: 4 as the compiler picks 58.0 us, 2: 57.0, 1: 57.3; config 4 same at 2)
           for (uint32_t j = pga; j < pge; j += 4u) {
             const float4 v = *reinterpret_cast<const float4*>(s_xbuf + j);
             r0 += lt(v.x, x); r1 += lt(v.y, x);
