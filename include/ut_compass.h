@@ -170,6 +170,26 @@ int32_t ut_decode(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_
                   const ut_geometry* geometry, ut_hits* hits_out, uint32_t* hit_offsets_out,
                   ut_stream_t stream);
 
+/* ut_decode_static -- ut_decode for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same kernel, same arguments, same results as ut_decode; the one
+ * difference is where the kernel's scratch lives: the control words and the per-event look-back words that ut_decode
+ * keeps in hits_out->workspace sit in ONE array built into the library (a file-scope __device__ array of
+ * 32 + 8 * UT_DECODE_STATIC_MAX_EVENTS + 8 bytes rounded up to 256, about 128 KB, held by every GPU that loads the
+ * library until the process exits).  hits_out->workspace is not read and may be NULL; no ut_decode_workspace_bytes /
+ * ut_decode_workspace_init call is needed.  The call itself performs no cudaMalloc, cudaFree or other allocating
+ * routine; inputs and outputs are the caller's as for ut_decode.
+ *   - n_events > UT_DECODE_STATIC_MAX_EVENTS returns UT_ERR_LIMIT (ut_last_error() says so); nothing is launched.
+ *   - Every call on a device shares the array and finds the previous call's contents in it: the call clears the two
+ *     counters that must start at zero (stream-ordered, in front of the kernel) and keeps the epoch word, which makes
+ *     the previous call's look-back words recognisable as stale.
+ *   - Calls that OVERLAP on one GPU (two streams, two host threads, ut_decode_static inside concurrently replayed
+ *     graphs) race on that array and produce wrong offsets or hang: serialise them (one stream, or events between
+ *     streams).  ut_decode with one workspace per container has no such limit. */
+#define UT_DECODE_STATIC_MAX_EVENTS 16384
+int32_t ut_decode_static(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_t n_events,
+                         const ut_geometry* geometry, ut_hits* hits_out, uint32_t* hit_offsets_out,
+                         ut_stream_t stream);
+
 /* VELO states: straight lines x(z) = x + tx*(z - z0), same for y, SoA. */
 typedef struct {
   const float *x, *y, *tx, *ty; /* [n_velo_total] */
@@ -346,7 +366,8 @@ int32_t ut_tuning_get(ut_tuning* out);
 int32_t ut_tuning_set(const ut_tuning* in);
 
 const char* ut_version(void);
-/* Text of the last UT_ERR_CUDA on this thread ("<call>: <cuda error string>"), "" if none. */
+/* Text of the last UT_ERR_CUDA on this thread ("<call>: <cuda error string>") or of the last UT_ERR_LIMIT of
+ * ut_decode_static, "" if none. */
 const char* ut_last_error(void);
 
 #ifdef __cplusplus

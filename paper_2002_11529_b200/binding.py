@@ -21,6 +21,7 @@ if not os.path.exists(_LIBPATH):
 _lib = C.CDLL(_LIBPATH)
 
 UT_OK = 0
+UT_ERR_NULL, UT_ERR_ARG, UT_ERR_GEOMETRY, UT_ERR_CUDA, UT_ERR_LIMIT = -1, -2, -3, -4, -5
 UT_STATUS_UNKNOWN_SECTOR, UT_STATUS_DUPLICATE_SECTOR, UT_STATUS_BAD_BANK_SIZE, UT_STATUS_CAPACITY = 1, 2, 4, 8
 UT_STATUS_BAD_OFFSETS, UT_STATUS_EVENT_TOO_LARGE, UT_STATUS_BAD_HIT_ID = 16, 32, 64
 UT_MAX_CANDIDATES = 32
@@ -92,7 +93,7 @@ EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get"
            "ut_sector_offsets_stride", "compass_search_windows", "compass_tracklets_from_windows", "ut_geometry_upload", "ut_geometry_free",
            "ut_decode_workspace_bytes", "ut_decode_workspace_init", "ut_decode", "compass_config_default",
            "compass_track", "compass_consolidate", "compass_consolidate_workspace_bytes", "ut_pipeline_create", "ut_pipeline_destroy", "ut_pipeline_run_host",
-           "ut_pipeline_device_hits", "ut_host_alloc", "ut_host_free", "ut_pipeline_timeline"]
+           "ut_pipeline_device_hits", "ut_host_alloc", "ut_host_free", "ut_pipeline_timeline", "ut_decode_static"]
 
 _lib.ut_version.restype = C.c_char_p
 _lib.ut_last_error.restype = C.c_char_p
@@ -103,6 +104,7 @@ _lib.ut_geometry_upload.argtypes = [C.POINTER(ut_geometry), C.POINTER(ut_geometr
 _lib.ut_geometry_free.argtypes = [C.POINTER(ut_geometry)]
 _lib.ut_decode.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(ut_geometry), C.POINTER(ut_hits),
                            C.c_void_p, C.c_void_p]
+_lib.ut_decode_static.argtypes = _lib.ut_decode.argtypes
 _lib.compass_config_default.argtypes = [C.c_float, C.c_float, C.c_int32, C.c_int32, C.POINTER(ut_geometry),
                                         C.POINTER(compass_config)]
 _lib.compass_track.argtypes = [C.POINTER(ut_hits), C.c_void_p, C.POINTER(velo_states), C.c_void_p, C.c_int32,
@@ -331,6 +333,23 @@ def ut_decode(raw_banks: torch.Tensor, bank_offsets: torch.Tensor, n_events: int
     rc = _lib.ut_decode(raw_banks.data_ptr(), bank_offsets.data_ptr(), n_events, C.byref(geometry.c),
                         C.byref(hits_out.c), ho.data_ptr(), _stream_ptr(stream))
     _check(rc, "ut_decode")
+    return rc
+
+
+UT_DECODE_STATIC_MAX_EVENTS = 16384
+
+
+def ut_decode_static(raw_banks: torch.Tensor, bank_offsets: torch.Tensor, n_events: int, geometry: Geometry,
+                     hits_out: Hits, hit_offsets_out: torch.Tensor | None = None, stream=None) -> int:
+    """ut_decode with the kernel's scratch in the library's built-in device array (include/ut_compass.h): no device
+    allocation anywhere in the call, at most UT_DECODE_STATIC_MAX_EVENTS events, calls on one GPU must not overlap.
+    The container's own workspace is not handed over (the descriptor goes in with workspace = NULL)."""
+    ho = hits_out.hit_offsets if hit_offsets_out is None else hit_offsets_out
+    d = hits_out.descriptor()
+    d.workspace = None
+    rc = _lib.ut_decode_static(raw_banks.data_ptr(), bank_offsets.data_ptr(), n_events, C.byref(geometry.c),
+                               C.byref(d), ho.data_ptr(), _stream_ptr(stream))
+    _check(rc, "ut_decode_static")
     return rc
 
 

@@ -39,6 +39,10 @@ int32_t cuda_fail(const char* what, cudaError_t err) {
   snprintf(g_last_error, sizeof(g_last_error), "%s: %s", what, cudaGetErrorString(err));
   return UT_ERR_CUDA;
 }
+int32_t fail_with(int32_t code, const char* text) {
+  snprintf(g_last_error, sizeof(g_last_error), "%s", text);
+  return code;
+}
 
 namespace {
 constexpr int kMaxDevices = 64;

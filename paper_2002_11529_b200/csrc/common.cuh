@@ -37,6 +37,8 @@ inline GeomDev make_geom_dev(const ut_geometry* g) {
 ut_launch_info& launch_info();
 // records "<what>: <cuda error string>" for ut_last_error(); returns UT_ERR_CUDA
 int32_t cuda_fail(const char* what, cudaError_t err);
+// records `text` for ut_last_error(); returns `code`
+int32_t fail_with(int32_t code, const char* text);
 
 // Per-device facts and the dynamic shared-memory opt-in of the kernels.  cudaFuncAttributeMaxDynamicSharedMemorySize
 // is a per-DEVICE attribute: the table is keyed by the current device and filled under a mutex, so any number of

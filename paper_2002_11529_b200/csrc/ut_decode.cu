@@ -36,6 +36,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -676,4 +677,53 @@ int32_t launch_decode(const uint8_t* raw, const uint32_t* bank_offsets, int32_t 
   return UT_OK;
 }
 
+// ---- ut_decode_static: the decode kernel's workspace in a file-scope device array (include/ut_compass.h) ----------
+// Layout as ut_decode_workspace_bytes(): 8 control words, one look-back word per event, 8 spare bytes.  Zero at module
+// load, which is the state ut_decode_workspace_init() produces.  One instance per GPU that loads the library.
+constexpr size_t kStaticWorkspaceBytes = (32 + 8 * (size_t)UT_DECODE_STATIC_MAX_EVENTS + 8 + 255) / 256 * 256;
+static __device__ __align__(256) unsigned char g_static_workspace[kStaticWorkspaceBytes];
+
+// In host code `g_static_workspace` is only a handle for the runtime, never a device address: the address of this
+// device's instance comes from cudaGetSymbolAddress, asked once per device with that device current.
+static int32_t static_workspace(void** out) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static void* ptrs[kMaxDev] = {};
+  int dev = -1;
+  UTC_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) return fail_with(UT_ERR_LIMIT, "ut_decode_static: device ordinal above 63");
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptrs[dev]) {
+    void* p = nullptr;
+    UTC_CUDA(cudaGetSymbolAddress(&p, g_static_workspace));
+    if (!p) return fail_with(UT_ERR_CUDA, "ut_decode_static: cudaGetSymbolAddress returned a null address");
+    ptrs[dev] = p;
+  }
+  *out = ptrs[dev];
+  return UT_OK;
+}
+
 }  // namespace utc
+
+extern "C" int32_t ut_decode_static(const uint8_t* raw_banks, const uint32_t* bank_offsets, int32_t n_events,
+                                    const ut_geometry* geometry, ut_hits* hits_out, uint32_t* hit_offsets_out,
+                                    ut_stream_t stream) {
+  if (!hits_out) return UT_ERR_NULL;
+  if (n_events > UT_DECODE_STATIC_MAX_EVENTS) {
+    char text[160];
+    snprintf(text, sizeof(text), "ut_decode_static: n_events = %d exceeds UT_DECODE_STATIC_MAX_EVENTS = %d (use ut_decode "
+             "with a caller-owned workspace)", (int)n_events, (int)UT_DECODE_STATIC_MAX_EVENTS);
+    return utc::fail_with(UT_ERR_LIMIT, text);
+  }
+  void* ws = nullptr;
+  if (const int32_t rc = utc::static_workspace(&ws)) return rc;
+  // The array keeps what the last call left in it.  [0] ticket and [1] CTAs done must start at zero (the kernel's last
+  // CTA re-arms them, a call that was cut short would not have); [2], the epoch, is kept: it tags the look-back words,
+  // so those of earlier calls read as "not written yet".
+  if (n_events > 0) UTC_CUDA(cudaMemsetAsync(ws, 0, 8, (cudaStream_t)stream));
+  ut_hits h = *hits_out;                       // the caller's container with the built-in workspace in place of its own
+  h.workspace = ws;
+  const int32_t rc = ut_decode(raw_banks, bank_offsets, n_events, geometry, &h, hit_offsets_out, stream);
+  if (rc == UT_OK) hits_out->geom = h.geom;    // (what ut_decode records in the container)
+  return rc;
+}
