@@ -536,9 +536,11 @@ def main():
         velo_h = [velo_blk[r * Tp:r * Tp + T] for r in range(4)]
         for dst, src in zip(velo_h, (batch.velo_x, batch.velo_y, batch.velo_tx, batch.velo_ty)):
             dst.numpy()[:] = src
-        res_blk = B.host_tensor(3 * Tp, torch.int32)
-        out_h = {"hit_idx": B.host_tensor(4 * max(T, 1), torch.int32), "n_hits": res_blk[0:max(T, 1)],
-                 "qop": res_blk[Tp:Tp + max(T, 1)].view(torch.float32), "chi2": res_blk[2 * Tp:2 * Tp + max(T, 1)].view(torch.float32),
+        # ... and the track SoA is one [7][T] block (4 rows of hit_idx, n_hits, qop, chi2): one strided copy per chunk
+        T1 = max(T, 1)
+        res_blk = B.host_tensor(7 * T1, torch.int32)
+        out_h = {"hit_idx": res_blk[0:4 * T1], "n_hits": res_blk[4 * T1:5 * T1],
+                 "qop": res_blk[5 * T1:6 * T1].view(torch.float32), "chi2": res_blk[6 * T1:7 * T1].view(torch.float32),
                  "status": B.host_tensor(2, torch.int32), "n_hits_total": B.host_tensor(1, torch.int32)}
         out_h["status"].zero_()
         out_h["n_hits_total"].zero_()
@@ -576,7 +578,7 @@ def main():
         e2e["matches_device_path"] = bool(ok)
         e2e["timeline_ms_last_step"] = pipe.timeline()      # device-side events of the last step, per chunk
         pipe.destroy()
-        for t_ in [raw_h, bo_h, vo_h, velo_blk, res_blk, out_h["hit_idx"], out_h["status"], out_h["n_hits_total"]]:
+        for t_ in [raw_h, bo_h, vo_h, velo_blk, res_blk, out_h["status"], out_h["n_hits_total"]]:
             B.host_free(t_)
 
     sampler = ClockSampler(local_rank) if rank == 0 and not os.environ.get("BENCH_NO_SAMPLER") else None

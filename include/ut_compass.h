@@ -304,8 +304,13 @@ typedef struct ut_pipeline ut_pipeline;
 int32_t ut_pipeline_create(const ut_geometry* device_geometry, int32_t max_events, size_t max_raw_bytes,
                            uint64_t max_hits, uint32_t max_velo, ut_pipeline** out);
 int32_t ut_pipeline_destroy(ut_pipeline* p);
-/* All pointers HOST.  tracks_host receives hit_idx/n_hits/qop/chi2; *status_host the OR of both status
- * words; *n_hits_host the total decoded hits.  Returns after enqueueing; sync the stream to read. */
+/* All pointers HOST.  tracks_host receives hit_idx/n_hits/qop/chi2; status_host[0] the decode's status word and
+ * status_host[1] Compass's; *n_hits_host the total decoded hits.  Returns after enqueueing; sync the stream to read.
+ * Any host pointers work.  Every copy costs ~10 us of engine latency on top of its bytes, so layouts that let several
+ * arrays travel as ONE strided copy are the fast ones: the four VELO arrays evenly spaced inside one page-locked
+ * allocation (x, y, tx, ty rows of one block), and the track SoA as one [7][n_velo_total] block -- hit_idx (4 rows),
+ * then n_hits, qop, chi2 back to back (n_hits == hit_idx + 4*n_velo_total ...), which leaves by a single copy per
+ * chunk; n_hits/qop/chi2 evenly spaced but apart from hit_idx take two.  The call recognises these layouts itself. */
 int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_banks_host, size_t raw_bytes,
                              const uint32_t* bank_offsets_host, const velo_states* velo_host,
                              const uint32_t* velo_offsets_host, uint32_t n_velo_total, int32_t n_events,

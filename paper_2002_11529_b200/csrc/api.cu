@@ -460,7 +460,7 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   const size_t s_raw = up(max_raw_bytes + 16), s_bo = up(((size_t)max_events * g->n_sectors + 1) * 4),
                s_ho = up(((size_t)max_events * g->n_groups + 1) * 4), s_vo = up(((size_t)max_events + 1) * 4),
                s_st = 256, s_v = up((size_t)max_velo * 4), s_h = up((size_t)max_hits * 4 + 32),
-               s_ws = up(ut_decode_workspace_bytes(max_events, g)), s_ti = up((size_t)max_velo * 16),
+               s_ws = up(ut_decode_workspace_bytes(max_events, g)), s_ti = 4 * s_v,
                s_so = up((size_t)max_events * ut_sector_offsets_stride(g) * 2);
   const size_t total = s_raw + s_bo + s_ho + s_vo + s_st + 4 * s_v + 9 * s_h + s_ws + s_ti + 3 * s_v + s_so;
   if (cudaMalloc(&p->block, total) != cudaSuccess) { delete p; return UT_ERR_CUDA; }
@@ -477,6 +477,7 @@ int32_t ut_pipeline_create(const ut_geometry* g, int32_t max_events, size_t max_
   p->hits.workspace = take(s_ws);
   p->hits.x_by_sector = (float*)take(s_h); p->hits.idx_by_sector = (uint16_t*)take(s_h);   // (half of the slot used)
   p->hits.sector_offsets = (uint16_t*)take(s_so);
+  // the track SoA is 7 rows s_v bytes apart (4 of hit_idx, n_hits, qop, chi2): one strided copy takes a range of tracks out
   p->tracks.hit_idx = (int32_t*)take(s_ti);
   p->tracks.n_hits = (int32_t*)take(s_v); p->tracks.qop = (float*)take(s_v); p->tracks.chi2 = (float*)take(s_v);
   p->tracks.status = p->status + 4;                    // 4 words: status + the kernel's work ticket
@@ -530,6 +531,10 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   const int kChunkEvents = tuned(tuning_snapshot().pipeline_chunk_events, 333);
   int K = n_events / (kChunkEvents > 0 ? kChunkEvents : 333);
   K = K < 1 ? 1 : (K > 4 ? 4 : K);
+  // busy events (config 4: ~8000 hits each) make the call compute-bound: Compass of chunk k holds every SM while chunk
+  // k + 1 waits decoded-or-not, so what counts is an early start -- 4 chunks, the first copy-in 40 % of the bytes
+  // instead of 50 % (config 4: 2.22 -> 2.07 ms per call)
+  if (tuning_snapshot().pipeline_chunk_events < 0 && K == 3 && raw_bytes / (size_t)n_events > 6 * (size_t)ns + 2 * 4096) K = 4;
   bool ok = cudaMemsetAsync(p->status, 0, 64, s) == cudaSuccess && cudaEventRecord(p->ev_start, s) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in, p->ev_start, 0) == cudaSuccess &&
             cudaStreamWaitEvent(p->s_in2, p->ev_start, 0) == cudaSuccess &&
@@ -597,19 +602,25 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
   };
   velo_states vd = {p->vx, p->vy, p->vtx, p->vty, velo_h->z};
   const size_t dv_pitch = (size_t)((unsigned char*)p->vy - (unsigned char*)p->vx);
-  // The VELO states and their offsets (15 % of the input bytes) go in at once on a second copy-in stream, beside the first
-  // chunk's banks: Compass needs them only after the first decode.
+  // The VELO states and their offsets (15 % of the input bytes) go in at once, in FRONT of the first chunk's banks on the
+  // one copy-in stream.  On a second stream beside the banks the two copies took the link in either order from call to
+  // call: states first 0.47-0.49 ms per call on config 3 (device timeline), states last 0.52-0.54 ms, as every Compass
+  // launch waits for them.  The states of each chunk in front of that chunk's banks cost three more copies: 0.50 ms.
   {
     void* const hv[4] = {const_cast<float*>(velo_h->x), const_cast<float*>(velo_h->y), const_cast<float*>(velo_h->tx),
                          const_cast<float*>(velo_h->ty)};
-    ok = cudaMemcpyAsync(p->velo_offsets, vo_h, ((size_t)n_events + 1) * 4, cudaMemcpyHostToDevice, p->s_in2) == cudaSuccess &&
-         rows_copy(hv, pitch_of(hv[0], hv[1], hv[2], hv[3]), (unsigned char*)p->vx, dv_pitch, (size_t)n_velo * 4, 4, false, p->s_in2) &&
-         cudaEventRecord(p->ev_velo[0], p->s_in2) == cudaSuccess && cudaStreamWaitEvent(p->s_cmp, p->ev_velo[0], 0) == cudaSuccess &&
+    cudaStream_t sv = p->s_in;
+    ok = cudaMemcpyAsync(p->velo_offsets, vo_h, ((size_t)n_events + 1) * 4, cudaMemcpyHostToDevice, sv) == cudaSuccess &&
+         rows_copy(hv, pitch_of(hv[0], hv[1], hv[2], hv[3]), (unsigned char*)p->vx, dv_pitch, (size_t)n_velo * 4, 4, false, sv) &&
+         cudaEventRecord(p->ev_velo[0], sv) == cudaSuccess && cudaStreamWaitEvent(p->s_cmp, p->ev_velo[0], 0) == cudaSuccess &&
          cudaStreamWaitEvent(p->s_cmp2, p->ev_velo[0], 0) == cudaSuccess;
     if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
   }
   const ptrdiff_t ht_pitch = pitch_of(tracks_h->n_hits, tracks_h->qop, tracks_h->chi2, nullptr);
-  const size_t dt_pitch = (size_t)((unsigned char*)p->tracks.qop - (unsigned char*)p->tracks.n_hits);
+  const size_t dt_pitch = (size_t)((unsigned char*)p->tracks.qop - (unsigned char*)p->tracks.n_hits);   // all 7 device rows
+  // host track arrays that form one [7][n_velo] block (hit_idx rows, n_hits, qop, chi2 back to back) leave by ONE copy
+  const bool one_block = (const void*)tracks_h->n_hits == (const void*)(tracks_h->hit_idx + 4 * (size_t)n_velo) &&
+                         ht_pitch == (ptrdiff_t)((size_t)n_velo * 4);
   int launched = 0;
   // Chunk sizes fall linearly (K = 4: 40 / 30 / 20 / 10 % of the events).  The copy-in is the longest stage (PCIe), every
   // chunk's kernels hide behind the next chunk's copy, and what remains exposed at the end is the last chunk's decode +
@@ -638,29 +649,48 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     // Compass runs beside the decode stream, chunks alternating between two streams (each launch with its own work
     // ticket): chunk k is tracked while chunk k + 1 is decoded and chunk k + 2 streams in, and the short last chunks,
     // which cost one event's latency whatever their size, overlap each other.  Both kernels leave issue slots idle alone.
-    cudaStream_t sc = (k & 1) ? p->s_cmp2 : p->s_cmp;
-    if (cudaEventRecord(p->ev_dec[k], s) != cudaSuccess || cudaStreamWaitEvent(sc, p->ev_dec[k], 0) != cudaSuccess)
+    // The last chunk has no decode behind it: its Compass and its copy-out stay on the decode's stream (no event hops
+    // between streams in the exposed tail of the call, and the launch overlaps the decode's end like two plain calls).
+    const bool tail = k == K - 1;
+    cudaStream_t sc = tail ? s : ((k & 1) ? p->s_cmp2 : p->s_cmp);
+    cudaStream_t so = tail ? s : p->s_out;
+    if (tail && cudaStreamWaitEvent(s, p->ev_velo[0], 0) != cudaSuccess)
       return cuda_fail("ut_pipeline_run_host (events)", cudaGetLastError());
-    rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, sc, n_velo, hint, p->status + 8 + 2 * (k & 1));
+    if (cudaEventRecord(p->ev_dec[k], s) != cudaSuccess || (!tail && cudaStreamWaitEvent(sc, p->ev_dec[k], 0) != cudaSuccess))
+      return cuda_fail("ut_pipeline_run_host (events)", cudaGetLastError());
+    rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, sc, (uint32_t)(dt_pitch / 4), hint,
+                        p->status + 8 + 2 * (k & 1));
     if (rc) return rc;
     launched += launch_info().kernels_launched;
-    ok = cudaEventRecord(p->ev_done[k], sc) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess;
+    // (the hit total is final once the last chunk is decoded: it leaves while that chunk is tracked, not behind its tracks)
+    if (k == K - 1 && n_hits_h &&
+        !(cudaStreamWaitEvent(p->s_out, p->ev_dec[k], 0) == cudaSuccess && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * ng, 4)))
+      return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
+    ok = cudaEventRecord(p->ev_done[k], sc) == cudaSuccess && (tail || cudaStreamWaitEvent(p->s_out, p->ev_done[k], 0) == cudaSuccess);
     {
       void* const hi[4] = {tracks_h->hit_idx + v0, tracks_h->hit_idx + (size_t)n_velo + v0, tracks_h->hit_idx + 2 * (size_t)n_velo + v0,
                            tracks_h->hit_idx + 3 * (size_t)n_velo + v0};
       void* const hr[3] = {tracks_h->n_hits + v0, tracks_h->qop + v0, tracks_h->chi2 + v0};
-      ok = ok && rows_copy(hi, (ptrdiff_t)n_velo * 4, (unsigned char*)(p->tracks.hit_idx + v0), (size_t)n_velo * 4, (size_t)(v1 - v0) * 4, 4,
-                           true, p->s_out) &&
-           rows_copy(hr, ht_pitch, (unsigned char*)(p->tracks.n_hits + v0), dt_pitch, (size_t)(v1 - v0) * 4, 3, true, p->s_out) &&
-           cudaEventRecord(p->ev_d2h[k], p->s_out) == cudaSuccess;
+      if (one_block) {
+        void* const h7[7] = {hi[0], hi[1], hi[2], hi[3], hr[0], hr[1], hr[2]};
+        ok = ok && rows_copy(h7, (ptrdiff_t)n_velo * 4, (unsigned char*)(p->tracks.hit_idx + v0), dt_pitch, (size_t)(v1 - v0) * 4, 7,
+                             true, so);
+      } else {
+        ok = ok && rows_copy(hi, (ptrdiff_t)n_velo * 4, (unsigned char*)(p->tracks.hit_idx + v0), dt_pitch, (size_t)(v1 - v0) * 4, 4,
+                             true, so) &&
+             rows_copy(hr, ht_pitch, (unsigned char*)(p->tracks.n_hits + v0), dt_pitch, (size_t)(v1 - v0) * 4, 3, true, so);
+      }
+      ok = ok && cudaEventRecord(p->ev_d2h[k], so) == cudaSuccess;
     }
     if (!ok) return cuda_fail("ut_pipeline_run_host", cudaGetLastError());
   }
   p->last_chunks = K;
   launch_info().kernels_launched = launched;
-  if (status_h) ok = ok && d2h(status_h, p->status, 4) && d2h(status_h + 1, p->status + 4, 4);
-  if (n_hits_h) ok = ok && d2h(n_hits_h, p->hit_offsets + (size_t)n_events * ng, 4);
+  // the decode's and Compass's status words (16 bytes apart) by one strided copy, behind everything: the caller's stream
+  // joins the copy-out stream first (the last chunk's Compass ran on the caller's stream itself)
+  void* const hs[2] = {status_h, status_h + 1};
   ok = ok && cudaEventRecord(p->ev_out, p->s_out) == cudaSuccess && cudaStreamWaitEvent(s, p->ev_out, 0) == cudaSuccess;
+  if (status_h) ok = ok && rows_copy(hs, 4, (unsigned char*)p->status, 16, 4, 2, true, s);
   return ok ? UT_OK : cuda_fail("ut_pipeline_run_host (copy out)", cudaGetLastError());
 }
 

@@ -383,12 +383,13 @@ def test_host_pipeline_matches_oracle(gpu, wl, n_events, zero_copy):
     gpu.B.ut_tuning_set(None)
 
 
-@pytest.mark.parametrize("chunk", [333, 120])
-def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk):
+@pytest.mark.parametrize("chunk,one_block", [(333, False), (120, False), (333, True), (250, True)])
+def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk, one_block):
     """ut_pipeline_run_host with buffers from ut_host_alloc: the four VELO arrays are rows of one allocation and so are
     n_hits / qop / chi2, which the call moves as one strided copy each (separate torch-pinned tensors, the test above,
-    take one copy per array); 3 and 4 chunks of linearly falling size.  The result equals the oracle's, and
-    ut_pipeline_timeline reports for every chunk: banks in <= decoded <= tracked <= tracks out."""
+    take one copy per array); one_block: the whole track SoA is one [7][T] host block (hit_idx rows, n_hits, qop, chi2
+    back to back), which leaves by a single strided copy per chunk; 3 and 4 chunks of linearly falling size.  The result
+    equals the oracle's, and ut_pipeline_timeline reports for every chunk: banks in <= decoded <= tracked <= tracks out."""
     import torch
     B = gpu.B
     B.ut_tuning_set(pipeline_chunk_events=chunk)
@@ -402,10 +403,19 @@ def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk):
     velo_h = [velo_blk[r * Tp:r * Tp + T] for r in range(4)]
     for dst, src in zip(velo_h, (b.velo_x, b.velo_y, b.velo_tx, b.velo_ty)):
         dst.numpy()[:] = src
-    res = B.host_tensor(3 * Tp, torch.int32)
-    res.fill_(-7)
-    out_h = {"hit_idx": B.host_tensor(4 * T, torch.int32), "n_hits": res[0:T], "qop": res[Tp:Tp + T].view(torch.float32),
-             "chi2": res[2 * Tp:2 * Tp + T].view(torch.float32), "status": B.host_tensor(2, torch.int32),
+    if one_block:
+        Tp = T
+        res = B.host_tensor(7 * T + 64, torch.int32)                 # (+ a canary tail)
+        res.fill_(-7)
+        idx_h = res[0:4 * T]
+        res3 = res[4 * T:]
+    else:
+        res = B.host_tensor(3 * Tp, torch.int32)
+        res.fill_(-7)
+        idx_h = B.host_tensor(4 * T, torch.int32)
+        res3 = res
+    out_h = {"hit_idx": idx_h, "n_hits": res3[0:T], "qop": res3[Tp:Tp + T].view(torch.float32),
+             "chi2": res3[2 * Tp:2 * Tp + T].view(torch.float32), "status": B.host_tensor(2, torch.int32),
              "n_hits_total": B.host_tensor(1, torch.int32)}
     pipe = B.Pipeline(gpu.geom, b.n_events, int(b.raw.size) + 32, b.hit_capacity, T)
     try:
@@ -417,7 +427,10 @@ def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk):
             assert np.array_equal(out_h["n_hits"].numpy(), t_ref.n_hits)
             assert np.array_equal(out_h["chi2"].numpy().view(np.uint32), t_ref.chi2.view(np.uint32))
             assert np.array_equal(out_h["qop"].numpy().view(np.uint32), t_ref.qop.view(np.uint32))
-            assert np.all(res.numpy()[T:Tp] == -7) and np.all(res.numpy()[Tp + T:2 * Tp] == -7)   # the pads between the rows
+            if one_block:
+                assert np.all(res.numpy()[7 * T:] == -7)                                          # nothing past the block
+            else:
+                assert np.all(res.numpy()[T:Tp] == -7) and np.all(res.numpy()[Tp + T:2 * Tp] == -7)   # the pads between the rows
             tl = pipe.timeline()
             assert len(tl) == min(4, 1000 // chunk)
             for c in tl:
@@ -427,7 +440,7 @@ def test_host_pipeline_library_buffers_and_timeline(gpu, wl, chunk):
     finally:
         pipe.destroy()
         B.ut_tuning_set(None)
-        for t_ in (raw_h, bo_h, vo_h, velo_blk, res, out_h["hit_idx"], out_h["status"], out_h["n_hits_total"]):
+        for t_ in (raw_h, bo_h, vo_h, velo_blk, res, out_h["status"], out_h["n_hits_total"]) + (() if one_block else (idx_h,)):
             B.host_free(t_)
 
 
