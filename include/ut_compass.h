@@ -342,6 +342,7 @@ typedef struct {
   int32_t compass_view;             /* 1: the container's per-sector view was offered to the kernel */
   int32_t decode_hit_stage;         /* hits (padded fill order) of an event the decode CTA orders as a whole; larger events
                                        and UT_ORDER_Y containers are ordered warp per sector group */
+  int32_t compass_event_order;      /* events the Compass CTAs hand out heaviest first (0: in batch order) */
 } ut_launch_info;
 void ut_last_launch_info(ut_launch_info* out);
 

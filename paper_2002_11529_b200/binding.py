@@ -86,7 +86,7 @@ class ut_launch_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("kernels_launched", "decode_grid", "decode_block", "decode_smem_bytes", "decode_raw_stage_bytes",
                  "decode_sort_buf", "compass_grid", "compass_block", "compass_smem_bytes", "compass_hit_stage",
-                 "compass_split", "compass_view", "decode_hit_stage")]
+                 "compass_split", "compass_view", "decode_hit_stage", "compass_event_order")]
 
 
 EXPORTS = ["ut_version", "ut_last_error", "ut_last_launch_info", "ut_tuning_get", "ut_tuning_set",

@@ -45,6 +45,7 @@
 // global x-sorted arrays (the plain definition of the window, per-hit y test).
 // fp32 arithmetic uses __f*_rn intrinsics in the order of DESIGN.md section 3 (bit-exact, no FMA).
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 
 #include "common.cuh"
@@ -86,6 +87,7 @@ struct CompassArgs {
   uint32_t* ticket;                    // [0] next work item, [1] CTAs done (one pair per launch that may run at a time)
   uint32_t hit_stage;                  // elements of the staged (bucketed) arrays
   uint32_t trk_stage;                  // tracks of an item that can be ordered by radius (0: never)
+  uint32_t ev_stage;                   // events of a batch that can be handed out heaviest first (0: never)
   unsigned long long capacity;         // elements of the hit arrays (bulk copies never read past it)
   uint32_t bulk_ok;                    // hit arrays are 16-byte aligned: the event's x and id ranges come by TMA
   uint32_t idx_stride;                 // row stride of out_idx (0: velo_offsets[n_events])
@@ -716,6 +718,57 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
   }
 }
 
+// Event order of a batch: the events with the most VELO tracks first.
+// A batch of more events than resident CTAs ends with CTAs that find no work while others still hold a whole event
+// (config 3: 1000 events on 592 CTAs).  Handing the heavy events out first leaves the light ones for the end (events
+// sorted like this on the host: Compass 101.8 -> 97 us).  Every CTA computes the same order itself: a stable counting
+// sort of the events by track count relative to the batch mean (32 bins of 1/32 of the mean, heaviest bin first; events
+// of a bin keep their order) -- each warp owns a contiguous range of events, counts per (warp, bin), a scan, then the
+// same walk again.  Results do not depend on the order.  (Not inlined: its registers are its own, the kernel's
+// allocation is tight.)  scratch: 128 bytes per warp + n_events bytes.
+__device__ __noinline__ void order_events(const uint32_t* velo_offsets, uint32_t ne, uint32_t Tend, unsigned char* scratch,
+                                          uint16_t* perm) {
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  uint32_t* cnt = reinterpret_cast<uint32_t*>(scratch);               // [nwarps][32]
+  unsigned char* ebin = scratch + (size_t)nwarps * 128;               // [ne] bin of every event
+  const int mean = (int)max(Tend / ne, 1u);
+  for (uint32_t e = tid; e < ne; e += nt) {                           // (all loads in flight at once)
+    const uint32_t v0 = __ldg(velo_offsets + e), v1 = __ldg(velo_offsets + e + 1);
+    const int nTe = v1 >= v0 ? (int)min(v1 - v0, 0x3FFFFFu) : 0;
+    ebin[e] = (unsigned char)(31 - max(0, min(31, 16 + (nTe - mean) * 32 / mean)));
+  }
+  const uint32_t per_warp = ((ne + (uint32_t)nwarps - 1u) / (uint32_t)nwarps + 31u) & ~31u;
+  const uint32_t eb = min((uint32_t)warp * per_warp, ne), ee = min(eb + per_warp, ne);
+  cnt[warp * 32 + lane] = 0;
+  __syncthreads();
+  for (int pass = 0; pass < 2; ++pass) {
+    for (uint32_t e0 = eb; e0 < ee; e0 += 32u) {
+      const uint32_t e = e0 + (uint32_t)lane;
+      const uint32_t b = e < ee ? (uint32_t)ebin[e] : 32u;            // 32: no event in this lane
+      const uint32_t m = __match_any_sync(0xFFFFFFFFu, b);
+      if (pass == 1 && b < 32u) perm[cnt[warp * 32 + b] + __popc(m & lt_mask)] = (uint16_t)e;
+      __syncwarp();
+      if (b < 32u && (m & lt_mask) == 0u) cnt[warp * 32 + b] += __popc(m);
+      __syncwarp();
+    }
+    if (pass == 0) {
+      __syncthreads();
+      // first slot of (warp, bin): the events of the heavier bins, then those of the same bin in earlier warps
+      uint32_t col = 0, before = 0;
+      for (int w = 0; w < nwarps; ++w) {
+        const uint32_t c = cnt[w * 32 + lane];
+        if (w < warp) before += c;
+        col += c;
+      }
+      const uint32_t base = warp_incl_scan(col, lane) - col;
+      __syncthreads();                                                // every warp has read the counts
+      cnt[warp * 32 + lane] = base + before;
+      __syncwarp();
+    }
+  }
+}
+
 // One CTA works through work items (event, part) handed out by the ticket.  Geometry tables are staged once.
 // INTERVAL: the seed search of long, d-sorted partner lists by interval (worth its code only when
 // max_candidates_per_layer allows long lists; the kernel without it is the faster one for short lists).
@@ -728,6 +781,10 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t ng = a.n_groups, ns = a.n_sectors;
   const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
+  // The event order exists in the large-CTA kernels only (one CTA per SM, shared memory to spare).  The small kernels
+  // have no room for the table at 4 CTAs per SM, and the code alone costs them 1.3 % (config 3: 101.9 -> 103.2 us).
+  constexpr bool EVO = MINB == 1;
+  uint16_t* s_evperm = cvr.take<uint16_t>(EVO ? a.ev_stage : 0u);      // (first: its address is a constant)
   float4* s_gA = cvr.take<float4>(ng + 8);
   uint2* s_gB = cvr.take<uint2>(ng + 8);
   float2* s_yr = cvr.take<float2>(4 * a.rows_uniform);
@@ -793,6 +850,10 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t K = a.split;
   const uint32_t n_items = (uint32_t)a.n_events * K;
 
+  // ---- event order: the events with the most VELO tracks first (order_events above; ev_stage != 0: the launch found room
+  // for the order and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
+  if (EVO && a.ev_stage != 0u) order_events(a.velo_offsets, (uint32_t)a.n_events, Tend, s_warp_areas, s_evperm);
+
   // Launched with programmatic stream serialization the CTAs may be resident, with their tables staged, while the
   // preceding kernel of the stream (ut_decode) still runs on other SMs: everything it wrote is read after this point.
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -803,8 +864,9 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     __syncthreads();                               // tables staged / previous item fully consumed
     const uint32_t item = s_item[k & 1];
     if (item >= n_items) break;
-    const int e = (int)(item / K);
-    const uint32_t part = item - (uint32_t)e * K;
+    const uint32_t ei = item / K;
+    const uint32_t part = item - ei * K;
+    const int e = (EVO && a.ev_stage != 0u) ? (int)reinterpret_cast<const uint16_t*>(smem_raw)[ei] : (int)ei;
     const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
     const uint32_t* go = a.hit_offsets + (size_t)e * ng;
     const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
@@ -1018,13 +1080,15 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
 }
 
 static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32_t soff_stride, uint32_t hit_stage, int C,
-                                 int block, uint32_t trk_stage = 0) {
+                                 int block, uint32_t trk_stage = 0, uint32_t ev_stage = 0) {
   size_t b = align16((size_t)(ng + 8) * 16) + align16((size_t)(ng + 8) * 8) + align16((size_t)rows * 32);
   b += align16((ng + 1) * 4) + align16((size_t)soff_stride * 2);
   b += align16((size_t)(hit_stage + 8) * 4) + align16((size_t)(hit_stage + 16) * 2) + align16((size_t)trk_stage * 2);
+  b += align16((size_t)ev_stage * 2);
   b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C)),
                  align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4),   // re-bucketing scratch aliases the warp areas
-                 align16((size_t)(kBins + trk_stage) * 4)});                            // and so do the radius bins
+                 align16((size_t)(kBins + trk_stage) * 4),                              // and so do the radius bins
+                 align16((size_t)(block / 32) * 128 + ev_stage)});                      // and the scratch of the event order
   return b;
 }
 
@@ -1127,14 +1191,22 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  // room for ordering up to 2048 (else 1024, 512) tracks per item, if it costs no resident CTA
+  // room for ordering up to 2048 (else 1024, 512) tracks per item and, first, the events of the batch (large-CTA kernels,
+  // a batch of more events than SMs and at most 4096: beyond that the tail of the launch is a small part of it), if it
+  // costs no resident CTA
   a.trk_stage = 0;
-  for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
-    const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, want);
-    if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
-      a.trk_stage = want;
-      smem = with;
-      break;
+  a.ev_stage = 0;
+  const uint32_t ev_want = (block > kSmallBlock && n_events > n_sm && n_events <= 4096) ? ((uint32_t)n_events + 7u) & ~7u : 0u;
+  for (int with_ev = ev_want ? 1 : 0; with_ev >= 0 && a.trk_stage == 0; --with_ev) {
+    for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
+      const uint32_t evs = with_ev ? ev_want : 0u;
+      const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, want, evs);
+      if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
+        a.trk_stage = want;
+        a.ev_stage = evs;
+        smem = with;
+        break;
+      }
     }
   }
   const void* kernel = kKernels[block <= kSmallBlock ? 0 : 1][iv][kk];
@@ -1157,6 +1229,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   split = split >= 4 ? 4 : (split >= 2 ? 2 : 1);
   a.split = (uint32_t)split;
+  if (split != 1) a.ev_stage = 0;            // (the room stays allocated, the kernel leaves the order out)
   const int grid = std::max(1, (int)std::min<long long>((long long)n_events * split, resident));
   void* params[] = {&a};
   {
@@ -1171,6 +1244,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   ut_launch_info& li = launch_info();
   li.kernels_launched = 1; li.compass_grid = grid; li.compass_block = block; li.compass_smem_bytes = (int)smem;
   li.compass_hit_stage = (int)hit_stage; li.compass_split = split; li.compass_view = view_ok ? 1 : 0;
+  li.compass_event_order = (int)a.ev_stage;
   return UT_OK;
 }
 

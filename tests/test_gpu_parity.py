@@ -159,6 +159,29 @@ def test_config4_full_size(gpu, wl):
     assert b.n_events == 1000
     h, t = check_batch(gpu, geom, b, p)
     assert (t.cand_n > p.max_candidates_per_layer).sum() > 1000
+    assert gpu.B.last_launch_info()["compass_event_order"] >= 1000     # large-CTA kernel: events handed out heaviest first
+
+
+def test_compass_event_order_uneven_batch(gpu, wl):
+    """The large-CTA Compass kernels hand the events of a batch out by descending track count (a stable counting sort
+    every CTA computes for itself).  A batch of more events than SMs whose track counts differ wildly -- every 7th event
+    without tracks, every 5th with a quarter of its tracks, the last event empty too: every track of every event still
+    gets exactly the oracle's result."""
+    geom, b, p = wl(4, 170)
+    vo = b.velo_offsets.astype(np.int64)
+    keep = []
+    for e in range(b.n_events):
+        n = int(vo[e + 1] - vo[e])
+        k = 0 if (e % 7 == 3 or e == b.n_events - 1) else (n // 4 if e % 5 == 1 else n)
+        keep.append(np.arange(vo[e], vo[e] + k))
+    idx = np.concatenate(keep)
+    vo_new = np.concatenate([[0], np.cumsum([len(k) for k in keep])]).astype(np.uint32)
+    b2 = dataclasses.replace(b, velo_x=b.velo_x[idx], velo_y=b.velo_y[idx], velo_tx=b.velo_tx[idx], velo_ty=b.velo_ty[idx],
+                             velo_offsets=vo_new, truth_hit_id=b.truth_hit_id[idx], truth_q=b.truth_q[idx],
+                             truth_p=b.truth_p[idx])
+    check_batch(gpu, geom, b2, p)
+    li = gpu.B.last_launch_info()
+    assert li["compass_block"] > 224 and li["compass_split"] == 1 and li["compass_event_order"] >= b.n_events
 
 
 def test_config5_first_1000_events_all_settings(gpu, wl):
