@@ -138,8 +138,11 @@ __host__ __device__ inline int cand_stride(int C) { return C | 1; }
 // kernels with CC are for row-uniform geometries (UT_GEOM_ROWS_UNIFORM), whose per-sector y search they leave out
 template <int CC>
 __device__ __forceinline__ int stride_of(const WarpArea& wa) { return CC ? (CC | 1) : wa.CS; }
-__host__ __device__ inline size_t warp_area_bytes(int C) {
-  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 * 4 + kTPW * 4 * 2;
+// (zs / ws exist in the kernels that are not for layer-uniform geometries, srt in those with the interval search, tzm / tkap
+//  in those with a kick table: at 4 CTAs per SM every byte of the 7 warp areas counts)
+__host__ __device__ inline size_t warp_area_bytes(int C, bool lu, bool interval, bool kick) {
+  return (size_t)cand_stride(C) * 32 * 8 + kSeedQ * 4 + kTPW * 8 + 32 * 4 + (lu ? 0 : 32 * 4 * 2) + (interval ? 32 * 4 : 0) +
+         (kick ? kTPW * 4 * 2 : 0);
 }
 
 // Sorted insert by hit index with the cap rule of step 3: keep the C smallest in (|d|, h).
@@ -781,10 +784,6 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t ng = a.n_groups, ns = a.n_sectors;
   const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
-  // The event order exists in the large-CTA kernels only (one CTA per SM, shared memory to spare).  The small kernels
-  // have no room for the table at 4 CTAs per SM, and the code alone costs them 1.3 % (config 3: 101.9 -> 103.2 us).
-  constexpr bool EVO = MINB == 1;
-  uint16_t* s_evperm = cvr.take<uint16_t>(EVO ? a.ev_stage : 0u);      // (first: its address is a constant)
   float4* s_gA = cvr.take<float4>(ng + 8);
   uint2* s_gB = cvr.take<uint2>(ng + 8);
   float2* s_yr = cvr.take<float2>(4 * a.rows_uniform);
@@ -793,6 +792,12 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   float* s_hx = cvr.take<float>(a.hit_stage + 8);
   uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage + 16);
   uint16_t* s_perm = cvr.take<uint16_t>(a.trk_stage);
+  // The event order exists in the large-CTA kernels only.  In the small ones (72 registers, 4 CTAs per SM) the code
+  // alone, wherever it is placed and inlined or not, makes the compiler spill more in the track loop (24 -> 56 bytes of
+  // stack): config 3 Compass alone 101.9 -> 104.2 us with the order off, 105.9 us with it on (its prologue is exposed),
+  // although the two calls back to back gain from it (152.6 -> 150.8 us): not worth a slower kernel.
+  constexpr bool EVO = MINB == 1;
+  uint16_t* s_evperm = cvr.take<uint16_t>(EVO ? a.ev_stage : 0u);       // event of every ticket (read by thread 0 only)
   unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by the scratch below
   // scratch while no warp is in the track loop: radius bins + per-track (bin, position); re-bucketing counters and
   // the event's id and x ranges (two bulk copies) when the container carries no per-sector view
@@ -807,6 +812,11 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   uint32_t bar_phase = 0;
   if (tid == 0) { mbar_init(&s_bar, 1); fence_mbar_init(); }
   const uint32_t lt_mask = (1u << lane) - 1u;
+
+  // ---- event order: the events with the most VELO tracks first (order_events above; ev_stage != 0: the launch found room
+  // for the order and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
+  if (EVO && a.ev_stage != 0u)
+    order_events(a.velo_offsets, (uint32_t)a.n_events, __ldg(a.velo_offsets + a.n_events), s_warp_areas, s_evperm);
 
   // ---- geometry tables, once per CTA ---------------------------------------------------------------------
   for (uint32_t g = tid; g < ng; g += nt) {
@@ -831,7 +841,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   WarpArea wa;
   {
     const int CS = cand_stride(C);
-    unsigned char* p = s_warp_areas + (size_t)warp * warp_area_bytes(C);
+    unsigned char* p = s_warp_areas + (size_t)warp * warp_area_bytes(C, LU, INTERVAL, KICK);
     wa.CS = CS;
     wa.cd = reinterpret_cast<float*>(p);
     wa.chs = reinterpret_cast<uint32_t*>(p + (size_t)CS * 32 * 4);
@@ -839,10 +849,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     wa.best = reinterpret_cast<unsigned long long*>(p);
     wa.seedq = reinterpret_cast<uint32_t*>(p + kTPW * 8);
     wa.n = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4);
-    wa.zs = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 4);
-    wa.ws = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 8);
-    wa.srt = reinterpret_cast<int*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 12);
-    wa.tzm = reinterpret_cast<float*>(p + kTPW * 8 + kSeedQ * 4 + 32 * 16);
+    p += kTPW * 8 + kSeedQ * 4 + 32 * 4;
+    wa.zs = reinterpret_cast<float*>(p);               // (arrays a kernel variant does not use take no room: their
+    wa.ws = reinterpret_cast<float*>(p + 32 * 4);      //  pointers are never dereferenced there)
+    if (!LU) p += 32 * 8;
+    wa.srt = reinterpret_cast<int*>(p);
+    if (INTERVAL) p += 32 * 4;
+    wa.tzm = reinterpret_cast<float*>(p);
     wa.tkap = wa.tzm + kTPW;
   }
   const uint32_t Tend = __ldg(a.velo_offsets + a.n_events);
@@ -850,23 +863,21 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t K = a.split;
   const uint32_t n_items = (uint32_t)a.n_events * K;
 
-  // ---- event order: the events with the most VELO tracks first (order_events above; ev_stage != 0: the launch found room
-  // for the order and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
-  if (EVO && a.ev_stage != 0u) order_events(a.velo_offsets, (uint32_t)a.n_events, Tend, s_warp_areas, s_evperm);
-
   // Launched with programmatic stream serialization the CTAs may be resident, with their tables staged, while the
   // preceding kernel of the stream (ut_decode) still runs on other SMs: everything it wrote is read after this point.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   __shared__ uint32_t s_item[2];                   // double-buffered: a slow thread still reads the previous ticket
   for (int k = 0;; ++k) {
     // work items are dealt out dynamically: CTAs that finish early take more
-    if (tid == 0) s_item[k & 1] = atomicAdd(a.ticket, 1u);
-    __syncthreads();                               // tables staged / previous item fully consumed
+    if (tid == 0) {                                // (ev_stage != 0: K == 1, the item is the event the order gives the ticket)
+      const uint32_t t = atomicAdd(a.ticket, 1u);
+      s_item[k & 1] = (EVO && a.ev_stage != 0u && t < n_items) ? (uint32_t)s_evperm[t] : t;
+    }
+    __syncthreads();                               // tables staged, event order written / previous item fully consumed
     const uint32_t item = s_item[k & 1];
     if (item >= n_items) break;
-    const uint32_t ei = item / K;
-    const uint32_t part = item - ei * K;
-    const int e = (EVO && a.ev_stage != 0u) ? (int)reinterpret_cast<const uint16_t*>(smem_raw)[ei] : (int)ei;
+    const int e = (int)(item / K);
+    const uint32_t part = item - (uint32_t)e * K;
     const uint32_t t0 = __ldg(a.velo_offsets + e), t1 = __ldg(a.velo_offsets + e + 1);
     const uint32_t* go = a.hit_offsets + (size_t)e * ng;
     const uint32_t h0 = __ldg(go), h1 = __ldg(go + ng);
@@ -1080,12 +1091,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
 }
 
 static size_t compass_smem_bytes(uint32_t ns, uint32_t ng, uint32_t rows, uint32_t soff_stride, uint32_t hit_stage, int C,
-                                 int block, uint32_t trk_stage = 0, uint32_t ev_stage = 0) {
+                                 int block, int variant, uint32_t trk_stage = 0, uint32_t ev_stage = 0) {
+  const bool lu = (variant & 3) == 1, kick = (variant & 3) == 2, interval = (variant & 4) != 0;   // kk | iv << 2
   size_t b = align16((size_t)(ng + 8) * 16) + align16((size_t)(ng + 8) * 8) + align16((size_t)rows * 32);
   b += align16((ng + 1) * 4) + align16((size_t)soff_stride * 2);
   b += align16((size_t)(hit_stage + 8) * 4) + align16((size_t)(hit_stage + 16) * 2) + align16((size_t)trk_stage * 2);
   b += align16((size_t)ev_stage * 2);
-  b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C)),
+  b += std::max({align16((size_t)(block / 32) * warp_area_bytes(C, lu, interval, kick)),
                  align16((size_t)ns * 8) + 2 * align16((size_t)(hit_stage + 8) * 4),   // re-bucketing scratch aliases the warp areas
                  align16((size_t)(kBins + trk_stage) * 4),                              // and so do the radius bins
                  align16((size_t)(block / 32) * 128 + ev_stage)});                      // and the scratch of the event order
@@ -1170,7 +1182,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= kLargeBlock; b += 32) {
-      const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b) + 1024;
+      const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b, kk | iv << 2) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
@@ -1180,14 +1192,14 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
     if (block <= 0) block = 192;
   }
   block = std::max(32, std::min(kLargeBlock, (block / 32) * 32));
-  size_t smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
+  size_t smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, kk | iv << 2);
   while (smem > budget && block > 64) {             // fewer warps before giving up staging
     block -= 32;
-    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, kk | iv << 2);
   }
   while (smem > budget && hit_stage > 0) {
     hit_stage = hit_stage > 1024 ? hit_stage - 1024 : 0;
-    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block);
+    smem = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, kk | iv << 2);
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
@@ -1200,7 +1212,7 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   for (int with_ev = ev_want ? 1 : 0; with_ev >= 0 && a.trk_stage == 0; --with_ev) {
     for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
       const uint32_t evs = with_ev ? ev_want : 0u;
-      const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, want, evs);
+      const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, kk | iv << 2, want, evs);
       if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
         a.trk_stage = want;
         a.ev_stage = evs;
