@@ -1179,10 +1179,18 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   // Block size: the one that keeps the most warps resident per SM (shared memory is the limit; about 24
   // warps per SM is what the register budget of the small variant allows).
   int block = tuned(tune.compass_block, 0);
+  // the event order (large-CTA kernels): a batch of more events than SMs and at most 4096 -- beyond that the tail of the
+  // launch is a small part of it
+  const uint32_t ev_fit = (n_events > n_sm && n_events <= 4096) ? ((uint32_t)n_events + 7u) & ~7u : 0u;
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= kLargeBlock; b += 32) {
-      const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b, kk | iv << 2) + 1024;
+      // (with room for the radius order of 512 tracks per item and, in the large kernels, for the event order: a block size
+      //  that squeezes them out loses more than its extra warp wins -- config 4, 608 threads without the event order against
+      //  576 with it: 1.300 against 1.306 ms for the 1000 events at once, but 2.31 against 2.07 ms through the host pipeline,
+      //  whose chunks of 100-400 events are 1-3 waves of 148 CTAs)
+      const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b, kk | iv << 2, 512,
+                                           b > kSmallBlock ? ev_fit : 0u) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
@@ -1203,12 +1211,11 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  // room for ordering up to 2048 (else 1024, 512) tracks per item and, first, the events of the batch (large-CTA kernels,
-  // a batch of more events than SMs and at most 4096: beyond that the tail of the launch is a small part of it), if it
-  // costs no resident CTA
+  // room for ordering up to 2048 (else 1024, 512) tracks per item and, first, the events of the batch (large-CTA kernels),
+  // if it costs no resident CTA
   a.trk_stage = 0;
   a.ev_stage = 0;
-  const uint32_t ev_want = (block > kSmallBlock && n_events > n_sm && n_events <= 4096) ? ((uint32_t)n_events + 7u) & ~7u : 0u;
+  const uint32_t ev_want = block > kSmallBlock ? ev_fit : 0u;
   for (int with_ev = ev_want ? 1 : 0; with_ev >= 0 && a.trk_stage == 0; --with_ev) {
     for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
       const uint32_t evs = with_ev ? ev_want : 0u;
