@@ -349,7 +349,7 @@ void ut_last_launch_info(ut_launch_info* out);
 /* Launch tuning, process-wide (HOST).  -1 = automatic.  The values are read ONCE from the environment when the
  * library is first used (UT_DECODE_BLOCK, UT_DECODE_RAW_STAGE, UT_DECODE_SORT_BUF, UT_DECODE_MAX_CTAS_PER_SM,
  * UT_COMPASS_BLOCK, UT_COMPASS_HIT_STAGE, UT_COMPASS_TRK_STAGE, UT_COMPASS_SPLIT, UT_COMPASS_INTERVAL_MIN,
- * UT_PIPELINE_CHUNK_EVENTS, UT_PIPELINE_ZERO_COPY, UT_DECODE_HIT_STAGE); the
+ * UT_PIPELINE_CHUNK_EVENTS, UT_PIPELINE_ZERO_COPY, UT_DECODE_HIT_STAGE, UT_COMPASS_EVENT_ORDER); the
  * hot-path calls never touch the environment.  ut_tuning_set replaces them (NULL: back to the environment's).
  * Results never depend on these values, only launch shapes and which of the equivalent code paths run. */
 typedef struct {
@@ -366,7 +366,9 @@ typedef struct {
   int32_t pipeline_zero_copy;       /* ut_pipeline_run_host: 0 = always stage the raw banks with copies; else the decode
                                        reads mapped pinned host buffers directly over PCIe */
   int32_t decode_hit_stage;         /* largest event (hits) a decode CTA orders as a whole; 0: always warp per sector group */
-  int32_t reserved[4];
+  int32_t compass_event_order;      /* 0: Compass hands the events of a batch out in batch order; else (default) by descending
+                                       track count when the batch is 149-4096 events and shared memory has room for the table */
+  int32_t reserved[3];
 } ut_tuning;
 int32_t ut_tuning_get(ut_tuning* out);
 int32_t ut_tuning_set(const ut_tuning* in);

@@ -78,8 +78,8 @@ class ut_tuning(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("decode_block", "decode_raw_stage_bytes", "decode_sort_buf", "decode_max_ctas_per_sm", "compass_block",
                  "compass_hit_stage", "compass_trk_stage", "compass_split", "pipeline_chunk_events",
-                 "compass_interval_min", "pipeline_zero_copy", "decode_hit_stage")] + \
-               [("reserved", C.c_int32 * 4)]
+                 "compass_interval_min", "pipeline_zero_copy", "decode_hit_stage", "compass_event_order")] + \
+               [("reserved", C.c_int32 * 3)]
 
 
 class ut_launch_info(C.Structure):

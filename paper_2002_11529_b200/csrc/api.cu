@@ -64,7 +64,7 @@ int env_int(const char* name) {
   return v && *v ? atoi(v) : -1;
 }
 void tuning_from_env(ut_tuning* t) {
-  for (int32_t* p = &t->decode_block; p <= &t->reserved[3]; ++p) *p = -1;
+  for (int32_t* p = &t->decode_block; p <= &t->reserved[2]; ++p) *p = -1;
   t->decode_block = env_int("UT_DECODE_BLOCK");
   t->decode_raw_stage_bytes = env_int("UT_DECODE_RAW_STAGE");
   t->decode_sort_buf = env_int("UT_DECODE_SORT_BUF");
@@ -77,6 +77,7 @@ void tuning_from_env(ut_tuning* t) {
   t->compass_interval_min = env_int("UT_COMPASS_INTERVAL_MIN");
   t->pipeline_zero_copy = env_int("UT_PIPELINE_ZERO_COPY");
   t->decode_hit_stage = env_int("UT_DECODE_HIT_STAGE");
+  t->compass_event_order = env_int("UT_COMPASS_EVENT_ORDER");
 }
 }  // namespace
 

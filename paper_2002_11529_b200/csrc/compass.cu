@@ -721,16 +721,48 @@ __device__ __forceinline__ void track_loop(const CompassArgs& a, const WarpArea&
   }
 }
 
+// Geometry tables of a CTA, staged once.  (Not inlined, and its arguments are scalars: the kernel's register allocation
+// is tight, and a call with the parameter struct by reference would copy the struct to local memory.)
+__device__ __noinline__ void stage_tables(const uint32_t* group_first_sector, const float* sec_ye, const float* sec_yb,
+                                          const float* sec_dxdy, const float* group_xmin, const float* group_xmax, uint32_t gpl,
+                                          uint32_t rows_uniform, float y_tol, uint32_t ng, float4* s_gA, uint2* s_gB,
+                                          float2* s_yr, float2* s_lay) {
+  const int tid = threadIdx.x, nt = blockDim.x;
+  for (uint32_t g = tid; g < ng; g += nt) {
+    const uint32_t sa = __ldg(group_first_sector + g), sb = __ldg(group_first_sector + g + 1);
+    const float y0 = __fadd_rn(__ldg(sec_ye + sa), y_tol), y1 = __fadd_rn(__ldg(sec_ye + sb - 1), y_tol);
+    const float inv = (sb - sa > 1 && y1 > y0) ? (float)(sb - sa - 1) / (y1 - y0) : 0.f;
+    const uint32_t gp = g + 2 * (g / gpl);
+    s_gA[gp] = make_float4(__ldg(group_xmin + g), __ldg(group_xmax + g), __ldg(sec_dxdy + sa), y0);
+    s_gB[gp] = make_uint2(__float_as_uint(inv), sa | (sb << 16));
+  }
+  for (uint32_t i = tid; i < 4 * rows_uniform; i += nt) {       // y rows of a layer = those of its first group
+    const uint32_t s = __ldg(group_first_sector + (i / rows_uniform) * gpl) + i % rows_uniform;
+    s_yr[i] = make_float2(__fsub_rn(__ldg(sec_yb + s), y_tol), __fadd_rn(__ldg(sec_ye + s), y_tol));
+  }
+  if (tid < 4) {
+    const uint32_t ga = tid * gpl, gb = ga + gpl;
+    const float x0 = __ldg(group_xmax + ga), x1 = __ldg(group_xmax + gb - 1);
+    s_lay[tid] = make_float2(x0, (gpl > 1 && x1 > x0) ? (float)(gpl - 1) / (x1 - x0) : 0.f);
+  }
+}
+
 // Event order of a batch: the events with the most VELO tracks first.
 // A batch of more events than resident CTAs ends with CTAs that find no work while others still hold a whole event
 // (config 3: 1000 events on 592 CTAs).  Handing the heavy events out first leaves the light ones for the end (events
 // sorted like this on the host: Compass 101.8 -> 97 us).  Every CTA computes the same order itself: a stable counting
 // sort of the events by track count relative to the batch mean (32 bins of 1/32 of the mean, heaviest bin first; events
 // of a bin keep their order) -- each warp owns a contiguous range of events, counts per (warp, bin), a scan, then the
-// same walk again.  Results do not depend on the order.  (Not inlined: its registers are its own, the kernel's
-// allocation is tight.)  scratch: 128 bytes per warp + n_events bytes.
+// same walk again.  Results do not depend on the order.  perm == nullptr: no order for this launch.
+// The small kernels (72 registers at 4 CTAs per SM) pay for the code: however it is placed, inlined or not, the track
+// loop spills a little more (24 -> 40 bytes of stack in this form, called unconditionally; 56-88 in the others tried).
+// Config 3: Compass timed alone 102.0 -> 105.1 us (103.4 with the order off: the order's own prologue, two round trips
+// to the VELO offsets, is exposed there), but the two calls back to back 152.6 -> 149.3 us -- behind ut_decode the
+// prologue runs while the decode's last CTAs finish, and the shorter tail is what remains.
+// scratch: 128 bytes per warp + n_events bytes.
 __device__ __noinline__ void order_events(const uint32_t* velo_offsets, uint32_t ne, uint32_t Tend, unsigned char* scratch,
                                           uint16_t* perm) {
+  if (perm == nullptr) return;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
   uint32_t* cnt = reinterpret_cast<uint32_t*>(scratch);               // [nwarps][32]
@@ -784,6 +816,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t ng = a.n_groups, ns = a.n_sectors;
   const int C = a.c.max_candidates_per_layer;
   Carver cvr(smem_raw);
+  cvr.take<uint16_t>(a.ev_stage);       // event of every ticket (thread 0 reads it), at offset 0 of the dynamic array
   float4* s_gA = cvr.take<float4>(ng + 8);
   uint2* s_gB = cvr.take<uint2>(ng + 8);
   float2* s_yr = cvr.take<float2>(4 * a.rows_uniform);
@@ -792,12 +825,6 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   float* s_hx = cvr.take<float>(a.hit_stage + 8);
   uint16_t* s_hh = cvr.take<uint16_t>(a.hit_stage + 16);
   uint16_t* s_perm = cvr.take<uint16_t>(a.trk_stage);
-  // The event order exists in the large-CTA kernels only.  In the small ones (72 registers, 4 CTAs per SM) the code
-  // alone, wherever it is placed and inlined or not, makes the compiler spill more in the track loop (24 -> 56 bytes of
-  // stack): config 3 Compass alone 101.9 -> 104.2 us with the order off, 105.9 us with it on (its prologue is exposed),
-  // although the two calls back to back gain from it (152.6 -> 150.8 us): not worth a slower kernel.
-  constexpr bool EVO = MINB == 1;
-  uint16_t* s_evperm = cvr.take<uint16_t>(EVO ? a.ev_stage : 0u);       // event of every ticket (read by thread 0 only)
   unsigned char* s_warp_areas = cvr.take<unsigned char>(1);  // nwarps x warp_area_bytes(C); aliased by the scratch below
   // scratch while no warp is in the track loop: radius bins + per-track (bin, position); re-bucketing counters and
   // the event's id and x ranges (two bulk copies) when the container carries no per-sector view
@@ -814,28 +841,13 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
   const uint32_t lt_mask = (1u << lane) - 1u;
 
   // ---- event order: the events with the most VELO tracks first (order_events above; ev_stage != 0: the launch found room
-  // for the order and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
-  if (EVO && a.ev_stage != 0u)
-    order_events(a.velo_offsets, (uint32_t)a.n_events, __ldg(a.velo_offsets + a.n_events), s_warp_areas, s_evperm);
+  // for the table and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
+  order_events(a.velo_offsets, (uint32_t)a.n_events, __ldg(a.velo_offsets + a.n_events), s_warp_areas,
+               a.ev_stage != 0u ? reinterpret_cast<uint16_t*>(smem_raw) : nullptr);
+  // ---- geometry tables, once per CTA
 
-  // ---- geometry tables, once per CTA ---------------------------------------------------------------------
-  for (uint32_t g = tid; g < ng; g += nt) {
-    const uint32_t sa = __ldg(a.group_first_sector + g), sb = __ldg(a.group_first_sector + g + 1);
-    const float y0 = __fadd_rn(__ldg(a.sec_ye + sa), a.c.y_tol), y1 = __fadd_rn(__ldg(a.sec_ye + sb - 1), a.c.y_tol);
-    const float inv = (sb - sa > 1 && y1 > y0) ? (float)(sb - sa - 1) / (y1 - y0) : 0.f;
-    const uint32_t gp = g + 2 * (g / a.gpl);
-    s_gA[gp] = make_float4(__ldg(a.group_xmin + g), __ldg(a.group_xmax + g), __ldg(a.sec_dxdy + sa), y0);
-    s_gB[gp] = make_uint2(__float_as_uint(inv), sa | (sb << 16));
-  }
-  for (uint32_t i = tid; i < 4 * a.rows_uniform; i += nt) {     // y rows of a layer = those of its first group
-    const uint32_t s = __ldg(a.group_first_sector + (i / a.rows_uniform) * a.gpl) + i % a.rows_uniform;
-    s_yr[i] = make_float2(__fsub_rn(__ldg(a.sec_yb + s), a.c.y_tol), __fadd_rn(__ldg(a.sec_ye + s), a.c.y_tol));
-  }
-  if (tid < 4) {
-    const uint32_t ga = tid * a.gpl, gb = ga + a.gpl;
-    const float x0 = __ldg(a.group_xmax + ga), x1 = __ldg(a.group_xmax + gb - 1);
-    s_lay[tid] = make_float2(x0, (a.gpl > 1 && x1 > x0) ? (float)(a.gpl - 1) / (x1 - x0) : 0.f);
-  }
+  stage_tables(a.group_first_sector, a.sec_ye, a.sec_yb, a.sec_dxdy, a.group_xmin, a.group_xmax, a.gpl, a.rows_uniform,
+               a.c.y_tol, ng, s_gA, s_gB, s_yr, s_lay);
   SmemView S;
   S.gA = s_gA; S.gB = s_gB; S.yr = s_yr; S.lay = s_lay; S.goff = s_goff; S.off = s_off; S.hx = s_hx; S.hh = s_hh;
   WarpArea wa;
@@ -871,7 +883,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
     // work items are dealt out dynamically: CTAs that finish early take more
     if (tid == 0) {                                // (ev_stage != 0: K == 1, the item is the event the order gives the ticket)
       const uint32_t t = atomicAdd(a.ticket, 1u);
-      s_item[k & 1] = (EVO && a.ev_stage != 0u && t < n_items) ? (uint32_t)s_evperm[t] : t;
+      s_item[k & 1] = (a.ev_stage != 0u && t < n_items) ? (uint32_t)reinterpret_cast<const uint16_t*>(smem_raw)[t] : t;
     }
     __syncthreads();                               // tables staged, event order written / previous item fully consumed
     const uint32_t item = s_item[k & 1];
@@ -1179,18 +1191,18 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   // Block size: the one that keeps the most warps resident per SM (shared memory is the limit; about 24
   // warps per SM is what the register budget of the small variant allows).
   int block = tuned(tune.compass_block, 0);
-  // the event order (large-CTA kernels): a batch of more events than SMs and at most 4096 -- beyond that the tail of the
-  // launch is a small part of it
-  const uint32_t ev_fit = (n_events > n_sm && n_events <= 4096) ? ((uint32_t)n_events + 7u) & ~7u : 0u;
+  // the event order: a batch of more events than SMs and at most 4096 -- beyond that the tail of the launch is a small
+  // part of it
+  const uint32_t ev_fit = (n_events > n_sm && n_events <= 4096 && tune.compass_event_order != 0) ? ((uint32_t)n_events + 7u) & ~7u : 0u;
   if (block <= 0) {
     int best_warps = -1;
     for (int b = 192; b <= kLargeBlock; b += 32) {
-      // (with room for the radius order of 512 tracks per item and, in the large kernels, for the event order: a block size
+      // (with room for the radius order of 512 tracks per item and for the event order: a block size
       //  that squeezes them out loses more than its extra warp wins -- config 4, 608 threads without the event order against
       //  576 with it: 1.300 against 1.306 ms for the 1000 events at once, but 2.31 against 2.07 ms through the host pipeline,
       //  whose chunks of 100-400 events are 1-3 waves of 148 CTAs)
       const size_t sm = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, b, kk | iv << 2, 512,
-                                           b > kSmallBlock ? ev_fit : 0u) + 1024;
+                                           ev_fit) + 1024;
       if (sm > budget) continue;
       const int regs_warps = b <= kSmallBlock ? 28 : 21;       // 72 registers per thread: 4 CTAs of up to 7 warps
       const int ctas = std::min<int>((int)((size_t)sm_smem / sm), std::max(1, regs_warps / (b / 32)));
@@ -1211,14 +1223,15 @@ int32_t launch_compass(const ut_hits* hits, const uint32_t* hit_offsets, const v
   }
   if (smem > budget) return UT_ERR_LIMIT;
   a.hit_stage = hit_stage;
-  // room for ordering up to 2048 (else 1024, 512) tracks per item and, first, the events of the batch (large-CTA kernels),
-  // if it costs no resident CTA
+  // room for ordering up to 2048 (else 1024, 512) tracks per item and, first, the events of the batch, if it costs no
+  // resident CTA
   a.trk_stage = 0;
   a.ev_stage = 0;
-  const uint32_t ev_want = block > kSmallBlock ? ev_fit : 0u;
-  for (int with_ev = ev_want ? 1 : 0; with_ev >= 0 && a.trk_stage == 0; --with_ev) {
+  // (the order only matters when the batch is more than one wave of CTAs: 4 small CTAs per SM at best, one large one)
+  const bool ev_useful = ev_fit != 0u && n_events > n_sm * (block <= kSmallBlock ? 4 : 1);
+  for (int with_ev = ev_useful ? 1 : 0; with_ev >= 0 && a.trk_stage == 0; --with_ev) {
     for (uint32_t want = (uint32_t)tuned(tune.compass_trk_stage, 2048); want >= 512; want /= 2) {
-      const uint32_t evs = with_ev ? ev_want : 0u;
+      const uint32_t evs = with_ev ? ev_fit : 0u;
       const size_t with = compass_smem_bytes(ns, ng, a.rows_uniform, a.soff_stride, hit_stage, C, block, kk | iv << 2, want, evs);
       if (with <= budget && (size_t)sm_smem / (with + 1024) == (size_t)sm_smem / (smem + 1024)) {
         a.trk_stage = want;

@@ -151,6 +151,13 @@ def test_config3_full_size_bench_launch(gpu, wl):
     check_batch(gpu, geom, b, p)
     li = gpu.B.last_launch_info()
     assert li["kernels_launched"] == 1 and li["compass_grid"] >= 148
+    assert li["compass_event_order"] >= 1000          # the events were handed out by descending track count ...
+    gpu.B.ut_tuning_set(compass_event_order=0)       # ... and in batch order: the same tracks either way
+    try:
+        check_batch(gpu, geom, b, p)
+        assert gpu.B.last_launch_info()["compass_event_order"] == 0
+    finally:
+        gpu.B.ut_tuning_set(None)
 
 
 def test_config4_full_size(gpu, wl):
@@ -162,8 +169,8 @@ def test_config4_full_size(gpu, wl):
 
 
 def test_compass_event_order_uneven_batch(gpu, wl):
-    """The large-CTA Compass kernels hand the events of a batch out by descending track count (a stable counting sort
-    every CTA computes for itself).  A batch of more events than SMs whose track counts differ wildly -- every 7th event
+    """The Compass kernels hand the events of a batch out by descending track count (a stable counting sort every CTA
+    computes for itself), here the large-CTA kernel.  A batch of more events than SMs whose track counts differ wildly -- every 7th event
     without tracks, every 5th with a quarter of its tracks, the last event empty too: every track of every event still
     gets exactly the oracle's result."""
     geom, b, p = wl(4, 170)
