@@ -760,18 +760,29 @@ __device__ __noinline__ void stage_tables(const uint32_t* group_first_sector, co
 // to the VELO offsets, is exposed there), but the two calls back to back 152.6 -> 149.3 us -- behind ut_decode the
 // prologue runs while the decode's last CTAs finish, and the shorter tail is what remains.
 // scratch: 128 bytes per warp + n_events bytes.
-__device__ __noinline__ void order_events(const uint32_t* velo_offsets, uint32_t ne, uint32_t Tend, unsigned char* scratch,
-                                          uint16_t* perm) {
+__device__ __noinline__ void order_events(const uint32_t* velo_offsets, uint32_t ne, unsigned char* scratch, uint16_t* perm) {
   if (perm == nullptr) return;
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
   uint32_t* cnt = reinterpret_cast<uint32_t*>(scratch);               // [nwarps][32]
   unsigned char* ebin = scratch + (size_t)nwarps * 128;               // [ne] bin of every event
-  const int mean = (int)max(Tend / ne, 1u);
-  for (uint32_t e = tid; e < ne; e += nt) {                           // (all loads in flight at once)
-    const uint32_t v0 = __ldg(velo_offsets + e), v1 = __ldg(velo_offsets + e + 1);
-    const int nTe = v1 >= v0 ? (int)min(v1 - v0, 0x3FFFFFu) : 0;
-    ebin[e] = (unsigned char)(31 - max(0, min(31, 16 + (nTe - mean) * 32 / mean)));
+  // (4 events per thread and round, their loads and the one of the total in flight together: one round trip to the
+  //  offsets for a batch of up to 4 x blockDim events)
+  for (uint32_t e0 = tid; e0 < ne; e0 += 4u * (uint32_t)nt) {
+    uint32_t v0[4], v1[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint32_t e = e0 + (uint32_t)q * (uint32_t)nt;
+      v0[q] = v1[q] = 0u;
+      if (e < ne) { v0[q] = __ldg(velo_offsets + e); v1[q] = __ldg(velo_offsets + e + 1); }
+    }
+    const int mean = (int)max(__ldg(velo_offsets + ne) / ne, 1u);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint32_t e = e0 + (uint32_t)q * (uint32_t)nt;
+      const int nTe = v1[q] >= v0[q] ? (int)min(v1[q] - v0[q], 0x3FFFFFu) : 0;
+      if (e < ne) ebin[e] = (unsigned char)(31 - max(0, min(31, 16 + (nTe - mean) * 32 / mean)));
+    }
   }
   const uint32_t per_warp = ((ne + (uint32_t)nwarps - 1u) / (uint32_t)nwarps + 31u) & ~31u;
   const uint32_t eb = min((uint32_t)warp * per_warp, ne), ee = min(eb + per_warp, ne);
@@ -842,7 +853,7 @@ __global__ void __launch_bounds__(MAXT, MINB) compass_kernel(const CompassArgs a
 
   // ---- event order: the events with the most VELO tracks first (order_events above; ev_stage != 0: the launch found room
   // for the table and one CTA per event, K == 1).  Only the VELO offsets are read: none of it waits for ut_decode.
-  order_events(a.velo_offsets, (uint32_t)a.n_events, __ldg(a.velo_offsets + a.n_events), s_warp_areas,
+  order_events(a.velo_offsets, (uint32_t)a.n_events, s_warp_areas,
                a.ev_stage != 0u ? reinterpret_cast<uint16_t*>(smem_raw) : nullptr);
   // ---- geometry tables, once per CTA
 
