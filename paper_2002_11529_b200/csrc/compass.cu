@@ -776,12 +776,14 @@ __device__ __noinline__ void order_events(const uint32_t* velo_offsets, uint32_t
       v0[q] = v1[q] = 0u;
       if (e < ne) { v0[q] = __ldg(velo_offsets + e); v1[q] = __ldg(velo_offsets + e + 1); }
     }
-    const int mean = (int)max(__ldg(velo_offsets + ne) / ne, 1u);
+    // bin = 16 + 32 * (tracks - mean) / mean, in fp32 (the same instructions on the same numbers in every CTA)
+    const float mean = fmaxf((float)__ldg(velo_offsets + ne) / (float)ne, 1.f), scale = 32.f / mean;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const uint32_t e = e0 + (uint32_t)q * (uint32_t)nt;
-      const int nTe = v1[q] >= v0[q] ? (int)min(v1[q] - v0[q], 0x3FFFFFu) : 0;
-      if (e < ne) ebin[e] = (unsigned char)(31 - max(0, min(31, 16 + (nTe - mean) * 32 / mean)));
+      const float nTe = v1[q] >= v0[q] ? (float)min(v1[q] - v0[q], 0x3FFFFFu) : 0.f;
+      const int b = __float2int_rd(fminf(fmaxf(__fmul_rn(__fsub_rn(nTe, mean), scale), -16.f), 15.f));     // -16 .. 15
+      if (e < ne) ebin[e] = (unsigned char)(15 - b);                                                          // heavy first
     }
   }
   const uint32_t per_warp = ((ne + (uint32_t)nwarps - 1u) / (uint32_t)nwarps + 31u) & ~31u;
