@@ -660,7 +660,7 @@ int32_t ut_pipeline_run_host(ut_pipeline* p, const uint8_t* raw_h, size_t raw_by
     if (cudaEventRecord(p->ev_dec[k], s) != cudaSuccess || (!tail && cudaStreamWaitEvent(sc, p->ev_dec[k], 0) != cudaSuccess))
       return cuda_fail("ut_pipeline_run_host (events)", cudaGetLastError());
     rc = launch_compass(&hc, ho, &vd, p->velo_offsets + e0, ne, config, &p->tracks, sc, (uint32_t)(dt_pitch / 4), hint,
-                        p->status + 8 + 2 * (k & 1));
+                        p->status + 8 + (tail ? 4 : 2 * (k & 1)));   // (a ticket pair per stream: launches that may overlap never share one)
     if (rc) return rc;
     launched += launch_info().kernels_launched;
     // (the hit total is final once the last chunk is decoded: it leaves while that chunk is tracked, not behind its tracks)
